@@ -1,0 +1,160 @@
+/*
+ * qmcd.h -- C-ABI boundary of the B200 (sm_100a) delayed rank-K Slater-inverse
+ * update library (arXiv 1708.00744).  Citations are lines of
+ * /root/reference/PAPER.md; notation as in DESIGN.md:
+ *
+ *   N   electrons = matrix order          K  delay
+ *   A   Slater matrix, row = orbital, column = electron
+ *   B   = A^-1 ("Ainv"), row-major, row j contiguous
+ *   j   moved electron (column of A, row of B)
+ *   v   the NEW column j of A;  R = det(A_new)/det(A)
+ *   m   moves currently queued for a walker, 0 <= m <= K
+ *
+ * The operation: propose a single-electron move, get its determinant ratio
+ * from the STALE inverse plus the Woodbury correction of the <= K queued
+ * accepted moves (Eq. 3), accept or reject it, and
+ * after K accepted moves rebuild the inverse in one rank-K step (Eq. 4,
+ * PAPER.md:84-89).  K = 1 is classic Sherman-Morrison (Eqs. 1-2).
+ * `batch` independent walkers are processed together.
+ *
+ * Conventions common to every call
+ *   - All `*_dev` pointers are DEVICE pointers, fp64 unless stated, owned by the
+ *     caller (e.g. torch tensors).  The library never allocates device memory.
+ *   - Every call only ENQUEUES work on the handle's CUDA stream and returns; no
+ *     call synchronises except qmcd_status, qmcd_destroy and qmcd_sweep_host.
+ *   - Return value: QMCD_OK (0) or a negative QMCD_E* code.  Argument and state
+ *     checks are host-side.  There is NO CPU fallback: without a CUDA device
+ *     qmcd_create returns QMCD_ECUDA.
+ *   - State machine per handle: IDLE --ratio--> PROPOSED --accept/reject--> IDLE.
+ *     A second ratio in PROPOSED replaces the staged proposal.
+ */
+#ifndef QMCD_H
+#define QMCD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define QMCD_OK         0
+#define QMCD_EINVAL    (-1)   /* bad argument (range, NULL, size, alignment)       */
+#define QMCD_ESTATE    (-2)   /* call not legal in the handle's current state      */
+#define QMCD_ECUDA     (-3)   /* CUDA runtime/driver error (see qmcd_strerror)     */
+#define QMCD_ESINGULAR (-4)   /* device status: accept of a move with R==0/non-finite */
+
+typedef struct qmcd_ctx* qmcd_handle;   /* opaque */
+
+/* Bytes of device workspace qmcd_create needs for (N, K, batch); 0 on bad
+ * arguments (N < 1, K < 1, K > N, batch < 1).  Holds the queue of PAPER.md:84:
+ * C (queued new columns), W (queued rows of the stale inverse), Y (scratch of
+ * Eq. 4), M = (I + V'A^-1 U)^-1 (K x K), J, m and staging. */
+size_t qmcd_workspace_bytes(int N, int K, int batch);
+
+/* Create a handle.  workspace_dev: >= qmcd_workspace_bytes bytes, 256-byte
+ * aligned, caller-owned, must outlive the handle; it is zero-filled here
+ * (enqueued).  cuda_stream: a cudaStream_t (may be NULL = default stream).
+ * Errors: QMCD_EINVAL (ranges, K > N, NULL, too small, misaligned), QMCD_ECUDA. */
+int qmcd_create(qmcd_handle* out, int N, int K, int batch,
+                void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
+
+/* Waits for the stream, releases host resources.  NULL is a no-op. */
+int qmcd_destroy(qmcd_handle h);
+
+/* Adopt the explicit inverse.  Ainv_dev: [batch][N][N] row-major
+ * fp64, 16-byte aligned, BORROWED until the next set_inverse/destroy and
+ * updated IN PLACE by every flush.  Resets every walker's queue (m = 0).
+ * Errors: QMCD_EINVAL, QMCD_ESTATE (in PROPOSED). */
+int qmcd_set_inverse(qmcd_handle h, double* Ainv_dev);
+
+/* Look-ahead determinant ratio (Eqs. 1 and 3) of
+ * moving electron j to the position whose orbital column is v, for every
+ * walker: R = d - p^T M q with d = B0[j,:].v, p_i = B0[j,:].C[i,:] - delta(j,j_i),
+ * q_a = W[a,:].v (m = 0: R = d).  v_dev: [batch][N], read during this call only
+ * (the kernel stages a copy).  R_dev: [batch], valid in stream order; signed.
+ * Errors: QMCD_EINVAL (j outside [0,N), NULL), QMCD_ESTATE (no inverse set). */
+int qmcd_ratio(qmcd_handle h, int j, const double* v_dev, double* R_dev);
+
+/* Same with a per-walker electron index j_dev: [batch] int32 on the device.
+ * An index outside [0,N) sets the sticky device status to QMCD_EINVAL. */
+int qmcd_ratio_jv(qmcd_handle h, const int* j_dev, const double* v_dev, double* R_dev);
+
+/* Accept the staged proposal for walkers whose mask byte is non-zero, drop it
+ * for the others.  mask_dev: [batch] uint8, or NULL = accept all.  An accepted
+ * move is queued: M is bordered, (j, v, B0[j,:]) appended, m++.
+ * A walker whose m reaches K is flushed here (Eq. 4).  If j is already queued
+ * for that walker the queue is flushed first (reading G7).
+ * Accepting R == 0 or non-finite sets the sticky status QMCD_ESINGULAR and the
+ * move is dropped.  Errors: QMCD_ESTATE (not PROPOSED). */
+int qmcd_accept(qmcd_handle h, const unsigned char* mask_dev);
+
+/* Metropolis accept (BASELINE.json configs[2]): walker b accepts iff
+ * uniforms_dev[b] < min(1, R_b^2), decided on the device in fp64.
+ * acc_out_dev: [batch] uint8 decisions, may be NULL. */
+int qmcd_accept_metropolis(qmcd_handle h, const double* uniforms_dev,
+                           unsigned char* acc_out_dev);
+
+/* Drop the staged proposal for every walker (== accept with an all-zero mask). */
+int qmcd_reject(qmcd_handle h);
+
+/* Apply the queue of every walker with m > 0 (Eq. 4):
+ * B <- B0 - (B0 C^T - E_J) M W, any rank 1 <= m <= K; m <- 0.  Legal in IDLE
+ * only (QMCD_ESTATE otherwise); a no-op for walkers with m == 0. */
+int qmcd_flush(qmcd_handle h);
+
+/* Copy the per-walker queue lengths to m_dev: [batch] int32 (enqueued). */
+int qmcd_pending(qmcd_handle h, int* m_dev);
+
+/* Synchronise the stream and return the sticky device status in *host_out:
+ * 0, QMCD_ESINGULAR or QMCD_EINVAL.  info_out (may be NULL): int[2] =
+ * {first offending walker, its move counter}. */
+int qmcd_status(qmcd_handle h, int* host_out, int* info_out);
+
+/* Per-walker counters since set_inverse, copied (enqueued) to
+ * counters_dev: [batch][2] int64 = {accepted moves, flushes}. */
+int qmcd_counters(qmcd_handle h, long long* counters_dev);
+
+/* Device-resident run of n_moves proposals with no host round trip (the same
+ * ratio -> accept -> flush-when-full sequence, one persistent launch; results
+ * equal the call-by-call sequence).  Move t proposes electron
+ * (j_begin + t) mod N with new column proposals_dev[t][b][:].  Exactly one of
+ * mask_dev ([n_moves][batch] uint8) / uniforms_dev ([n_moves][batch] fp64,
+ * Metropolis u < min(1,R^2)) is non-NULL.  Outputs R_out_dev [n_moves][batch]
+ * fp64 and acc_out_dev [n_moves][batch] uint8 (either may be NULL).  Ends IDLE
+ * with moves possibly still queued (no implicit final flush).
+ * Errors: QMCD_EINVAL, QMCD_ESTATE (PROPOSED or no inverse). */
+int qmcd_sweep(qmcd_handle h, int j_begin, int n_moves,
+               const double* proposals_dev, const unsigned char* mask_dev,
+               const double* uniforms_dev, double* R_out_dev,
+               unsigned char* acc_out_dev);
+
+/* Same run from HOST buffers (end-to-end path): proposals/mask/uniforms are
+ * copied host->device in chunks through staging_dev (caller-owned device
+ * scratch, >= qmcd_sweep_host_min_staging bytes; larger = bigger chunks),
+ * double-buffered against the compute, and R/acc are copied back.  Host
+ * buffers should be pinned for overlap.  SYNCHRONISES before returning. */
+int qmcd_sweep_host(qmcd_handle h, int j_begin, int n_moves,
+                    const double* proposals_host, const unsigned char* mask_host,
+                    const double* uniforms_host, double* R_out_host,
+                    unsigned char* acc_out_host,
+                    void* staging_dev, size_t staging_bytes);
+size_t qmcd_sweep_host_min_staging(int N, int batch);
+
+/* Tuning / introspection.  key: "cluster" (CTAs per walker, 1..16),
+ * "flush_path" (0 auto, 1 CUDA-core, 2 DMMA), "threads".  get returns the
+ * value (>= 0) or a negative error. */
+int qmcd_set_option(qmcd_handle h, const char* key, int value);
+int qmcd_get_option(qmcd_handle h, const char* key);
+
+/* Roofline denominators measured on this device (not part of the method):
+ * kind 0 = register-resident DFMA loop, 1 = register-resident DMMA.8x8x4 loop.
+ * Runs on the given stream, synchronises, writes TFLOP/s to *tflops_out. */
+int qmcd_probe_fp64(int kind, int iters, void* cuda_stream, double* tflops_out);
+
+const char* qmcd_strerror(int code);
+const char* qmcd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QMCD_H */

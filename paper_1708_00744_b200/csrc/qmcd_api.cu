@@ -1,0 +1,385 @@
+// qmcd_api.cu -- host side of the C-ABI declared in include/qmcd.h: argument and
+// state checks, workspace carving, launch policy.  No CPU fallback anywhere.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+#include <new>
+
+#include "../../include/qmcd.h"
+#include "qmcd_kernel.cuh"
+
+enum { QMCD_IDLE = 0, QMCD_PROPOSED = 1 };
+
+struct qmcd_ctx {
+    int N, K, batch;
+    cudaStream_t stream;
+    cudaStream_t copy_stream;
+    cudaEvent_t ev_h2d[2], ev_done[2];
+    QmcdDev P;
+    int state;
+    bool has_inverse;
+    size_t smem_bytes;
+    int max_cluster;          // largest cluster size the device can co-schedule
+    char last_cuda_error[256];
+};
+
+static thread_local char g_last_error[256] = "";
+
+static int cuda_fail(qmcd_ctx* h, cudaError_t e, const char* what) {
+    snprintf(g_last_error, sizeof(g_last_error), "%s: %s", what, cudaGetErrorString(e));
+    if (h) memcpy(h->last_cuda_error, g_last_error, sizeof(g_last_error));
+    return QMCD_ECUDA;
+}
+#define CK(h, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(h, e_, #call); } while (0)
+
+static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct WsLayout { size_t C, W, Y, M, J, m, sj, sR, sp, sc, counters, status, total; };
+
+static WsLayout ws_layout(int N, int K, int batch) {
+    WsLayout L; size_t o = 0;
+    size_t kn = (size_t)batch * K * N * 8;
+    L.C = o; o += al256(kn);
+    L.W = o; o += al256(kn);
+    L.Y = o; o += al256(kn);
+    L.M = o; o += al256((size_t)batch * K * K * 8);
+    L.J = o; o += al256((size_t)batch * K * 4);
+    L.m = o; o += al256((size_t)batch * 4);
+    L.sj = o; o += al256((size_t)batch * 4);
+    L.sR = o; o += al256((size_t)batch * 8);
+    L.sp = o; o += al256((size_t)batch * K * 8);
+    L.sc = o; o += al256((size_t)batch * K * 8);
+    L.counters = o; o += al256((size_t)batch * 2 * 8);
+    L.status = o; o += 256;
+    L.total = o;
+    return L;
+}
+
+extern "C" size_t qmcd_workspace_bytes(int N, int K, int batch) {
+    if (N < 1 || K < 1 || K > N || batch < 1) return 0;
+    return ws_layout(N, K, batch).total;
+}
+
+static int pow2_floor(int x) { int p = 1; while (p * 2 <= x) p *= 2; return p; }
+
+// Pick CTAs per walker: fill the 148 SMs with batch*S CTAs, keep slices >= 64
+// columns, stay within what the device can co-schedule.
+static int default_cluster(int N, int batch, int sms, int max_cluster) {
+    int s = pow2_floor(sms / batch > 0 ? sms / batch : 1);
+    int cap_n = pow2_floor(N / 64 > 0 ? N / 64 : 1);
+    if (s > cap_n) s = cap_n;
+    if (s > max_cluster) s = max_cluster;
+    if (s < 1) s = 1;
+    return s;
+}
+
+static int configure_kernel(qmcd_ctx* h, int S) {
+    size_t smem = qmcd_smem_base_bytes(h->N, h->K, S) + qmcd_flush_mma_smem_bytes(h->N, h->K);
+    if (smem > 227 * 1024) smem = qmcd_smem_base_bytes(h->N, h->K, S);
+    if (smem > 227 * 1024) { snprintf(g_last_error, sizeof(g_last_error), "shared memory need %zu > 227 KB", smem); return QMCD_EINVAL; }
+    // the attribute is per function, not per handle: always allow the device maximum
+    CK(h, cudaFuncSetAttribute(qmcd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    CK(h, cudaFuncSetAttribute(qmcd_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    h->smem_bytes = smem;
+    h->P.S = S;
+    return QMCD_OK;
+}
+
+static int launch(qmcd_ctx* h, const QmcdArgs& a) {
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3((unsigned)(h->batch * h->P.S), 1, 1);
+    cfg.blockDim = dim3(QMCD_THREADS, 1, 1);
+    cfg.dynamicSmemBytes = h->smem_bytes;
+    cfg.stream = h->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)h->P.S;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    CK(h, cudaLaunchKernelEx(&cfg, qmcd_kernel, a));
+    return QMCD_OK;
+}
+
+extern "C" int qmcd_create(qmcd_handle* out, int N, int K, int batch,
+                           void* workspace_dev, size_t workspace_bytes, void* cuda_stream) {
+    if (!out) return QMCD_EINVAL;
+    *out = nullptr;
+    size_t need = qmcd_workspace_bytes(N, K, batch);
+    if (need == 0 || !workspace_dev || workspace_bytes < need || ((uintptr_t)workspace_dev & 255)) return QMCD_EINVAL;
+    int dev = 0;
+    CK(nullptr, cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    CK(nullptr, cudaGetDeviceProperties(&prop, dev));
+    if (prop.major < 10) { snprintf(g_last_error, sizeof(g_last_error), "device sm_%d%d is not Blackwell (sm_100a build)", prop.major, prop.minor); return QMCD_ECUDA; }
+    qmcd_ctx* h = new (std::nothrow) qmcd_ctx();
+    if (!h) return QMCD_EINVAL;
+    memset(h, 0, sizeof(*h));
+    h->N = N; h->K = K; h->batch = batch;
+    h->stream = (cudaStream_t)cuda_stream;
+    h->state = QMCD_IDLE;
+    unsigned char* ws = (unsigned char*)workspace_dev;
+    WsLayout L = ws_layout(N, K, batch);
+    QmcdDev& P = h->P;
+    P.N = N; P.K = K; P.batch = batch; P.S = 1; P.B = nullptr;
+    P.C = (double*)(ws + L.C); P.W = (double*)(ws + L.W); P.Y = (double*)(ws + L.Y);
+    P.M = (double*)(ws + L.M); P.J = (int*)(ws + L.J); P.m = (int*)(ws + L.m);
+    P.sj = (int*)(ws + L.sj); P.sR = (double*)(ws + L.sR);
+    P.sp = (double*)(ws + L.sp); P.sc = (double*)(ws + L.sc);
+    P.counters = (long long*)(ws + L.counters); P.status = (int*)(ws + L.status);
+    P.flush_path = 0;
+    int rc = QMCD_OK;
+    do {
+        cudaError_t e = cudaMemsetAsync(ws, 0, L.total, h->stream);
+        if (e != cudaSuccess) { rc = cuda_fail(h, e, "cudaMemsetAsync(workspace)"); break; }
+        e = cudaMemsetAsync(P.sj, 0xff, (size_t)batch * 4, h->stream);
+        if (e != cudaSuccess) { rc = cuda_fail(h, e, "cudaMemsetAsync(sj)"); break; }
+        e = cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking);
+        if (e != cudaSuccess) { rc = cuda_fail(h, e, "cudaStreamCreate"); break; }
+        for (int i = 0; i < 2 && rc == QMCD_OK; ++i) {
+            if ((e = cudaEventCreateWithFlags(&h->ev_h2d[i], cudaEventDisableTiming)) != cudaSuccess) rc = cuda_fail(h, e, "cudaEventCreate");
+            else if ((e = cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming)) != cudaSuccess) rc = cuda_fail(h, e, "cudaEventCreate");
+        }
+        if (rc != QMCD_OK) break;
+        h->max_cluster = 16;
+        int S = default_cluster(N, batch, prop.multiProcessorCount, h->max_cluster);
+        // shrink S until the device says a cluster of that size (with our smem) fits
+        for (;;) {
+            rc = configure_kernel(h, S);
+            if (rc != QMCD_OK) break;
+            cudaLaunchConfig_t cfg; memset(&cfg, 0, sizeof(cfg));
+            cfg.gridDim = dim3((unsigned)(batch * S)); cfg.blockDim = dim3(QMCD_THREADS);
+            cfg.dynamicSmemBytes = h->smem_bytes;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeClusterDimension;
+            attr[0].val.clusterDim.x = (unsigned)S; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+            cfg.attrs = attr; cfg.numAttrs = 1;
+            int nclusters = 0;
+            e = cudaOccupancyMaxActiveClusters(&nclusters, qmcd_kernel, &cfg);
+            if (e == cudaSuccess && nclusters >= 1 && (nclusters >= batch || S == 1)) break;
+            if (e != cudaSuccess) (void)cudaGetLastError();
+            if (S == 1) { if (e != cudaSuccess) rc = cuda_fail(h, e, "cudaOccupancyMaxActiveClusters"); break; }
+            S /= 2;
+        }
+    } while (0);
+    if (rc != QMCD_OK) {
+        if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+        for (int i = 0; i < 2; ++i) { if (h->ev_h2d[i]) cudaEventDestroy(h->ev_h2d[i]); if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]); }
+        delete h;
+        return rc;
+    }
+    *out = h;
+    return QMCD_OK;
+}
+
+extern "C" int qmcd_destroy(qmcd_handle h) {
+    if (!h) return QMCD_OK;
+    cudaStreamSynchronize(h->stream);
+    cudaStreamSynchronize(h->copy_stream);
+    cudaStreamDestroy(h->copy_stream);
+    for (int i = 0; i < 2; ++i) { cudaEventDestroy(h->ev_h2d[i]); cudaEventDestroy(h->ev_done[i]); }
+    delete h;
+    return QMCD_OK;
+}
+
+extern "C" int qmcd_set_inverse(qmcd_handle h, double* Ainv_dev) {
+    if (!h || !Ainv_dev || ((uintptr_t)Ainv_dev & 15)) return QMCD_EINVAL;
+    if (h->state != QMCD_IDLE) return QMCD_ESTATE;
+    h->P.B = Ainv_dev;
+    CK(h, cudaMemsetAsync(h->P.m, 0, (size_t)h->batch * 4, h->stream));
+    CK(h, cudaMemsetAsync(h->P.sj, 0xff, (size_t)h->batch * 4, h->stream));
+    CK(h, cudaMemsetAsync(h->P.counters, 0, (size_t)h->batch * 16, h->stream));
+    CK(h, cudaMemsetAsync(h->P.status, 0, 16, h->stream));
+    h->has_inverse = true;
+    return QMCD_OK;
+}
+
+static QmcdArgs base_args(qmcd_ctx* h, int mode) {
+    QmcdArgs a;
+    memset(&a, 0, sizeof(a));
+    a.P = h->P;
+    a.mode = mode;
+    return a;
+}
+
+extern "C" int qmcd_ratio(qmcd_handle h, int j, const double* v_dev, double* R_dev) {
+    if (!h || !v_dev || !R_dev || j < 0 || j >= h->N) return QMCD_EINVAL;
+    if (!h->has_inverse) return QMCD_ESTATE;
+    QmcdArgs a = base_args(h, QMCD_MODE_RATIO);
+    a.j = j; a.v = v_dev; a.R_out = R_dev;
+    int rc = launch(h, a);
+    if (rc == QMCD_OK) h->state = QMCD_PROPOSED;
+    return rc;
+}
+
+extern "C" int qmcd_ratio_jv(qmcd_handle h, const int* j_dev, const double* v_dev, double* R_dev) {
+    if (!h || !j_dev || !v_dev || !R_dev) return QMCD_EINVAL;
+    if (!h->has_inverse) return QMCD_ESTATE;
+    QmcdArgs a = base_args(h, QMCD_MODE_RATIO);
+    a.jv = j_dev; a.v = v_dev; a.R_out = R_dev;
+    int rc = launch(h, a);
+    if (rc == QMCD_OK) h->state = QMCD_PROPOSED;
+    return rc;
+}
+
+extern "C" int qmcd_accept(qmcd_handle h, const unsigned char* mask_dev) {
+    if (!h) return QMCD_EINVAL;
+    if (h->state != QMCD_PROPOSED) return QMCD_ESTATE;
+    QmcdArgs a = base_args(h, QMCD_MODE_ACCEPT);
+    a.mask = mask_dev; a.accept_all = (mask_dev == nullptr);
+    int rc = launch(h, a);
+    if (rc == QMCD_OK) h->state = QMCD_IDLE;
+    return rc;
+}
+
+extern "C" int qmcd_accept_metropolis(qmcd_handle h, const double* uniforms_dev, unsigned char* acc_out_dev) {
+    if (!h || !uniforms_dev) return QMCD_EINVAL;
+    if (h->state != QMCD_PROPOSED) return QMCD_ESTATE;
+    QmcdArgs a = base_args(h, QMCD_MODE_ACCEPT);
+    a.uniforms = uniforms_dev; a.acc_out = acc_out_dev;
+    int rc = launch(h, a);
+    if (rc == QMCD_OK) h->state = QMCD_IDLE;
+    return rc;
+}
+
+extern "C" int qmcd_reject(qmcd_handle h) {
+    if (!h) return QMCD_EINVAL;
+    if (h->state != QMCD_PROPOSED) return QMCD_ESTATE;
+    CK(h, cudaMemsetAsync(h->P.sj, 0xff, (size_t)h->batch * 4, h->stream));
+    h->state = QMCD_IDLE;
+    return QMCD_OK;
+}
+
+extern "C" int qmcd_flush(qmcd_handle h) {
+    if (!h) return QMCD_EINVAL;
+    if (h->state != QMCD_IDLE) return QMCD_ESTATE;
+    if (!h->has_inverse) return QMCD_OK;
+    QmcdArgs a = base_args(h, QMCD_MODE_FLUSH);
+    return launch(h, a);
+}
+
+extern "C" int qmcd_pending(qmcd_handle h, int* m_dev) {
+    if (!h || !m_dev) return QMCD_EINVAL;
+    CK(h, cudaMemcpyAsync(m_dev, h->P.m, (size_t)h->batch * 4, cudaMemcpyDeviceToDevice, h->stream));
+    return QMCD_OK;
+}
+
+extern "C" int qmcd_counters(qmcd_handle h, long long* counters_dev) {
+    if (!h || !counters_dev) return QMCD_EINVAL;
+    CK(h, cudaMemcpyAsync(counters_dev, h->P.counters, (size_t)h->batch * 16, cudaMemcpyDeviceToDevice, h->stream));
+    return QMCD_OK;
+}
+
+extern "C" int qmcd_status(qmcd_handle h, int* host_out, int* info_out) {
+    if (!h || !host_out) return QMCD_EINVAL;
+    int st[4] = {0, 0, 0, 0};
+    CK(h, cudaMemcpyAsync(st, h->P.status, 16, cudaMemcpyDeviceToHost, h->stream));
+    CK(h, cudaStreamSynchronize(h->stream));
+    *host_out = st[0];
+    if (info_out) { info_out[0] = st[1]; info_out[1] = st[2]; }
+    return QMCD_OK;
+}
+
+extern "C" int qmcd_sweep(qmcd_handle h, int j_begin, int n_moves,
+                          const double* proposals_dev, const unsigned char* mask_dev,
+                          const double* uniforms_dev, double* R_out_dev, unsigned char* acc_out_dev) {
+    if (!h || n_moves < 0 || j_begin < 0 || j_begin >= h->N) return QMCD_EINVAL;
+    if ((mask_dev == nullptr) == (uniforms_dev == nullptr)) return QMCD_EINVAL;
+    if (n_moves > 0 && !proposals_dev) return QMCD_EINVAL;
+    if (h->state != QMCD_IDLE || !h->has_inverse) return QMCD_ESTATE;
+    if (n_moves == 0) return QMCD_OK;
+    QmcdArgs a = base_args(h, QMCD_MODE_SWEEP);
+    a.j_begin = j_begin; a.n_moves = n_moves; a.v = proposals_dev;
+    a.mask = mask_dev; a.uniforms = uniforms_dev; a.R_out = R_out_dev; a.acc_out = acc_out_dev;
+    return launch(h, a);
+}
+
+extern "C" size_t qmcd_sweep_host_min_staging(int N, int batch) {
+    if (N < 1 || batch < 1) return 0;
+    // two buffers of one move each
+    size_t per_move = al256((size_t)batch * N * 8) + 4 * al256((size_t)batch * 8);
+    return 2 * per_move;
+}
+
+extern "C" int qmcd_sweep_host(qmcd_handle h, int j_begin, int n_moves,
+                               const double* proposals_host, const unsigned char* mask_host,
+                               const double* uniforms_host, double* R_out_host,
+                               unsigned char* acc_out_host, void* staging_dev, size_t staging_bytes) {
+    if (!h || n_moves < 0 || j_begin < 0 || j_begin >= h->N) return QMCD_EINVAL;
+    if ((mask_host == nullptr) == (uniforms_host == nullptr)) return QMCD_EINVAL;
+    if (n_moves > 0 && (!proposals_host || !staging_dev)) return QMCD_EINVAL;
+    if (((uintptr_t)staging_dev & 255) || staging_bytes < qmcd_sweep_host_min_staging(h->N, h->batch)) return QMCD_EINVAL;
+    if (h->state != QMCD_IDLE || !h->has_inverse) return QMCD_ESTATE;
+    const size_t bn = (size_t)h->batch * h->N * 8, b8 = (size_t)h->batch * 8, b1 = (size_t)h->batch;
+    // moves per chunk: largest cm with 2 * (al256(cm*bn) + 4*al256(cm*b8)) <= staging
+    long long cm = (long long)((staging_bytes / 2 - 5 * 256) / (bn + 4 * b8));
+    if (cm < 1) cm = 1;
+    if (cm > n_moves) cm = n_moves > 0 ? n_moves : 1;
+    const size_t half = staging_bytes / 2 & ~(size_t)255;
+    for (int c = 0, t0 = 0; t0 < n_moves; ++c, t0 += (int)cm) {
+        const int cnt = (int)((n_moves - t0 < cm) ? n_moves - t0 : cm);
+        const int buf = c & 1;
+        unsigned char* base = (unsigned char*)staging_dev + (size_t)buf * half;
+        double* d_prop = (double*)base;
+        double* d_uni = (double*)(base + al256((size_t)cm * bn));
+        double* d_R = (double*)((unsigned char*)d_uni + al256((size_t)cm * b8));
+        unsigned char* d_mask = (unsigned char*)d_R + al256((size_t)cm * b8);
+        unsigned char* d_acc = d_mask + al256((size_t)cm * b8);
+        if (c >= 2) CK(h, cudaStreamWaitEvent(h->copy_stream, h->ev_done[buf], 0));
+        CK(h, cudaMemcpyAsync(d_prop, (const unsigned char*)proposals_host + (size_t)t0 * bn, (size_t)cnt * bn, cudaMemcpyHostToDevice, h->copy_stream));
+        if (mask_host) CK(h, cudaMemcpyAsync(d_mask, mask_host + (size_t)t0 * b1, (size_t)cnt * b1, cudaMemcpyHostToDevice, h->copy_stream));
+        else CK(h, cudaMemcpyAsync(d_uni, (const unsigned char*)uniforms_host + (size_t)t0 * b8, (size_t)cnt * b8, cudaMemcpyHostToDevice, h->copy_stream));
+        CK(h, cudaEventRecord(h->ev_h2d[buf], h->copy_stream));
+        CK(h, cudaStreamWaitEvent(h->stream, h->ev_h2d[buf], 0));
+        int rc = qmcd_sweep(h, (j_begin + t0) % h->N, cnt, d_prop, mask_host ? d_mask : nullptr,
+                            mask_host ? nullptr : d_uni, d_R, d_acc);
+        if (rc != QMCD_OK) return rc;
+        if (R_out_host) CK(h, cudaMemcpyAsync((unsigned char*)R_out_host + (size_t)t0 * b8, d_R, (size_t)cnt * b8, cudaMemcpyDeviceToHost, h->stream));
+        if (acc_out_host) CK(h, cudaMemcpyAsync(acc_out_host + (size_t)t0 * b1, d_acc, (size_t)cnt * b1, cudaMemcpyDeviceToHost, h->stream));
+        CK(h, cudaEventRecord(h->ev_done[buf], h->stream));
+    }
+    CK(h, cudaStreamSynchronize(h->stream));
+    CK(h, cudaStreamSynchronize(h->copy_stream));
+    return QMCD_OK;
+}
+
+extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
+    if (!h || !key) return QMCD_EINVAL;
+    if (h->state != QMCD_IDLE) return QMCD_ESTATE;
+    if (!strcmp(key, "cluster")) {
+        if (value < 1 || value > 16 || value > h->N) return QMCD_EINVAL;
+        CK(h, cudaStreamSynchronize(h->stream));
+        return configure_kernel(h, value);
+    }
+    if (!strcmp(key, "flush_path")) {
+        if (value < 0 || value > 2) return QMCD_EINVAL;
+        h->P.flush_path = value;
+        return QMCD_OK;
+    }
+    return QMCD_EINVAL;
+}
+
+extern "C" int qmcd_get_option(qmcd_handle h, const char* key) {
+    if (!h || !key) return QMCD_EINVAL;
+    if (!strcmp(key, "cluster")) return h->P.S;
+    if (!strcmp(key, "flush_path")) return h->P.flush_path;
+    if (!strcmp(key, "threads")) return QMCD_THREADS;
+    if (!strcmp(key, "smem_bytes")) return (int)h->smem_bytes;
+    return QMCD_EINVAL;
+}
+
+extern "C" const char* qmcd_strerror(int code) {
+    switch (code) {
+        case QMCD_OK: return "ok";
+        case QMCD_EINVAL: return "invalid argument";
+        case QMCD_ESTATE: return "call not legal in the current state";
+        case QMCD_ECUDA: return g_last_error[0] ? g_last_error : "CUDA error";
+        case QMCD_ESINGULAR: return "accepted a move with R == 0 or non-finite R (singular)";
+        default: return "unknown error";
+    }
+}
+
+extern "C" const char* qmcd_version(void) { return "qmcd 0.1 (sm_100a)"; }

@@ -1,0 +1,119 @@
+// qmcd_dev.cuh -- device-side state, shared-memory carving and small helpers.
+// One thread-block CLUSTER of S CTAs owns one walker (walkers are
+// independent, so there is no cross-cluster dependency anywhere).  CTA r of the
+// cluster owns COLUMN slice [N r/S, N (r+1)/S) of every length-N vector in the
+// look-ahead (Eq. 3) and ROW slice [N r/S, N (r+1)/S) of B in the flush (Eq. 4).
+#pragma once
+#include <cuda_runtime.h>
+#include <cooperative_groups.h>
+#include <stdint.h>
+
+namespace cg = cooperative_groups;
+
+#define QMCD_THREADS 256
+#define QMCD_WARPS (QMCD_THREADS / 32)
+
+// Status codes mirrored from include/qmcd.h (kept numerically identical).
+#define QMCD_DEV_EINVAL (-1)
+#define QMCD_DEV_ESINGULAR (-4)
+
+struct QmcdDev {
+    int N, K, batch, S;       // S = CTAs per walker (cluster size)
+    double* B;                // [batch][N][N]  inverse, borrowed, updated in place
+    double* C;                // [batch][K][N]  queued new columns v_i (one per row)
+    double* W;                // [batch][K][N]  rows j_i of the stale inverse B0
+    double* Y;                // [batch][K][N]  scratch: Y = M W of Eq. 4
+    double* M;                // [batch][K][K]  (I + V'A^-1 U)^-1 = (W C^T)^-1, ld = K
+    int* J;                   // [batch][K]     queued electron indices
+    int* m;                   // [batch]        queue length
+    int* sj;                  // [batch]        staged electron, -1 = none
+    double* sR;               // [batch]        staged ratio
+    double* sp;               // [batch][K]     staged p (delta term applied)
+    double* sc;               // [batch][K]     staged c = M q
+    long long* counters;      // [batch][2]     accepted, flushes
+    int* status;              // [4]            sticky: code, walker, move counter
+    int flush_path;           // 0 auto, 1 CUDA-core, 2 DMMA
+};
+
+enum QmcdMode { QMCD_MODE_RATIO = 0, QMCD_MODE_ACCEPT = 1, QMCD_MODE_FLUSH = 2, QMCD_MODE_SWEEP = 3 };
+
+struct QmcdArgs {
+    QmcdDev P;
+    int mode;
+    // RATIO
+    int j;                        // electron (all walkers) when jv == nullptr
+    const int* jv;                // [batch] per-walker electron or nullptr
+    const double* v;              // [batch][N]
+    double* R_out;                // [batch]
+    // ACCEPT
+    const unsigned char* mask;    // [batch] or nullptr
+    const double* uniforms;       // [batch] or nullptr (Metropolis)
+    unsigned char* acc_out;       // [batch] or nullptr
+    int accept_all;
+    // SWEEP: v/mask/uniforms/R_out/acc_out are [n_moves][batch]...
+    int j_begin, n_moves;
+};
+
+// Shared-memory carving; every CTA of the cluster has the same layout.
+struct QmcdSmem {
+    double* rs;      // [Ns]  slice of B0[j,:]
+    double* vs;      // [Ns]  slice of v
+    double* part;    // [S][2K+1] partial p, q, d from every CTA (used in the leader)
+    double* pf;      // [K]
+    double* qf;      // [K]
+    double* cf;      // [K]
+    double* rf;      // [K]
+    double* Ts;      // [QMCD_WARPS][K]  T rows of the CUDA-core flush
+    double* red;     // [32]
+    int* iflag;      // [8]
+    unsigned char* dyn;  // rest: flush tiles (DMMA path)
+};
+
+__host__ __device__ inline int qmcd_slice_lo(int N, int S, int r) { return (int)(((long long)N * r) / S); }
+__host__ __device__ inline size_t qmcd_align16(size_t x) { return (x + 15) & ~(size_t)15; }
+
+__host__ __device__ inline size_t qmcd_smem_base_bytes(int N, int K, int S) {
+    size_t ns = (size_t)(N + S - 1) / S + 1;
+    size_t b = 0;
+    b += qmcd_align16(ns * 8) * 2;                 // rs, vs
+    b += qmcd_align16((size_t)S * (2 * K + 1) * 8);  // part
+    b += qmcd_align16((size_t)K * 8) * 4;          // pf qf cf rf
+    b += qmcd_align16((size_t)QMCD_WARPS * K * 8); // Ts
+    b += 32 * 8 + 8 * 4 + 16;
+    return qmcd_align16(b);
+}
+
+__device__ inline QmcdSmem qmcd_carve(unsigned char* base, int N, int K, int S) {
+    QmcdSmem s;
+    size_t ns = (size_t)(N + S - 1) / S + 1;
+    unsigned char* p = base;
+    s.rs = (double*)p; p += qmcd_align16(ns * 8);
+    s.vs = (double*)p; p += qmcd_align16(ns * 8);
+    s.part = (double*)p; p += qmcd_align16((size_t)S * (2 * K + 1) * 8);
+    s.pf = (double*)p; p += qmcd_align16((size_t)K * 8);
+    s.qf = (double*)p; p += qmcd_align16((size_t)K * 8);
+    s.cf = (double*)p; p += qmcd_align16((size_t)K * 8);
+    s.rf = (double*)p; p += qmcd_align16((size_t)K * 8);
+    s.Ts = (double*)p; p += qmcd_align16((size_t)QMCD_WARPS * K * 8);
+    s.red = (double*)p; p += 32 * 8;
+    s.iflag = (int*)p; p += 8 * 4 + 16;
+    s.dyn = base + qmcd_smem_base_bytes(N, K, S);
+    return s;
+}
+
+__device__ __forceinline__ double qmcd_warp_sum(double x) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    return x;
+}
+
+// L2-coherent loads for data another CTA of the cluster may have written
+// (B rows after a flush, Y, M): bypass the (non-coherent) L1.
+__device__ __forceinline__ double qmcd_ldcg(const double* p) { return __ldcg(p); }
+
+__device__ __forceinline__ void qmcd_set_status(const QmcdDev& P, int code, int walker, long long move) {
+    if (atomicCAS(P.status, 0, code) == 0) {
+        P.status[1] = walker;
+        P.status[2] = (int)move;
+    }
+}

@@ -1,0 +1,317 @@
+"""GPU parity: the CUDA path (through the C-ABI / binding) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json's north_star: identical
+accept sequence, every ratio to relative error <= 1e-10, max|A.Ainv - I| <= 1e-8 after every
+flush (fp64)."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1708_00744_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+RTOL_RATIO = 1e-10
+TOL_RESID = 1e-8
+
+
+def _dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _rel(a, b):
+    return np.max(np.abs(a - b) / np.maximum(np.abs(b), 1e-300))
+
+
+def gpu_sweep(qmcd, wl, K, mask=None, uniforms=None, final_flush=True, cluster=None, j_begin=0):
+    import torch
+    q = qmcd.Qmcd(wl.N, K, wl.batch)
+    if cluster is not None:
+        q.set_option("cluster", cluster)
+    B = _dev(wl.Ainv)
+    q.set_inverse(B)
+    P = _dev(wl.proposals)
+    R = torch.zeros((wl.n_moves, wl.batch), dtype=torch.float64, device="cuda")
+    acc = torch.zeros((wl.n_moves, wl.batch), dtype=torch.uint8, device="cuda")
+    q.sweep(j_begin, P, mask=None if mask is None else _dev(mask),
+            uniforms=None if uniforms is None else _dev(uniforms), R_out=R, acc_out=acc)
+    if final_flush:
+        q.flush()
+    st, info = q.status()
+    cnt = q.counters().cpu().numpy()
+    pend = q.pending().cpu().numpy()
+    out = dict(R=R.cpu().numpy(), acc=acc.cpu().numpy(), B=B.cpu().numpy(), status=st, info=info,
+               counters=cnt, pending=pend, S=q.get_option("cluster"))
+    q.close()
+    return out
+
+
+def gpu_calls(qmcd, wl, K, mask, flush_every=None, residual_cb=None):
+    """The per-call API: ratio -> accept(mask) per move."""
+    import torch
+    q = qmcd.Qmcd(wl.N, K, wl.batch)
+    B = _dev(wl.Ainv)
+    q.set_inverse(B)
+    P = _dev(wl.proposals)
+    Md = _dev(mask)
+    R = torch.zeros((wl.n_moves, wl.batch), dtype=torch.float64, device="cuda")
+    for t in range(wl.n_moves):
+        q.ratio(t % wl.N, P[t], R[t])
+        q.accept(Md[t])
+        if flush_every and (t + 1) % flush_every == 0:
+            q.flush()
+        if residual_cb is not None:
+            residual_cb(t, q, B)
+    q.flush()
+    st, _ = q.status()
+    out = dict(R=R.cpu().numpy(), B=B.cpu().numpy(), status=st, counters=q.counters().cpu().numpy())
+    q.close()
+    return out
+
+
+def check_residuals(wl, acc, B):
+    for w in range(wl.batch):
+        A_cur = inputs.current_matrix(wl.A[w], wl.proposals[:, w, :], acc[:, w], wl.n_moves)
+        res = np.max(np.abs(A_cur @ B[w] - np.eye(wl.N)))
+        assert res <= TOL_RESID, (w, res)
+
+
+# ------------------------------------------------------------------ config 0, every check
+def test_c0_calls_vs_oracle_delayed_rank1_and_residual_after_every_flush(qmcd):
+    """BASELINE.json configs[0]: N=64, K=4, 2 sweeps, Bernoulli(0.99); per-call API."""
+    wl = inputs.make_config("c0")
+    mask = wl.bernoulli_mask(0.99)
+    K = 4
+    B1 = wl.Ainv.copy(); R1, acc1, _ = oracle.run(1, B1, 1, wl.proposals, mask=mask)
+    B2 = wl.Ainv.copy(); R2, acc2, _ = oracle.run(2, B2, K, wl.proposals, mask=mask)
+    seen = {"flushes": 0, "last": 0}
+
+    def cb(t, q, B):
+        c = int(q.counters()[0, 1].item())
+        if c != seen["last"]:           # a flush happened inside this accept
+            seen["last"] = c; seen["flushes"] += 1
+            assert int(q.pending()[0].item()) == 0
+            A_cur = inputs.current_matrix(wl.A[0], wl.proposals[:, 0, :], mask[:, 0], t + 1)
+            res = np.max(np.abs(A_cur @ B[0].cpu().numpy() - np.eye(wl.N)))
+            assert res <= TOL_RESID, (t, res)
+
+    g = gpu_calls(qmcd, wl, K, mask, residual_cb=cb)
+    assert g["status"] == 0
+    assert seen["flushes"] == int(mask.sum()) // K
+    assert _rel(g["R"], R2) <= RTOL_RATIO and _rel(g["R"], R1) <= RTOL_RATIO
+    assert np.max(np.abs(g["B"] - B2)) <= 1e-11 and np.max(np.abs(g["B"] - B1)) <= 1e-11
+    check_residuals(wl, mask, g["B"])
+    assert int(g["counters"][0, 0]) == int(mask.sum())
+    # explicit LU at sampled moves (path 0)
+    A = wl.A[0].copy()
+    for t in range(wl.n_moves):
+        if t % 9 == 0:
+            Rb = oracle.ratio_bruteforce(A, t % wl.N, wl.proposals[t, 0])
+            assert abs(g["R"][t, 0] - Rb) <= RTOL_RATIO * abs(Rb)
+        if mask[t, 0]:
+            A[:, t % wl.N] = wl.proposals[t, 0]
+
+
+# ------------------------------------------------------------------ ragged sizes, several tiles
+@pytest.mark.parametrize("N,K,batch,cluster", [
+    (100, 7, 3, 1), (100, 7, 3, 2), (130, 16, 2, 4), (257, 33, 2, 8), (96, 96, 1, 1), (64, 1, 2, 1),
+    (520, 40, 2, 16), (33, 5, 150, 1),
+])
+def test_sweep_matches_oracle_ragged(qmcd, N, K, batch, cluster):
+    wl = inputs.make_workload(batch, N, n_moves=min(2 * N + 3, 300), seed=7)
+    mask = wl.bernoulli_mask(0.8)
+    Bo = wl.Ainv.copy(); Ro, acco, _ = oracle.run(2, Bo, K, wl.proposals, mask=mask)
+    g = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster)
+    assert g["status"] == 0 and g["S"] == cluster
+    assert np.array_equal(g["acc"], acco)
+    assert _rel(g["R"], Ro) <= RTOL_RATIO
+    assert np.max(np.abs(g["B"] - Bo)) <= 1e-10
+    check_residuals(wl, mask, g["B"])
+    assert np.array_equal(g["counters"][:, 0], mask.sum(axis=0))
+    assert np.all(g["pending"] == 0)
+
+
+def test_sweep_equals_call_by_call(qmcd):
+    """qmcd_sweep must reproduce the ratio -> accept(mask) sequence (include/qmcd.h)."""
+    wl = inputs.make_workload(4, 128, 200, seed=3)
+    mask = wl.bernoulli_mask(0.7)
+    a = gpu_sweep(qmcd, wl, 8, mask=mask)
+    b = gpu_calls(qmcd, wl, 8, mask)
+    assert np.array_equal(a["R"], b["R"])
+    assert np.array_equal(a["B"], b["B"])
+
+
+@pytest.mark.parametrize("K", [1, 16, 32])
+def test_c1_full_size_vs_rank1_oracle(qmcd, K):
+    """BASELINE.json configs[1] at full size, in bench.py's launch configuration (qmcd_sweep):
+    ratios and accept sequence are K-independent, so one rank-1 oracle run is the
+    reference for every K."""
+    wl = inputs.make_config("c1")
+    mask = wl.bernoulli_mask(0.99)
+    ref = getattr(test_c1_full_size_vs_rank1_oracle, "_ref", None)
+    if ref is None:
+        B1 = wl.Ainv.copy(); R1, acc1, _ = oracle.run(1, B1, 1, wl.proposals, mask=mask)
+        ref = (R1, acc1, B1)
+        test_c1_full_size_vs_rank1_oracle._ref = ref
+    R1, acc1, B1 = ref
+    g = gpu_sweep(qmcd, wl, K, mask=mask)
+    assert g["status"] == 0
+    assert np.array_equal(g["acc"], acc1)
+    assert _rel(g["R"], R1) <= RTOL_RATIO
+    assert np.max(np.abs(g["B"] - B1)) <= 1e-9
+    check_residuals(wl, mask, g["B"])
+
+
+def test_metropolis_accept_sequence_identical(qmcd):
+    """BASELINE.json configs[2] rule u < min(1, R^2), reduced size."""
+    wl = inputs.make_workload(8, 256, 512, seed=11)
+    Bo = wl.Ainv.copy(); Ro, acco, _ = oracle.run(2, Bo, 16, wl.proposals, uniforms=wl.uniforms)
+    g = gpu_sweep(qmcd, wl, 16, uniforms=wl.uniforms)
+    near_tie = np.abs(wl.uniforms - np.minimum(1.0, Ro * Ro)) < 1e-9      # reading G20
+    assert np.array_equal(g["acc"][~near_tie], acco[~near_tie])
+    assert near_tie.sum() == 0
+    assert _rel(g["R"], Ro) <= RTOL_RATIO
+    assert 0.9 < acco.mean() < 1.0
+    check_residuals(wl, acco, g["B"])
+
+
+def test_metropolis_per_call(qmcd):
+    import torch
+    wl = inputs.make_workload(3, 96, 120, seed=5)
+    Bo = wl.Ainv.copy(); Ro, acco, _ = oracle.run(2, Bo, 6, wl.proposals, uniforms=wl.uniforms)
+    q = qmcd.Qmcd(wl.N, 6, wl.batch)
+    B = _dev(wl.Ainv); q.set_inverse(B)
+    P, U = _dev(wl.proposals), _dev(wl.uniforms)
+    R = torch.zeros((wl.n_moves, wl.batch), dtype=torch.float64, device="cuda")
+    acc = torch.zeros((wl.n_moves, wl.batch), dtype=torch.uint8, device="cuda")
+    for t in range(wl.n_moves):
+        q.ratio(t % wl.N, P[t], R[t])
+        q.accept_metropolis(U[t], acc[t])
+    q.flush()
+    assert q.status()[0] == 0
+    assert np.array_equal(acc.cpu().numpy(), acco)
+    assert _rel(R.cpu().numpy(), Ro) <= RTOL_RATIO
+    assert np.max(np.abs(B.cpu().numpy() - Bo)) <= 1e-10
+
+
+def test_flush_neutrality_and_K_independence(qmcd):
+    """delayed == one at a time; inserting qmcd_flush anywhere changes no ratio."""
+    wl = inputs.make_workload(2, 128, 256, seed=13)
+    mask = wl.bernoulli_mask(0.9)
+    base = gpu_calls(qmcd, wl, 16, mask)
+    for fe in (1, 5, 37):
+        o = gpu_calls(qmcd, wl, 16, mask, flush_every=fe)
+        assert _rel(o["R"], base["R"]) <= 1e-11
+        assert np.max(np.abs(o["B"] - base["B"])) <= 1e-11
+    for K in (1, 3, 128):
+        o = gpu_sweep(qmcd, wl, K, mask=mask)
+        assert _rel(o["R"], base["R"]) <= 1e-11
+        assert np.max(np.abs(o["B"] - base["B"])) <= 1e-11
+
+
+def test_repeated_electron_in_window_and_ratio_jv(qmcd):
+    """Reading G7: the delta term keeps the ratio exact for an already-queued electron, and
+    accepting it flushes first.  Uses per-walker electron indices (qmcd_ratio_jv)."""
+    import torch
+    N, K, batch = 48, 6, 3
+    wl = inputs.make_workload(batch, N, 12, seed=21)
+    js = np.array([[0, 5, 9], [1, 5, 3], [0, 7, 9], [2, 5, 9], [0, 5, 1], [4, 4, 4], [4, 4, 4]], dtype=np.int32)
+    q = qmcd.Qmcd(N, K, batch)
+    B = _dev(wl.Ainv); q.set_inverse(B)
+    P = _dev(wl.proposals)
+    R = torch.zeros(batch, dtype=torch.float64, device="cuda")
+    D = [oracle.Delayed(wl.Ainv[w].copy(), K) for w in range(batch)]
+    A = [wl.A[w].copy() for w in range(batch)]
+    for t in range(js.shape[0]):
+        q.ratio(_dev(js[t]), P[t], R)
+        q.accept()
+        Rg = R.cpu().numpy()
+        for w in range(batch):
+            Ro = D[w].ratio(int(js[t, w]), wl.proposals[t, w])
+            Rb = oracle.ratio_bruteforce(A[w], int(js[t, w]), wl.proposals[t, w])
+            assert abs(Rg[w] - Ro) <= RTOL_RATIO * abs(Ro)
+            assert abs(Rg[w] - Rb) <= 1e-9 * abs(Rb)
+            D[w].accept()
+            A[w][:, js[t, w]] = wl.proposals[t, w]
+    pend = q.pending().cpu().numpy()
+    assert list(pend) == [D[w].pending for w in range(batch)]
+    q.flush()
+    assert q.status()[0] == 0
+    Bg = B.cpu().numpy()
+    for w in range(batch):
+        assert np.max(np.abs(A[w] @ Bg[w] - np.eye(N))) <= TOL_RESID
+    q.close()
+
+
+def test_closed_form_current_column_gives_one_and_linear_combination(qmcd):
+    """Pin P2 on the GPU: v = A_cur alpha  =>  R = alpha_j exactly, mid-window too."""
+    import torch
+    N, K = 80, 8
+    wl = inputs.make_workload(1, N, 5, seed=4)
+    q = qmcd.Qmcd(N, K, 1)
+    B = _dev(wl.Ainv); q.set_inverse(B)
+    R = torch.zeros(1, dtype=torch.float64, device="cuda")
+    A = wl.A[0].copy()
+    for t in range(5):                                   # queue 5 moves
+        q.ratio(t, _dev(wl.proposals[t]), R); q.accept()
+        A[:, t] = wl.proposals[t, 0]
+    rng = np.random.default_rng(0)
+    alpha = rng.standard_normal(N)
+    for j in (2, 40):                                    # queued and not queued electron
+        q.ratio(j, _dev((A @ alpha)[None, :]), R); q.reject()
+        assert abs(R.item() - alpha[j]) <= 1e-11 * max(1, abs(alpha[j]))
+        q.ratio(j, _dev(A[:, j][None, :].copy()), R); q.reject()
+        assert abs(R.item() - 1.0) <= 1e-12
+    q.close()
+
+
+def test_state_machine_and_singular_status(qmcd):
+    import torch
+    N = 32
+    wl = inputs.make_workload(1, N, 2, seed=2)
+    q = qmcd.Qmcd(N, 4, 1)
+    R = torch.zeros(1, dtype=torch.float64, device="cuda")
+    v = _dev(wl.proposals[0])
+    with pytest.raises(qmcd.QmcdError) as e:
+        q.ratio(0, v, R)                                 # no inverse yet
+    assert e.value.code == qmcd.ESTATE
+    B = _dev(wl.Ainv); q.set_inverse(B)
+    with pytest.raises(qmcd.QmcdError):
+        q.accept()                                       # IDLE
+    with pytest.raises(qmcd.QmcdError):
+        q.ratio(N, v, R)                                 # j out of range
+    q.ratio(0, v, R)
+    with pytest.raises(qmcd.QmcdError):
+        q.flush()                                        # PROPOSED
+    q.ratio(1, v, R)                                     # replaces the staged proposal
+    q.reject()
+    q.flush()                                            # legal when idle, no-op
+    assert q.status()[0] == 0
+    # singular: new column = another column of A  ->  R ~ 0 exactly only if forced; use zeros
+    q.ratio(3, torch.zeros((1, N), dtype=torch.float64, device="cuda"), R)
+    q.accept()
+    st, info = q.status()
+    assert R.item() == 0.0 and st == qmcd.ESINGULAR and info[0] == 0
+    assert int(q.pending()[0].item()) == 0               # the move was dropped
+    q.close()
+
+
+def test_sweep_host_matches_device_sweep(qmcd):
+    """The end-to-end path (host buffers, chunked double-buffered copies) gives the same results."""
+    import torch
+    wl = inputs.make_workload(4, 128, 300, seed=9)
+    mask = wl.bernoulli_mask(0.9)
+    ref = gpu_sweep(qmcd, wl, 8, mask=mask, final_flush=False)
+    q = qmcd.Qmcd(wl.N, 8, wl.batch)
+    B = _dev(wl.Ainv); q.set_inverse(B)
+    Ph = torch.from_numpy(wl.proposals).pin_memory()
+    Mh = torch.from_numpy(mask).pin_memory()
+    Rh = torch.zeros((wl.n_moves, wl.batch), dtype=torch.float64).pin_memory()
+    Ah = torch.zeros((wl.n_moves, wl.batch), dtype=torch.uint8).pin_memory()
+    need = qmcd.load().qmcd_sweep_host_min_staging(wl.N, wl.batch)
+    staging = torch.empty(need * 7 + 256, dtype=torch.uint8, device="cuda")   # forces many chunks
+    q.sweep_host(0, Ph, mask=Mh, R_out=Rh, acc_out=Ah, staging=staging)
+    assert np.array_equal(Rh.numpy(), ref["R"])
+    assert np.array_equal(Ah.numpy(), ref["acc"])
+    assert np.array_equal(B.cpu().numpy(), ref["B"])
+    q.close()
