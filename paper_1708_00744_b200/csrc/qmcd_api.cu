@@ -75,9 +75,12 @@ static int default_cluster(int N, int batch, int sms, int max_cluster) {
 }
 
 static int configure_kernel(qmcd_ctx* h, int S) {
-    size_t smem = qmcd_smem_base_bytes(h->N, h->K, S) + qmcd_flush_mma_smem_bytes(h->N, h->K);
-    if (smem > 227 * 1024) smem = qmcd_smem_base_bytes(h->N, h->K, S);
-    if (smem > 227 * 1024) { snprintf(g_last_error, sizeof(g_last_error), "shared memory need %zu > 227 KB", smem); return QMCD_EINVAL; }
+    const size_t base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S);
+    const size_t mma = QMCD_SMEM_HEADER + qmcd_flush_mma_smem_bytes(h->N, h->K);
+    const size_t cap = 227 * 1024;
+    if (base > cap) { snprintf(g_last_error, sizeof(g_last_error), "shared memory need %zu > 227 KB", base); return QMCD_EINVAL; }
+    h->P.mma_smem_ok = (mma <= cap) ? 1 : 0;
+    const size_t smem = (h->P.mma_smem_ok && mma > base) ? mma : base;
     // the attribute is per function, not per handle: always allow the device maximum
     CK(h, cudaFuncSetAttribute(qmcd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     CK(h, cudaFuncSetAttribute(qmcd_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));

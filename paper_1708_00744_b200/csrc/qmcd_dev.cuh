@@ -33,6 +33,7 @@ struct QmcdDev {
     long long* counters;      // [batch][2]     accepted, flushes
     int* status;              // [4]            sticky: code, walker, move counter
     int flush_path;           // 0 auto, 1 CUDA-core, 2 DMMA
+    int mma_smem_ok;          // host: the DMMA flush's shared memory fits
 };
 
 enum QmcdMode { QMCD_MODE_RATIO = 0, QMCD_MODE_ACCEPT = 1, QMCD_MODE_FLUSH = 2, QMCD_MODE_SWEEP = 3 };
@@ -66,12 +67,16 @@ struct QmcdSmem {
     double* Ts;      // [QMCD_WARPS][K]  T rows of the CUDA-core flush
     double* red;     // [32]
     int* iflag;      // [8]
-    unsigned char* dyn;  // rest: flush tiles (DMMA path)
+    unsigned char* dyn;  // start of the region after the header (aliased by the DMMA flush)
 };
 
 __host__ __device__ inline int qmcd_slice_lo(int N, int S, int r) { return (int)(((long long)N * r) / S); }
 __host__ __device__ inline size_t qmcd_align16(size_t x) { return (x + 15) & ~(size_t)15; }
 
+#define QMCD_SMEM_HEADER (32 * 8 + 8 * 4 + 32)      // red[32], iflag[8]; multiple of 16
+
+// Bytes of the look-ahead / accept arrays (after the header).  The DMMA flush
+// ALIASES this region (s.dyn): nothing in it is live across a flush.
 __host__ __device__ inline size_t qmcd_smem_base_bytes(int N, int K, int S) {
     size_t ns = (size_t)(N + S - 1) / S + 1;
     size_t b = 0;
@@ -79,7 +84,6 @@ __host__ __device__ inline size_t qmcd_smem_base_bytes(int N, int K, int S) {
     b += qmcd_align16((size_t)S * (2 * K + 1) * 8);  // part
     b += qmcd_align16((size_t)K * 8) * 4;          // pf qf cf rf
     b += qmcd_align16((size_t)QMCD_WARPS * K * 8); // Ts
-    b += 32 * 8 + 8 * 4 + 16;
     return qmcd_align16(b);
 }
 
@@ -87,6 +91,9 @@ __device__ inline QmcdSmem qmcd_carve(unsigned char* base, int N, int K, int S) 
     QmcdSmem s;
     size_t ns = (size_t)(N + S - 1) / S + 1;
     unsigned char* p = base;
+    s.red = (double*)p; p += 32 * 8;
+    s.iflag = (int*)p; p += 8 * 4 + 32;
+    s.dyn = p;
     s.rs = (double*)p; p += qmcd_align16(ns * 8);
     s.vs = (double*)p; p += qmcd_align16(ns * 8);
     s.part = (double*)p; p += qmcd_align16((size_t)S * (2 * K + 1) * 8);
@@ -95,9 +102,6 @@ __device__ inline QmcdSmem qmcd_carve(unsigned char* base, int N, int K, int S) 
     s.cf = (double*)p; p += qmcd_align16((size_t)K * 8);
     s.rf = (double*)p; p += qmcd_align16((size_t)K * 8);
     s.Ts = (double*)p; p += qmcd_align16((size_t)QMCD_WARPS * K * 8);
-    s.red = (double*)p; p += 32 * 8;
-    s.iflag = (int*)p; p += 8 * 4 + 16;
-    s.dyn = base + qmcd_smem_base_bytes(N, K, S);
     return s;
 }
 

@@ -23,11 +23,14 @@ def _rel(a, b):
     return np.max(np.abs(a - b) / np.maximum(np.abs(b), 1e-300))
 
 
-def gpu_sweep(qmcd, wl, K, mask=None, uniforms=None, final_flush=True, cluster=None, j_begin=0):
+def gpu_sweep(qmcd, wl, K, mask=None, uniforms=None, final_flush=True, cluster=None, j_begin=0,
+              flush_path=None):
     import torch
     q = qmcd.Qmcd(wl.N, K, wl.batch)
     if cluster is not None:
         q.set_option("cluster", cluster)
+    if flush_path is not None:
+        q.set_option("flush_path", flush_path)
     B = _dev(wl.Ainv)
     q.set_inverse(B)
     P = _dev(wl.proposals)
@@ -129,6 +132,33 @@ def test_sweep_matches_oracle_ragged(qmcd, N, K, batch, cluster):
     check_residuals(wl, mask, g["B"])
     assert np.array_equal(g["counters"][:, 0], mask.sum(axis=0))
     assert np.all(g["pending"] == 0)
+
+
+@pytest.mark.parametrize("N,K,batch,cluster,p", [
+    (128, 16, 2, 1, 0.8),      # one 128-row tile, ragged final rank
+    (128, 5, 2, 2, 1.0),       # rank 5 -> padded to 8, 64-row tiles
+    (256, 40, 2, 4, 0.8),      # 64 rows per CTA, rank 40
+    (256, 64, 3, 2, 0.95),     # full 64-wide block, 128-row tiles
+    (512, 96, 2, 4, 0.9),      # two m-blocks (64 + 32), R = 64 layout
+    (256, 200, 1, 1, 0.9),     # four m-blocks, several M row blocks
+    (320, 24, 2, 1, 0.7),      # N = 5 chunks, rows 320 = 2.5 tiles of 128
+    (192, 1, 2, 1, 0.9),       # rank 1 through the tensor path
+])
+def test_dmma_flush_matches_oracle(qmcd, N, K, batch, cluster, p):
+    """The FP64 tensor-core flush (flush_path = 2 forces it whenever N and N/S are multiples
+    of 64) against the oracle's delayed path: every ratio, the accept sequence, the inverse."""
+    wl = inputs.make_workload(batch, N, n_moves=N + K + 7, seed=17)
+    mask = wl.bernoulli_mask(p)
+    Bo = wl.Ainv.copy(); Ro, acco, _ = oracle.run(2, Bo, K, wl.proposals, mask=mask)
+    g = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, flush_path=2)
+    assert g["status"] == 0 and g["S"] == cluster
+    assert np.array_equal(g["acc"], acco)
+    assert _rel(g["R"], Ro) <= RTOL_RATIO
+    assert np.max(np.abs(g["B"] - Bo)) <= 1e-10
+    check_residuals(wl, mask, g["B"])
+    # and the CUDA-core path gives the same inverse to rounding
+    s = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, flush_path=1)
+    assert np.max(np.abs(g["B"] - s["B"])) <= 1e-11
 
 
 def test_sweep_equals_call_by_call(qmcd):
