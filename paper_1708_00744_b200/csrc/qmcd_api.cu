@@ -35,7 +35,7 @@ static int cuda_fail(qmcd_ctx* h, cudaError_t e, const char* what) {
 
 static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-struct WsLayout { size_t C, W, Y, M, J, m, sj, sR, sp, sc, counters, status, total; };
+struct WsLayout { size_t C, W, Y, M, J, m, sj, sR, sp, sc, sr, counters, status, total; };
 
 static WsLayout ws_layout(int N, int K, int batch) {
     WsLayout L; size_t o = 0;
@@ -50,6 +50,7 @@ static WsLayout ws_layout(int N, int K, int batch) {
     L.sR = o; o += al256((size_t)batch * 8);
     L.sp = o; o += al256((size_t)batch * K * 8);
     L.sc = o; o += al256((size_t)batch * K * 8);
+    L.sr = o; o += al256((size_t)batch * K * 8);
     L.counters = o; o += al256((size_t)batch * 2 * 8);
     L.status = o; o += 256;
     L.total = o;
@@ -75,9 +76,11 @@ static int default_cluster(int N, int batch, int sms, int max_cluster) {
 }
 
 static int configure_kernel(qmcd_ctx* h, int S) {
-    const size_t base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S);
-    const size_t mma = QMCD_SMEM_HEADER + qmcd_flush_mma_smem_bytes(h->N, h->K);
     const size_t cap = 227 * 1024;
+    size_t base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true);
+    h->P.m_in_smem = 1;
+    if (base > cap) { base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, false); h->P.m_in_smem = 0; }
+    const size_t mma = QMCD_SMEM_HEADER + qmcd_flush_mma_smem_bytes(h->N, h->K);
     if (base > cap) { snprintf(g_last_error, sizeof(g_last_error), "shared memory need %zu > 227 KB", base); return QMCD_EINVAL; }
     h->P.mma_smem_ok = (mma <= cap) ? 1 : 0;
     const size_t smem = (h->P.mma_smem_ok && mma > base) ? mma : base;
@@ -131,7 +134,7 @@ extern "C" int qmcd_create(qmcd_handle* out, int N, int K, int batch,
     P.C = (double*)(ws + L.C); P.W = (double*)(ws + L.W); P.Y = (double*)(ws + L.Y);
     P.M = (double*)(ws + L.M); P.J = (int*)(ws + L.J); P.m = (int*)(ws + L.m);
     P.sj = (int*)(ws + L.sj); P.sR = (double*)(ws + L.sR);
-    P.sp = (double*)(ws + L.sp); P.sc = (double*)(ws + L.sc);
+    P.sp = (double*)(ws + L.sp); P.sc = (double*)(ws + L.sc); P.sr = (double*)(ws + L.sr);
     P.counters = (long long*)(ws + L.counters); P.status = (int*)(ws + L.status);
     P.flush_path = 0;
     int rc = QMCD_OK;

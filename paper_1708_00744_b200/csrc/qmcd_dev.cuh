@@ -30,10 +30,12 @@ struct QmcdDev {
     double* sR;               // [batch]        staged ratio
     double* sp;               // [batch][K]     staged p (delta term applied)
     double* sc;               // [batch][K]     staged c = M q
+    double* sr;               // [batch][K]     staged r = M^T p
     long long* counters;      // [batch][2]     accepted, flushes
     int* status;              // [4]            sticky: code, walker, move counter
     int flush_path;           // 0 auto, 1 CUDA-core, 2 DMMA
     int mma_smem_ok;          // host: the DMMA flush's shared memory fits
+    int m_in_smem;            // host: every CTA keeps its own copy of M in shared memory
 };
 
 enum QmcdMode { QMCD_MODE_RATIO = 0, QMCD_MODE_ACCEPT = 1, QMCD_MODE_FLUSH = 2, QMCD_MODE_SWEEP = 3 };
@@ -55,35 +57,43 @@ struct QmcdArgs {
     int j_begin, n_moves;
 };
 
-// Shared-memory carving; every CTA of the cluster has the same layout.
+// Shared-memory carving; every CTA of the cluster has the same layout: a small
+// header, then the look-ahead arrays.  The flush (either path) ALIASES everything
+// after the header (s.dyn): nothing there is live across a flush (M is written
+// back to global memory first, and the queue is empty afterwards).
 struct QmcdSmem {
+    double* red;     // [40]  header: block-reduction scratch
+    int* iflag;      // [16]  header
+    unsigned char* dyn;  // start of the aliased region
     double* rs;      // [Ns]  slice of B0[j,:]
     double* vs;      // [Ns]  slice of v
-    double* part;    // [S][2K+1] partial p, q, d from every CTA (used in the leader)
+    double* part;    // [2][S][PL] partial p, q, d from every CTA, double buffered by move parity
     double* pf;      // [K]
     double* qf;      // [K]
     double* cf;      // [K]
     double* rf;      // [K]
     double* Ts;      // [QMCD_WARPS][K]  T rows of the CUDA-core flush
-    double* red;     // [32]
-    int* iflag;      // [8]
-    unsigned char* dyn;  // start of the region after the header (aliased by the DMMA flush)
+    int* Js;         // [K]   queued electron indices (copy of J)
+    double* Ms;      // [K][ldM]  this CTA's copy of M (when P.m_in_smem)
 };
 
 __host__ __device__ inline int qmcd_slice_lo(int N, int S, int r) { return (int)(((long long)N * r) / S); }
 __host__ __device__ inline size_t qmcd_align16(size_t x) { return (x + 15) & ~(size_t)15; }
+__host__ __device__ inline int qmcd_PL(int K) { return 2 * K + 2; }
+__host__ __device__ inline int qmcd_ldM(int K) { return K | 1; }
 
-#define QMCD_SMEM_HEADER (32 * 8 + 8 * 4 + 32)      // red[32], iflag[8]; multiple of 16
+#define QMCD_SMEM_HEADER (40 * 8 + 16 * 4)      // red[40], iflag[16]; multiple of 16
 
-// Bytes of the look-ahead / accept arrays (after the header).  The DMMA flush
-// ALIASES this region (s.dyn): nothing in it is live across a flush.
-__host__ __device__ inline size_t qmcd_smem_base_bytes(int N, int K, int S) {
+// Bytes of the look-ahead / accept arrays (after the header), without / with M.
+__host__ __device__ inline size_t qmcd_smem_base_bytes(int N, int K, int S, bool with_M) {
     size_t ns = (size_t)(N + S - 1) / S + 1;
     size_t b = 0;
-    b += qmcd_align16(ns * 8) * 2;                 // rs, vs
-    b += qmcd_align16((size_t)S * (2 * K + 1) * 8);  // part
-    b += qmcd_align16((size_t)K * 8) * 4;          // pf qf cf rf
-    b += qmcd_align16((size_t)QMCD_WARPS * K * 8); // Ts
+    b += qmcd_align16(ns * 8) * 2;                             // rs, vs
+    b += qmcd_align16((size_t)2 * S * qmcd_PL(K) * 8);           // part
+    b += qmcd_align16((size_t)K * 8) * 4;                      // pf qf cf rf
+    b += qmcd_align16((size_t)QMCD_WARPS * K * 8);             // Ts
+    b += qmcd_align16((size_t)K * 4);                          // Js
+    if (with_M) b += qmcd_align16((size_t)K * qmcd_ldM(K) * 8);  // Ms
     return qmcd_align16(b);
 }
 
@@ -91,17 +101,19 @@ __device__ inline QmcdSmem qmcd_carve(unsigned char* base, int N, int K, int S) 
     QmcdSmem s;
     size_t ns = (size_t)(N + S - 1) / S + 1;
     unsigned char* p = base;
-    s.red = (double*)p; p += 32 * 8;
-    s.iflag = (int*)p; p += 8 * 4 + 32;
+    s.red = (double*)p; p += 40 * 8;
+    s.iflag = (int*)p; p += 16 * 4;
     s.dyn = p;
     s.rs = (double*)p; p += qmcd_align16(ns * 8);
     s.vs = (double*)p; p += qmcd_align16(ns * 8);
-    s.part = (double*)p; p += qmcd_align16((size_t)S * (2 * K + 1) * 8);
+    s.part = (double*)p; p += qmcd_align16((size_t)2 * S * qmcd_PL(K) * 8);
     s.pf = (double*)p; p += qmcd_align16((size_t)K * 8);
     s.qf = (double*)p; p += qmcd_align16((size_t)K * 8);
     s.cf = (double*)p; p += qmcd_align16((size_t)K * 8);
     s.rf = (double*)p; p += qmcd_align16((size_t)K * 8);
     s.Ts = (double*)p; p += qmcd_align16((size_t)QMCD_WARPS * K * 8);
+    s.Js = (int*)p; p += qmcd_align16((size_t)K * 4);
+    s.Ms = (double*)p;
     return s;
 }
 

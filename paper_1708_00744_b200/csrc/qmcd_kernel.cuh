@@ -5,10 +5,13 @@
 #include "qmcd_flush_mma.cuh"
 
 // Flush wrapper: all CTAs of the cluster call it with the same m > 0.
+// M goes back to global memory first (the flush reads it from there).
 // Barriers: (entry) queue slots / M written by other CTAs become visible;
 // (exit) nobody restages slot 0 or reads B rows before every CTA is done.
+template <bool MS>
 __device__ void qmcd_flush_phase(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
                                  const QmcdWalker& w, int m) {
+    qmcd_writeback_M<MS>(P, s, w, m);
     if (P.S > 1) cl.sync(); else __syncthreads();
     if (qmcd_flush_use_mma(P, m)) qmcd_flush_mma(P, s, cl, w, m);
     else qmcd_flush_simt(P, s, cl, w, m);
@@ -19,30 +22,119 @@ __device__ void qmcd_flush_phase(const QmcdDev& P, const QmcdSmem& s, cg::cluste
     if (P.S > 1) cl.sync(); else __syncthreads();
 }
 
-// Is electron j already queued?  (uniform over the cluster: J, m are stable here)
-__device__ inline bool qmcd_in_queue(const QmcdWalker& w, int j, int m) {
-    for (int i = 0; i < m; ++i)
-        if (__ldcg(w.J + i) == j) return true;
-    return false;
-}
-
 // Accept path shared by ACCEPT and SWEEP.  Called by ALL CTAs with the same
-// (j, m, R); pf/cf valid in the leader.  Returns the new m.
+// (j, m, R, inq) and cf / rf valid in every CTA.  Returns the new m.
+template <bool MS>
 __device__ int qmcd_do_accept(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
-                              const QmcdWalker& w, int j, int m, double R, bool leader_has_R) {
-    if (m > 0 && qmcd_in_queue(w, j, m)) {
+                              const QmcdWalker& w, int j, int m, double R, bool inq, int& pbuf) {
+    if (inq) {
         // repeated electron inside one window (G7): flush, then the move
         // is re-evaluated against the fresh inverse (m = 0) and queued.  Its v sits
-        // in slot m of C (staged by the ratio phase); slot 0 is free after the flush.
-        qmcd_flush_phase(P, s, cl, w, m);
-        double R2 = qmcd_ratio_phase(P, s, cl, w, j, 0, w.C + (size_t)m * P.N);
-        if (w.r == 0) R = R2;
+        // in slot m of C (staged by the look-ahead); slot 0 is free after the flush.
+        qmcd_flush_phase<MS>(P, s, cl, w, m);
+        R = qmcd_lookahead<MS>(P, s, cl, w, j, 0, w.C + (size_t)m * P.N, pbuf, nullptr);
         m = 0;
     }
-    if (w.r == 0) qmcd_accept_update(P, s, w, j, m, R);
+    if (!MS && P.S > 1) cl.sync();     // global M: nobody may still be reading it
+    qmcd_accept_update<MS>(P, s, w, j, m, R);
     m += 1;
-    if (m == P.K) { qmcd_flush_phase(P, s, cl, w, m); m = 0; }
+    if (m == P.K) { qmcd_flush_phase<MS>(P, s, cl, w, m); m = 0; }
     return m;
+}
+
+template <bool MS>
+__device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group& cl,
+                         const QmcdWalker& w) {
+    const QmcdDev& P = A.P;
+    const int S = P.S, r = w.r, b = w.b, tid = threadIdx.x;
+    int m = __ldcg(P.m + b);   // written by the leader only at the end of a launch or inside a flush
+    int pbuf = 0;
+
+    if (A.mode == QMCD_MODE_RATIO) {
+        int j = A.jv ? A.jv[b] : A.j;
+        if (j < 0 || j >= P.N) {
+            if (r == 0 && tid == 0) { qmcd_set_status(P, QMCD_DEV_EINVAL, b, P.counters[(size_t)b * 2]); P.sj[b] = -1; A.R_out[b] = 0.0; }
+            return;   // uniform over the cluster
+        }
+        qmcd_load_state<MS>(P, s, w, m);
+        double R = qmcd_lookahead<MS>(P, s, cl, w, j, m, A.v + (size_t)b * P.N, pbuf, nullptr);
+        if (r == 0) {
+            for (int i = tid; i < m; i += QMCD_THREADS) { P.sc[(size_t)b * P.K + i] = s.cf[i]; P.sr[(size_t)b * P.K + i] = s.rf[i]; }
+            if (tid == 0) { P.sR[b] = R; P.sj[b] = j; A.R_out[b] = R; }
+        }
+        return;
+    }
+
+    if (A.mode == QMCD_MODE_ACCEPT) {
+        const int j = __ldcg(P.sj + b);
+        if (j < 0) return;
+        const double R = __ldcg(P.sR + b);
+        // every CTA has read the staged proposal before the leader clears it
+        if (S > 1) cl.sync();
+        bool acc;
+        if (A.uniforms) { double pa = fmin(1.0, R * R); acc = A.uniforms[b] < pa; }
+        else acc = A.accept_all || (A.mask[b] != 0);
+        if (acc && (R == 0.0 || !isfinite(R))) {
+            if (r == 0 && tid == 0) qmcd_set_status(P, QMCD_DEV_ESINGULAR, b, P.counters[(size_t)b * 2]);
+            acc = false;
+        }
+        if (r == 0 && tid == 0) {
+            if (A.acc_out) A.acc_out[b] = acc ? 1 : 0;
+            P.sj[b] = -1;
+        }
+        if (!acc) return;
+        qmcd_load_state<MS>(P, s, w, m);
+        bool inq = false;
+        for (int i = tid; i < m; i += QMCD_THREADS) {
+            s.cf[i] = __ldcg(P.sc + (size_t)b * P.K + i); s.rf[i] = __ldcg(P.sr + (size_t)b * P.K + i);
+        }
+        for (int i = 0; i < m; ++i) inq |= (s.Js[i] == j);
+        __syncthreads();
+        m = qmcd_do_accept<MS>(P, s, cl, w, j, m, R, inq, pbuf);
+        qmcd_writeback_M<MS>(P, s, w, m);
+        if (r == 0 && tid == 0) P.m[b] = m;
+        return;
+    }
+
+    if (A.mode == QMCD_MODE_FLUSH) {
+        if (m > 0) qmcd_flush_phase<false>(P, s, cl, w, m);   // M is in global memory between launches
+        return;
+    }
+
+    // ---- QMCD_MODE_SWEEP: the whole move loop, no host round trip, one cluster
+    // barrier per move (inside the look-ahead); every CTA decides for itself.
+    qmcd_load_state<MS>(P, s, w, m);
+    const int len = w.khi - w.klo;
+    for (int t = 0; t < A.n_moves; ++t) {
+        const int j = (A.j_begin + t) % P.N;
+        const size_t tb = (size_t)t * P.batch + b;
+        // decision input and next move's operands: get them moving towards L2 early
+        double u = 0.0; unsigned char mk = 0;
+        if (A.uniforms) u = A.uniforms[tb]; else mk = A.mask[tb];
+        if (t + 1 < A.n_moves) {
+            const int jn = (j + 1 == P.N) ? 0 : j + 1;
+            for (int k = tid * 16; k < len; k += QMCD_THREADS * 16) {
+                qmcd_prefetch_l2(A.v + (tb + P.batch) * P.N + w.klo + k);
+                qmcd_prefetch_l2(w.B + (size_t)jn * P.N + w.klo + k);
+            }
+        }
+        bool inq;
+        double R = qmcd_lookahead<MS>(P, s, cl, w, j, m, A.v + tb * P.N, pbuf, &inq);
+        bool acc;
+        if (A.uniforms) { double pa = fmin(1.0, R * R); acc = u < pa; }
+        else acc = mk != 0;
+        if (acc && (R == 0.0 || !isfinite(R))) {
+            if (r == 0 && tid == 0) qmcd_set_status(P, QMCD_DEV_ESINGULAR, b, t);
+            acc = false;
+        }
+        if (r == 0 && tid == 0) {
+            if (A.R_out) A.R_out[tb] = R;
+            if (A.acc_out) A.acc_out[tb] = acc ? 1 : 0;
+        }
+        if (acc) m = qmcd_do_accept<MS>(P, s, cl, w, j, m, R, inq, pbuf);
+    }
+    qmcd_writeback_M<MS>(P, s, w, m);
+    if (r == 0 && tid == 0) { P.sj[b] = -1; P.m[b] = m; }
 }
 
 __global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel(const QmcdArgs A) {
@@ -54,73 +146,6 @@ __global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel(const QmcdArgs A)
     const int b = blockIdx.x / S;
     const QmcdSmem s = qmcd_carve(qmcd_smem_raw, P.N, P.K, S);
     const QmcdWalker w = qmcd_walker(P, b, r);
-    const int tid = threadIdx.x;
-    int m = __ldcg(P.m + b);
-
-    if (A.mode == QMCD_MODE_RATIO) {
-        int j = A.jv ? A.jv[b] : A.j;
-        if (j < 0 || j >= P.N) {
-            if (r == 0 && tid == 0) { qmcd_set_status(P, QMCD_DEV_EINVAL, b, P.counters[(size_t)b * 2]); P.sj[b] = -1; A.R_out[b] = 0.0; }
-            return;   // uniform over the cluster
-        }
-        double R = qmcd_ratio_phase(P, s, cl, w, j, m, A.v + (size_t)b * P.N);
-        if (r == 0) {
-            for (int i = tid; i < m; i += QMCD_THREADS) { P.sp[(size_t)b * P.K + i] = s.pf[i]; P.sc[(size_t)b * P.K + i] = s.cf[i]; }
-            if (tid == 0) { P.sR[b] = R; P.sj[b] = j; A.R_out[b] = R; }
-        }
-        return;
-    }
-
-    if (A.mode == QMCD_MODE_ACCEPT) {
-        const int j = __ldcg(P.sj + b);
-        if (j < 0) return;
-        const double R = __ldcg(P.sR + b);
-        bool acc;
-        if (A.uniforms) { double pa = fmin(1.0, R * R); acc = A.uniforms[b] < pa; }
-        else acc = A.accept_all || (A.mask[b] != 0);
-        if (acc && (R == 0.0 || !isfinite(R))) {
-            if (r == 0 && tid == 0) qmcd_set_status(P, QMCD_DEV_ESINGULAR, b, P.counters[(size_t)b * 2]);
-            acc = false;
-        }
-        if (r == 0 && tid == 0 && A.acc_out) A.acc_out[b] = acc ? 1 : 0;
-        if (!acc) { if (r == 0 && tid == 0) P.sj[b] = -1; return; }
-        if (r == 0) {
-            for (int i = tid; i < m; i += QMCD_THREADS) { s.pf[i] = P.sp[(size_t)b * P.K + i]; s.cf[i] = P.sc[(size_t)b * P.K + i]; }
-            __syncthreads();
-        }
-        qmcd_do_accept(P, s, cl, w, j, m, R, true);
-        return;
-    }
-
-    if (A.mode == QMCD_MODE_FLUSH) {
-        if (m > 0) qmcd_flush_phase(P, s, cl, w, m);
-        return;
-    }
-
-    // ---- QMCD_MODE_SWEEP: the whole move loop, no host round trip.
-    int* flag = s.iflag;                         // leader's decision, broadcast via DSMEM
-    for (int t = 0; t < A.n_moves; ++t) {
-        const int j = (A.j_begin + t) % P.N;
-        const size_t tb = (size_t)t * P.batch + b;
-        double R = qmcd_ratio_phase(P, s, cl, w, j, m, A.v + tb * P.N);
-        if (r == 0 && tid == 0) {
-            bool acc;
-            if (A.uniforms) { double pa = fmin(1.0, R * R); acc = A.uniforms[tb] < pa; }
-            else acc = A.mask[tb] != 0;
-            if (acc && (R == 0.0 || !isfinite(R))) {
-                qmcd_set_status(P, QMCD_DEV_ESINGULAR, b, t);
-                acc = false;
-            }
-            if (A.R_out) A.R_out[tb] = R;
-            if (A.acc_out) A.acc_out[tb] = acc ? 1 : 0;
-            for (int q = 0; q < S; ++q) {
-                int* f = (S > 1) ? cl.map_shared_rank(flag, q) : flag;
-                f[0] = acc ? 1 : 0;
-            }
-        }
-        if (S > 1) cl.sync(); else __syncthreads();
-        const bool acc = flag[0] != 0;
-        if (acc) m = qmcd_do_accept(P, s, cl, w, j, m, R, true);
-    }
-    if (r == 0 && tid == 0) P.sj[b] = -1;
+    if (P.m_in_smem) qmcd_run<true>(A, s, cl, w);
+    else qmcd_run<false>(A, s, cl, w);
 }

@@ -26,32 +26,51 @@ __device__ inline QmcdWalker qmcd_walker(const QmcdDev& P, int b, int r) {
     return w;
 }
 
+// M lives either in every CTA's shared memory (MS = true: s.Ms, row stride K|1,
+// identical copies kept in step by identical arithmetic) or, when K is too large
+// for that, in global memory (w.M, row stride K, written by the leader CTA only).
+template <bool MS> struct QmcdM {
+    static __device__ __forceinline__ const double* base(const QmcdSmem& s, const QmcdWalker& w) { return MS ? s.Ms : w.M; }
+    static __device__ __forceinline__ int ld(int K) { return MS ? qmcd_ldM(K) : K; }
+    static __device__ __forceinline__ double get(const double* p) { return MS ? *p : __ldcg(p); }
+};
+
+__device__ __forceinline__ void qmcd_prefetch_l2(const void* p) {
+    asm volatile("prefetch.global.L2 [%0];" :: "l"(p));
+}
+
 // ---------------------------------------------------------------------------
 // F1: look-ahead ratio (Eqs. 1 and 3).
 //   d = B0[j,:].v ; p_i = B0[j,:].C[i,:] - delta(j,j_i) ; q_a = W[a,:].v
 //   R = d - p^T M q                                   (m = 0: R = d)
-// Every CTA streams its column slice: 2m+2 vectors of length N/S, fully
-// coalesced; partial sums go to the leader CTA's shared memory through DSMEM.
+// Every CTA streams its column slice (2m+2 vectors of length N/S, coalesced) and
+// sends its partial sums to EVERY CTA of the cluster through distributed shared
+// memory; after ONE cluster barrier each CTA reduces them in the same order and
+// finishes the K x K part on its own, so all CTAs hold bit-identical R, c = M q
+// and r = M^T p and take the accept decision without another exchange.
 // The slices of B0[j,:] and v are also written to slot m of W and C -- the slot
-// the move will occupy if accepted -- so accept has nothing left to copy.
-// Returns R in the leader CTA (all threads); other CTAs return 0.
-// Ends with the leader's pf (delta applied), cf = M q valid in ITS smem.
+// the move will occupy if accepted.  `pbuf` is the partial-buffer parity, toggled
+// here.  Returns R in every thread; *inq = (j is already queued).
 // ---------------------------------------------------------------------------
-__device__ double qmcd_ratio_phase(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
-                                   const QmcdWalker& w, int j, int m, const double* __restrict__ v) {
+template <bool MS>
+__device__ double qmcd_lookahead(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
+                                 const QmcdWalker& w, int j, int m, const double* v,
+                                 int& pbuf, bool* inq) {
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int N = P.N, K = P.K, S = P.S;
     const int len = w.khi - w.klo;
-    const int PL = 2 * K + 1;
+    const int PL = qmcd_PL(K);
     const double* rowj = w.B + (size_t)j * N + w.klo;
     const double* vv = v + w.klo;
     double* Wm = w.W + (size_t)m * N + w.klo;
     double* Cm = w.C + (size_t)m * N + w.klo;
+    const int buf = pbuf;
+    pbuf ^= 1;
 
     double dpart = 0.0;
     for (int k = tid; k < len; k += QMCD_THREADS) {
-        double rv = qmcd_ldcg(rowj + k);
-        double xv = vv[k];
+        double rv = __ldcg(rowj + k);
+        double xv = __ldcg(vv + k);
         s.rs[k] = rv; s.vs[k] = xv;
         Wm[k] = rv; Cm[k] = xv;
         dpart += rv * xv;
@@ -60,13 +79,14 @@ __device__ double qmcd_ratio_phase(const QmcdDev& P, const QmcdSmem& s, cg::clus
     if (lane == 0) s.red[wid] = dpart;
     __syncthreads();
 
-    double* lead_part = (S > 1) ? cl.map_shared_rank(s.part, 0) : s.part;
-    double* mine = lead_part + (size_t)w.r * PL;
-    if (tid == 0) {
+    // my partials go to slot [buf][w.r] of every CTA q (lane q of each warp stores)
+    double* dst = nullptr;
+    if (lane < S) dst = ((S > 1) ? cl.map_shared_rank(s.part, lane) : s.part) + ((size_t)buf * S + w.r) * PL;
+    if (wid == 0) {
         double d = 0.0;
 #pragma unroll
         for (int i = 0; i < QMCD_WARPS; ++i) d += s.red[i];
-        mine[2 * K] = d;
+        if (lane < S) dst[2 * K] = d;
     }
     // dots: each warp takes two queue rows at a time (4 independent streams)
     for (int i = wid * 2; i < m; i += QMCD_WARPS * 2) {
@@ -79,50 +99,61 @@ __device__ double qmcd_ratio_phase(const QmcdDev& P, const QmcdSmem& s, cg::clus
 #pragma unroll 4
         for (int k = lane; k < len; k += 32) {
             double rk = s.rs[k], vk = s.vs[k];
-            p0 += rk * qmcd_ldcg(C0 + k);
-            q0 += qmcd_ldcg(W0 + k) * vk;
-            p1 += rk * qmcd_ldcg(C1 + k);
-            q1 += qmcd_ldcg(W1 + k) * vk;
+            p0 += rk * __ldcg(C0 + k);
+            q0 += __ldcg(W0 + k) * vk;
+            p1 += rk * __ldcg(C1 + k);
+            q1 += __ldcg(W1 + k) * vk;
         }
         p0 = qmcd_warp_sum(p0); q0 = qmcd_warp_sum(q0);
         p1 = qmcd_warp_sum(p1); q1 = qmcd_warp_sum(q1);
-        if (lane == 0) {
-            mine[i] = p0; mine[K + i] = q0;
-            if (two) { mine[i + 1] = p1; mine[K + i + 1] = q1; }
+        if (lane < S) {
+            dst[i] = p0; dst[K + i] = q0;
+            if (two) { dst[i + 1] = p1; dst[K + i + 1] = q1; }
         }
     }
     if (S > 1) cl.sync(); else __syncthreads();
-    if (w.r != 0) return 0.0;
 
-    // ---- leader: reduce partials, c = M q, R = d - p.c
+    // ---- every CTA: reduce the S partial vectors in rank order
+    const double* mypart = s.part + (size_t)buf * S * PL;
     for (int i = tid; i < m; i += QMCD_THREADS) {
         double p = 0, q = 0;
-        for (int r = 0; r < S; ++r) { p += s.part[(size_t)r * PL + i]; q += s.part[(size_t)r * PL + K + i]; }
-        if (w.J[i] == j) p -= 1.0;
+        for (int r = 0; r < S; ++r) { p += mypart[(size_t)r * PL + i]; q += mypart[(size_t)r * PL + K + i]; }
+        if (s.Js[i] == j) p -= 1.0;
         s.pf[i] = p; s.qf[i] = q;
     }
-    if (tid == 0) {
-        double d = 0;
-        for (int r = 0; r < S; ++r) d += s.part[(size_t)r * PL + 2 * K];
-        s.red[8] = d;
+    double d = 0;
+    for (int r = 0; r < S; ++r) d += mypart[(size_t)r * PL + 2 * K];
+    __syncthreads();
+    // ---- c = M q and r = M^T p: 8 threads per index x, strided partial sums
+    {
+        const double* Mb = QmcdM<MS>::base(s, w);
+        const int ldM = QmcdM<MS>::ld(K);
+        const int h = tid & 7;
+        for (int x0 = 0; x0 < m; x0 += QMCD_THREADS / 8) {
+            const int x = x0 + (tid >> 3);
+            double ca = 0, ra = 0;
+            if (x < m) {
+                for (int b = h; b < m; b += 8) {
+                    ca += QmcdM<MS>::get(Mb + (size_t)x * ldM + b) * s.qf[b];
+                    ra += s.pf[b] * QmcdM<MS>::get(Mb + (size_t)b * ldM + x);
+                }
+            }
+#pragma unroll
+            for (int o = 4; o > 0; o >>= 1) {
+                ca += __shfl_xor_sync(0xffffffffu, ca, o);
+                ra += __shfl_xor_sync(0xffffffffu, ra, o);
+            }
+            if (x < m && h == 0) { s.cf[x] = ca; s.rf[x] = ra; }
+        }
     }
     __syncthreads();
-    for (int a = wid; a < m; a += QMCD_WARPS) {
-        const double* Ma = w.M + (size_t)a * K;
-        double acc = 0;
-        for (int bb = lane; bb < m; bb += 32) acc += qmcd_ldcg(Ma + bb) * s.qf[bb];
-        acc = qmcd_warp_sum(acc);
-        if (lane == 0) s.cf[a] = acc;
-    }
-    __syncthreads();
-    if (wid == 0) {
-        double acc = 0;
-        for (int a = lane; a < m; a += 32) acc += s.pf[a] * s.cf[a];
-        acc = qmcd_warp_sum(acc);
-        if (lane == 0) s.red[9] = s.red[8] - acc;
-    }
-    __syncthreads();
-    return s.red[9];
+    // ---- every warp: R = d - p.c, and whether j is already queued
+    double acc = 0;
+    bool q_in = false;
+    for (int a = lane; a < m; a += 32) { acc += s.pf[a] * s.cf[a]; q_in |= (s.Js[a] == j); }
+    acc = qmcd_warp_sum(acc);
+    if (inq) *inq = __any_sync(0xffffffffu, q_in);
+    return d - acc;
 }
 
 // ---------------------------------------------------------------------------
@@ -130,37 +161,62 @@ __device__ double qmcd_ratio_phase(const QmcdDev& P, const QmcdSmem& s, cg::clus
 // and Schur complement R = d - p^T M q:
 //   M_new = [[M + sigma c r^T, -sigma c], [-sigma r^T, sigma]],
 //   c = M q, r^T = p^T M, sigma = 1/R.
-// Leader CTA only; pf/cf must be valid in its smem (delta term is zero because
-// the caller flushes first when j is already queued).  C[m], W[m] were staged by
-// the ratio phase.
+// cf / rf must be valid in shared memory (the delta term is zero because the
+// caller flushes first when j is already queued).  C[m], W[m] were staged by the
+// look-ahead.  MS: every CTA updates its own copy; otherwise the leader only.
 // ---------------------------------------------------------------------------
+template <bool MS>
 __device__ void qmcd_accept_update(const QmcdDev& P, const QmcdSmem& s, const QmcdWalker& w,
                                    int j, int m, double R) {
     const int tid = threadIdx.x;
     const int K = P.K;
     const double sigma = 1.0 / R;
-    for (int bb = tid; bb < m; bb += QMCD_THREADS) {
-        double acc = 0;
-        for (int a = 0; a < m; ++a) acc += s.pf[a] * qmcd_ldcg(w.M + (size_t)a * K + bb);
-        s.rf[bb] = acc;
-    }
-    __syncthreads();
-    for (int idx = tid; idx < m * m; idx += QMCD_THREADS) {
-        int a = idx / m, bb = idx - a * m;
-        double* p = w.M + (size_t)a * K + bb;
-        *p = qmcd_ldcg(p) + sigma * s.cf[a] * s.rf[bb];
-    }
-    for (int a = tid; a < m; a += QMCD_THREADS) {
-        w.M[(size_t)a * K + m] = -sigma * s.cf[a];
-        w.M[(size_t)m * K + a] = -sigma * s.rf[a];
+    if (MS || w.r == 0) {
+        double* Mb = MS ? s.Ms : w.M;
+        const int ldM = QmcdM<MS>::ld(K);
+        for (int idx = tid; idx < m * m; idx += QMCD_THREADS) {
+            int a = idx / m, bb = idx - a * m;
+            double* p = Mb + (size_t)a * ldM + bb;
+            *p = QmcdM<MS>::get(p) + sigma * s.cf[a] * s.rf[bb];
+        }
+        for (int a = tid; a < m; a += QMCD_THREADS) {
+            Mb[(size_t)a * ldM + m] = -sigma * s.cf[a];
+            Mb[(size_t)m * ldM + a] = -sigma * s.rf[a];
+        }
+        if (tid == 0) Mb[(size_t)m * ldM + m] = sigma;
     }
     if (tid == 0) {
-        w.M[(size_t)m * K + m] = sigma;
-        w.J[m] = j;
-        P.m[w.b] = m + 1;
-        P.sj[w.b] = -1;
-        P.counters[(size_t)w.b * 2 + 0] += 1;
+        s.Js[m] = j;
+        if (w.r == 0) {
+            w.J[m] = j;
+            P.counters[(size_t)w.b * 2 + 0] += 1;
+        }
     }
+    __syncthreads();
+}
+
+// Leader: copy this walker's M from shared to global memory (before a flush, or
+// at the end of a launch).  No-op when M already lives in global memory.
+template <bool MS>
+__device__ void qmcd_writeback_M(const QmcdDev& P, const QmcdSmem& s, const QmcdWalker& w, int m) {
+    if (!MS || w.r != 0) return;
+    const int K = P.K, ldM = qmcd_ldM(K);
+    for (int idx = threadIdx.x; idx < m * m; idx += QMCD_THREADS) {
+        int a = idx / m, bb = idx - a * m;
+        w.M[(size_t)a * K + bb] = s.Ms[(size_t)a * ldM + bb];
+    }
+}
+
+// Every CTA: load the walker's queue state (J and, if MS, M) into shared memory.
+template <bool MS>
+__device__ void qmcd_load_state(const QmcdDev& P, const QmcdSmem& s, const QmcdWalker& w, int m) {
+    const int K = P.K, ldM = qmcd_ldM(K);
+    for (int i = threadIdx.x; i < m; i += QMCD_THREADS) s.Js[i] = __ldcg(w.J + i);
+    if (MS)
+        for (int idx = threadIdx.x; idx < m * m; idx += QMCD_THREADS) {
+            int a = idx / m, bb = idx - a * m;
+            s.Ms[(size_t)a * ldM + bb] = __ldcg(w.M + (size_t)a * K + bb);
+        }
     __syncthreads();
 }
 
@@ -199,7 +255,7 @@ __device__ void qmcd_flush_simt(const QmcdDev& P, const QmcdSmem& s, cg::cluster
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 double t = qmcd_warp_sum(acc[u]);
-                if (lane == 0 && u < na) Tw[a0 + u] = t - ((w.J[a0 + u] == r) ? 1.0 : 0.0);
+                if (lane == 0 && u < na) Tw[a0 + u] = t - ((__ldcg(w.J + a0 + u) == r) ? 1.0 : 0.0);
             }
         }
         __syncwarp();
