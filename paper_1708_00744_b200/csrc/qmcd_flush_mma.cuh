@@ -25,7 +25,7 @@ __host__ __device__ inline size_t qmcd_flush_mma_smem_bytes(int N, int K) {
 }
 
 __device__ __forceinline__ void qmcd_dmma(double& d0, double& d1, double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                  : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 __device__ __forceinline__ void qmcd_cp_async16(void* smem_dst, const void* gsrc) {
@@ -79,7 +79,7 @@ __device__ __forceinline__ void qmcd_stg128(double* p, double x, double y) {
 // from global memory (16 B per lane, prefetched one k-group ahead), the C chunk
 // is staged once per CTA with cp.async and shared by the 8 warps.
 // ---------------------------------------------------------------------------
-template <int A_T>
+template <int A_T, int NB>
 __device__ void qmcd_mma_nt(const double* Bw, int N, int row0, int nvalid,
                             const double* __restrict__ Cq, const int* __restrict__ Jq, int m,
                             double* __restrict__ Ts, int ldT, double* __restrict__ cb) {
@@ -94,13 +94,14 @@ __device__ void qmcd_mma_nt(const double* Bw, int N, int row0, int nvalid,
         av[a] = r < nvalid;
         ap[a] = Bw + (size_t)(row0 + (av[a] ? r : 0)) * N + 2 * c;
     }
-    for (int col0 = 0; col0 < mp8; col0 += 64) {
-        const int ncols = min(64, mp8 - col0), nb = ncols >> 3;
-        double acc[A_T][8][2];
+    // T is produced NB*8 columns at a time (rows of C past m are staged as zeros)
+    for (int col0 = 0; col0 < mp8; col0 += NB * 8) {
+        constexpr int ncols = NB * 8;
+        double acc[A_T][NB][2];
 #pragma unroll
         for (int a = 0; a < A_T; ++a)
 #pragma unroll
-            for (int b = 0; b < 8; ++b) { acc[a][b][0] = 0.0; acc[a][b][1] = 0.0; }
+            for (int b = 0; b < NB; ++b) { acc[a][b][0] = 0.0; acc[a][b][1] = 0.0; }
         qmcd_stage_chunk<QMCD_MMA_LDC>(cb, Cq, (size_t)N, col0, ncols, m, 0);
         qmcd_cp_async_commit();
         double2 a_next[A_T];
@@ -128,25 +129,26 @@ __device__ void qmcd_mma_nt(const double* Bw, int N, int row0, int nvalid,
                     for (int a = 0; a < A_T; ++a)
                         if (av[a]) a_next[a] = qmcd_ldg128(ap[a] + nk);
                 }
+                // all k-step-0 MMAs, then all k-step-1 MMAs: consecutive DMMAs are independent
+                double2 bv[NB];
 #pragma unroll
-                for (int b = 0; b < 8; ++b) {
-                    if (b < nb) {
-                        const double2 bv = qmcd_lds128(cur + b * 8 * QMCD_MMA_LDC + 8 * q);
+                for (int b = 0; b < NB; ++b) bv[b] = qmcd_lds128(cur + b * 8 * QMCD_MMA_LDC + 8 * q);
 #pragma unroll
-                        for (int a = 0; a < A_T; ++a) {
-                            qmcd_dmma(acc[a][b][0], acc[a][b][1], a_cur[a].x, bv.x);
-                            qmcd_dmma(acc[a][b][0], acc[a][b][1], a_cur[a].y, bv.y);
-                        }
-                    }
-                }
+                for (int b = 0; b < NB; ++b)
+#pragma unroll
+                    for (int a = 0; a < A_T; ++a) qmcd_dmma(acc[a][b][0], acc[a][b][1], a_cur[a].x, bv[b].x);
+#pragma unroll
+                for (int b = 0; b < NB; ++b)
+#pragma unroll
+                    for (int a = 0; a < A_T; ++a) qmcd_dmma(acc[a][b][0], acc[a][b][1], a_cur[a].y, bv[b].y);
             }
             __syncthreads();
         }
 #pragma unroll
         for (int a = 0; a < A_T; ++a)
 #pragma unroll
-            for (int b = 0; b < 8; ++b)
-                if (b < nb)
+            for (int b = 0; b < NB; ++b)
+                if (col0 + b * 8 < mp8)
                     *reinterpret_cast<double2*>(Ts + (size_t)(wid * 8 * A_T + a * 8 + g) * ldT + col0 + b * 8 + 2 * c) =
                         make_double2(-acc[a][b][0], -acc[a][b][1]);
     }
@@ -222,18 +224,26 @@ __device__ void qmcd_mma_nn(const double* __restrict__ Ts, int ldT, int kext,
                 double2 avv[A_T];
 #pragma unroll
                 for (int a = 0; a < A_T; ++a) avv[a] = qmcd_lds128(tp[a] + kb * 64 + 8 * q);
+                double2 x0[4], x1[4];
 #pragma unroll
                 for (int G = 0; G < 4; ++G) {
-                    const double2 x0 = qmcd_lds128(cur + (8 * q) * QMCD_MMA_LDX + 16 * G);
-                    const double2 x1 = qmcd_lds128(cur + (8 * q + 1) * QMCD_MMA_LDX + 16 * G);
+                    x0[G] = qmcd_lds128(cur + (8 * q) * QMCD_MMA_LDX + 16 * G);
+                    x1[G] = qmcd_lds128(cur + (8 * q + 1) * QMCD_MMA_LDX + 16 * G);
+                }
+#pragma unroll
+                for (int G = 0; G < 4; ++G)
 #pragma unroll
                     for (int a = 0; a < A_T; ++a) {
-                        qmcd_dmma(acc[a][G][0][0], acc[a][G][0][1], avv[a].x, x0.x);
-                        qmcd_dmma(acc[a][G][1][0], acc[a][G][1][1], avv[a].x, x0.y);
-                        qmcd_dmma(acc[a][G][0][0], acc[a][G][0][1], avv[a].y, x1.x);
-                        qmcd_dmma(acc[a][G][1][0], acc[a][G][1][1], avv[a].y, x1.y);
+                        qmcd_dmma(acc[a][G][0][0], acc[a][G][0][1], avv[a].x, x0[G].x);
+                        qmcd_dmma(acc[a][G][1][0], acc[a][G][1][1], avv[a].x, x0[G].y);
                     }
-                }
+#pragma unroll
+                for (int G = 0; G < 4; ++G)
+#pragma unroll
+                    for (int a = 0; a < A_T; ++a) {
+                        qmcd_dmma(acc[a][G][0][0], acc[a][G][0][1], avv[a].y, x1[G].x);
+                        qmcd_dmma(acc[a][G][1][0], acc[a][G][1][1], avv[a].y, x1[G].y);
+                    }
             }
             __syncthreads();
         }
@@ -274,7 +284,8 @@ __device__ void qmcd_flush_mma_impl(const QmcdDev& P, const QmcdSmem& s, cg::clu
     // ---- my row slice, R rows at a time:  T = -(B C^T - E_J);  B += T Y
     for (int row0 = w.klo; row0 < w.khi; row0 += R) {
         const int nvalid = min(R, w.khi - row0);
-        qmcd_mma_nt<A_T>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
+        if (mp8 <= 32) qmcd_mma_nt<A_T, 4>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
+        else qmcd_mma_nt<A_T, 8>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
         qmcd_mma_nn<A_T, true>(Ts, ldT, mp8, w.Y, m, N, w.B, row0, nvalid, 0, N, cb);
         __syncthreads();
     }
