@@ -116,7 +116,10 @@ int qmcd_counters(qmcd_handle h, long long* counters_dev);
 
 /* Device-resident run of n_moves proposals with no host round trip (the same
  * ratio -> accept -> flush-when-full sequence, one persistent launch; results
- * equal the call-by-call sequence).  Move t proposes electron
+ * equal the call-by-call sequence -- bit for bit with option "lookahead" = 1,
+ * to rounding (another summation order, and an already-queued electron is
+ * flushed before its block instead of at its accept) with the default blocked
+ * look-ahead, which needs proposals_dev 16-byte aligned).  Move t proposes electron
  * (j_begin + t) mod N with new column proposals_dev[t][b][:].  Exactly one of
  * mask_dev ([n_moves][batch] uint8) / uniforms_dev ([n_moves][batch] fp64,
  * Metropolis u < min(1,R^2)) is non-NULL.  Outputs R_out_dev [n_moves][batch]
@@ -140,9 +143,11 @@ int qmcd_sweep_host(qmcd_handle h, int j_begin, int n_moves,
                     void* staging_dev, size_t staging_bytes);
 size_t qmcd_sweep_host_min_staging(int N, int batch);
 
-/* Tuning / introspection.  key: "cluster" (CTAs per walker, 1..16),
- * "flush_path" (0 auto, 1 CUDA-core, 2 DMMA), "threads".  get returns the
- * value (>= 0) or a negative error. */
+/* Tuning / introspection.  set: "cluster" (CTAs per walker, 1..16), "flush_path"
+ * (0 auto, 1 CUDA-core, 2 DMMA), "lookahead" (qmcd_sweep: 0 auto = blocked
+ * look-ahead when the shape allows, 1 = per move, the arithmetic of the per-call
+ * API).  get: those plus "threads", "smem_bytes", "m_in_smem", "blocked_ok".
+ * get returns the value (>= 0) or a negative error. */
 int qmcd_set_option(qmcd_handle h, const char* key, int value);
 int qmcd_get_option(qmcd_handle h, const char* key);
 

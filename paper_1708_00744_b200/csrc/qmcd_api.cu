@@ -21,6 +21,7 @@ struct qmcd_ctx {
     bool has_inverse;
     size_t smem_bytes;
     int max_cluster;          // largest cluster size the device can co-schedule
+    int lookahead;            // qmcd_sweep: 0 auto (blocked when possible), 1 per move
     char last_cuda_error[256];
 };
 
@@ -77,9 +78,13 @@ static int default_cluster(int N, int batch, int sms, int max_cluster) {
 
 static int configure_kernel(qmcd_ctx* h, int S) {
     const size_t cap = 227 * 1024;
-    size_t base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true);
-    h->P.m_in_smem = 1;
-    if (base > cap) { base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, false); h->P.m_in_smem = 0; }
+    // blocked look-ahead: 16-byte vector access to every slice, <= 40 output tiles
+    const bool blk_shape = h->N >= QMCD_TB && (h->N % (8 * S) == 0) && (2 * ((h->K + 7) / 8) + 2 <= 8 * QMCD_BLK_MAXU);
+    const size_t blk = blk_shape ? qmcd_blk_smem_bytes(h->K) : 0;
+    size_t base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, blk);
+    h->P.m_in_smem = 1; h->P.blk_ok = blk_shape ? 1 : 0;
+    if (base > cap) { base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, 0); h->P.blk_ok = 0; }
+    if (base > cap) { base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, false, 0); h->P.m_in_smem = 0; }
     const size_t mma = QMCD_SMEM_HEADER + qmcd_flush_mma_smem_bytes(h->N, h->K);
     if (base > cap) { snprintf(g_last_error, sizeof(g_last_error), "shared memory need %zu > 227 KB", base); return QMCD_EINVAL; }
     h->P.mma_smem_ok = (mma <= cap) ? 1 : 0;
@@ -300,6 +305,7 @@ extern "C" int qmcd_sweep(qmcd_handle h, int j_begin, int n_moves,
     QmcdArgs a = base_args(h, QMCD_MODE_SWEEP);
     a.j_begin = j_begin; a.n_moves = n_moves; a.v = proposals_dev;
     a.mask = mask_dev; a.uniforms = uniforms_dev; a.R_out = R_out_dev; a.acc_out = acc_out_dev;
+    a.blocked = (h->lookahead != 1 && h->P.blk_ok && h->P.m_in_smem && (((uintptr_t)proposals_dev & 15) == 0)) ? 1 : 0;
     return launch(h, a);
 }
 
@@ -365,6 +371,11 @@ extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
         h->P.flush_path = value;
         return QMCD_OK;
     }
+    if (!strcmp(key, "lookahead")) {
+        if (value < 0 || value > 1) return QMCD_EINVAL;
+        h->lookahead = value;
+        return QMCD_OK;
+    }
     return QMCD_EINVAL;
 }
 
@@ -372,6 +383,9 @@ extern "C" int qmcd_get_option(qmcd_handle h, const char* key) {
     if (!h || !key) return QMCD_EINVAL;
     if (!strcmp(key, "cluster")) return h->P.S;
     if (!strcmp(key, "flush_path")) return h->P.flush_path;
+    if (!strcmp(key, "lookahead")) return h->lookahead;
+    if (!strcmp(key, "blocked_ok")) return h->P.blk_ok && h->P.m_in_smem;
+    if (!strcmp(key, "m_in_smem")) return h->P.m_in_smem;
     if (!strcmp(key, "threads")) return QMCD_THREADS;
     if (!strcmp(key, "smem_bytes")) return (int)h->smem_bytes;
     return QMCD_EINVAL;

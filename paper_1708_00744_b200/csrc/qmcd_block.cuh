@@ -1,0 +1,347 @@
+// qmcd_block.cuh -- blocked look-ahead for qmcd_sweep (pre-staged proposals).
+//
+// Inside one window (between two flushes) the stale inverse B0 is fixed, so every
+// quantity the look-ahead of Eq. 3 needs for the next L
+// proposals t0..t0+L-1 is an entry of three small products over the long axis N:
+//     P[tl][i]  = B0[j_tl,:] . C[i,:]      (L x m0)   -> p of move tl, queued part
+//     Q[tl][i]  = W[i,:]     . v_tl        (L x m0)   -> q of move tl, queued part
+//     D[sl][tl] = B0[j_sl,:] . v_tl        (L x L)    -> d = D[tl][tl]; p, q against
+//                                                        moves accepted inside the block
+// They are computed ONCE per block with DMMA (each CTA on its column slice),
+// summed over the cluster by a reduce-scatter + all-gather through distributed
+// shared memory (two cluster barriers per BLOCK instead of one per move), and the
+// per-move chain (c = M q, r = M^T p, R, decision, bordering of M) then runs out
+// of shared memory alone, replicated in every CTA.  The arithmetic per entry is
+// the same dot product the per-call path computes; only the summation order
+// differs.  Accepted moves are appended to the queue (C, W, J) at the block's end.
+#pragma once
+// (included by qmcd_kernel.cuh after qmcd_flush_phase is defined)
+
+#define QMCD_TB 16              // proposals per block
+#define QMCD_BLK_KC 64          // columns per staged chunk of the left operands
+#define QMCD_BLK_LDA 72         // its row stride (== 8 mod 16 doubles)
+#define QMCD_BLK_MAXU 5         // units (8-column output tiles) per warp: 2*ceil(K/8)+2 <= 40
+
+__host__ __device__ inline int qmcd_blk_Kp(int K) { return (K + 7) & ~7; }
+__host__ __device__ inline int qmcd_blk_RL(int K) { return 2 * qmcd_blk_Kp(K) + QMCD_TB; }
+// As[2][32][LDA] | recv[16][RL] | G[16][RL] | pq[2][2][Kp] | ub[16]
+__host__ __device__ inline size_t qmcd_blk_smem_bytes(int K) {
+    return ((size_t)2 * 32 * QMCD_BLK_LDA + (size_t)2 * QMCD_TB * qmcd_blk_RL(K) + 4 * (size_t)qmcd_blk_Kp(K) + 16) * 8;
+}
+
+struct QmcdBlk {
+    double* As;     // [2][32][LDA]  rows 0..15: B0[j_tl, chunk], rows 16..31: v_tl[chunk]
+    double* recv;   // [S][RPO][RL]  partial strips of the rows this CTA reduces
+    double* G;      // [16][RL]      reduced strips: P | Q | D
+    double* pq;     // [2][2][Kp]    p, q of the current move, double buffered by move parity
+    double* ub;     // [16]          decision inputs of the block (uniform or mask as 0/1)
+};
+
+__device__ inline QmcdBlk qmcd_blk_carve(double* base, int K) {
+    QmcdBlk x;
+    const int RL = qmcd_blk_RL(K);
+    x.As = base; base += 2 * 32 * QMCD_BLK_LDA;
+    x.recv = base; base += QMCD_TB * RL;
+    x.G = base; base += QMCD_TB * RL;
+    x.pq = base; base += 4 * qmcd_blk_Kp(K);
+    x.ub = base;
+    return x;
+}
+
+__device__ __forceinline__ double2 qmcd_ldcg128(const double* p) {
+    double2 v;
+    asm volatile("ld.global.cg.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p) : "memory");
+    return v;
+}
+
+// Stage chunk kc (columns [klo + 64 kc, + cw)) of the block's left operands:
+// rows 0..15 = B0[j_tl, :], rows 16..31 = v_tl, tl < L (rows >= L are zeroed).
+__device__ __forceinline__ void qmcd_blk_stage(double* dst, const QmcdArgs& A, const QmcdWalker& w,
+                                               int t0, int L, int kc, int cw) {
+    const QmcdDev& P = A.P;
+    const int N = P.N;
+    const int vpr = cw >> 1;                       // 16-byte vectors per row
+    for (int idx = threadIdx.x; idx < 32 * vpr; idx += QMCD_THREADS) {
+        const int row = idx / vpr, c2 = (idx - row * vpr) * 2;
+        const int tl = row & 15;
+        double* d = dst + row * QMCD_BLK_LDA + c2;
+        if (tl < L) {
+            const int col = w.klo + kc * QMCD_BLK_KC + c2;
+            const double* src;
+            if (row < 16) { int j = A.j_begin + t0 + tl; j %= N; src = w.B + (size_t)j * N + col; }
+            else src = A.v + ((size_t)(t0 + tl) * P.batch + w.b) * N + col;
+            qmcd_cp_async16(d, src);
+        } else { d[0] = 0.0; d[1] = 0.0; }
+    }
+}
+
+// Row pointer (at this CTA's column slice) of the RIGHT operand row `row` of unit u:
+//   u <  nP      : C[u*8 + g]        (valid while < m0)
+//   u < 2 nP     : W[(u-nP)*8 + g]   (valid while < m0)
+//   else         : v_{t0 + (u-2nP)*8 + g}  (valid while < L)
+__device__ __forceinline__ const double* qmcd_blk_right(const QmcdArgs& A, const QmcdWalker& w, int u, int nP,
+                                                        int g, int m0, int t0, int L) {
+    const int N = A.P.N;
+    if (u < nP) { const int i = u * 8 + g; return (i < m0) ? w.C + (size_t)i * N + w.klo : nullptr; }
+    if (u < 2 * nP) { const int i = (u - nP) * 8 + g; return (i < m0) ? w.W + (size_t)i * N + w.klo : nullptr; }
+    const int tl = (u - 2 * nP) * 8 + g;
+    return (tl < L) ? A.v + ((size_t)(t0 + tl) * A.P.batch + w.b) * N + w.klo : nullptr;
+}
+
+// ---------------------------------------------------------------------------
+// G strips of one block: DMMA on this CTA's column slice, then the cluster-wide
+// sum.  On return every CTA holds, for tl < 16:
+//   G[tl][i]            = P[tl][i]   i < m0
+//   G[tl][Kp + i]       = Q[tl][i]   i < m0
+//   G[tl][2 Kp + sl]    = D[tl][sl] = B0[j_tl,:] . v_sl
+// ---------------------------------------------------------------------------
+__device__ void qmcd_blk_strips(const QmcdArgs& A, const QmcdSmem& s, const QmcdBlk& x, cg::cluster_group& cl,
+                                const QmcdWalker& w, int t0, int L, int m0) {
+    const QmcdDev& P = A.P;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, g = lane >> 2, c = lane & 3;
+    const int S = P.S, K = P.K, Kp = qmcd_blk_Kp(K), RL = qmcd_blk_RL(K);
+    const int len = w.khi - w.klo;
+    const int nP = (m0 + 7) >> 3, U = 2 * nP + 2;
+    const int nchunks = (len + QMCD_BLK_KC - 1) / QMCD_BLK_KC;
+    // my units: u = wid, wid + 8, ...
+    int nu = 0;
+    const double* rp[QMCD_BLK_MAXU];
+#pragma unroll
+    for (int i = 0; i < QMCD_BLK_MAXU; ++i) {
+        const int u = wid + 8 * i;
+        rp[i] = nullptr;
+        if (u < U) { nu = i + 1; rp[i] = qmcd_blk_right(A, w, u, nP, g, m0, t0, L); }
+    }
+    double acc[QMCD_BLK_MAXU][2][2];
+#pragma unroll
+    for (int i = 0; i < QMCD_BLK_MAXU; ++i) { acc[i][0][0] = acc[i][0][1] = acc[i][1][0] = acc[i][1][1] = 0.0; }
+
+    qmcd_blk_stage(x.As, A, w, t0, L, 0, min(QMCD_BLK_KC, len));
+    qmcd_cp_async_commit();
+    for (int kc = 0; kc < nchunks; ++kc) {
+        const int cw = min(QMCD_BLK_KC, len - kc * QMCD_BLK_KC);
+        if (kc + 1 < nchunks) {
+            qmcd_blk_stage(x.As + ((kc + 1) & 1) * 32 * QMCD_BLK_LDA, A, w, t0, L, kc + 1,
+                           min(QMCD_BLK_KC, len - (kc + 1) * QMCD_BLK_KC));
+            qmcd_cp_async_commit();
+        }
+        // right-operand fragments of this chunk for all my units: straight from L2
+        // (each element is read once per CTA), issued before waiting for the stage
+        const int nq = cw >> 3;
+        const double* cur = x.As + (kc & 1) * 32 * QMCD_BLK_LDA + g * QMCD_BLK_LDA + 2 * c;
+#pragma unroll
+        for (int i = 0; i < QMCD_BLK_MAXU; ++i) {
+            if (i < nu) {
+                const int u = wid + 8 * i;
+                const int left = (u >= nP && u < 2 * nP) ? 16 : 0;      // Q = V x W^T, else B0 rows
+                double2 bv[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q)
+                    bv[q] = (rp[i] != nullptr && q < nq) ? qmcd_ldcg128(rp[i] + kc * QMCD_BLK_KC + 8 * q + 2 * c)
+                                                         : make_double2(0.0, 0.0);
+                if (i == 0) {
+                    if (kc + 1 < nchunks) qmcd_cp_async_wait<1>(); else qmcd_cp_async_wait<0>();
+                    __syncthreads();
+                }
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    if (q < nq) {
+                        const double2 a0 = qmcd_lds128(cur + (left + 0) * QMCD_BLK_LDA + 8 * q);
+                        const double2 a1 = qmcd_lds128(cur + (left + 8) * QMCD_BLK_LDA + 8 * q);
+                        qmcd_dmma(acc[i][0][0], acc[i][0][1], a0.x, bv[q].x);
+                        qmcd_dmma(acc[i][1][0], acc[i][1][1], a1.x, bv[q].x);
+                        qmcd_dmma(acc[i][0][0], acc[i][0][1], a0.y, bv[q].y);
+                        qmcd_dmma(acc[i][1][0], acc[i][1][1], a1.y, bv[q].y);
+                    }
+                }
+            } else if (i == 0) {
+                if (kc + 1 < nchunks) qmcd_cp_async_wait<1>(); else qmcd_cp_async_wait<0>();
+                __syncthreads();
+            }
+        }
+        __syncthreads();
+    }
+
+    // ---- reduce-scatter: strip row `row` is summed by CTA (row % S); every CTA
+    // sends its partial of that row to slot [my rank][row / S] of the owner's recv
+    const int RPO = (QMCD_TB + S - 1) / S;
+#pragma unroll
+    for (int i = 0; i < QMCD_BLK_MAXU; ++i) {
+        if (i < nu) {
+            const int u = wid + 8 * i;
+            const int off = (u < nP) ? u * 8 : (u < 2 * nP) ? Kp + (u - nP) * 8 : 2 * Kp + (u - 2 * nP) * 8;
+#pragma unroll
+            for (int a = 0; a < 2; ++a) {
+                const int row = a * 8 + g;
+                const int owner = row % S;
+                double* rb = (S > 1) ? cl.map_shared_rank(x.recv, owner) : x.recv;
+                *reinterpret_cast<double2*>(rb + ((size_t)w.r * RPO + row / S) * RL + off + 2 * c) =
+                    make_double2(acc[i][a][0], acc[i][a][1]);
+            }
+        }
+    }
+    if (S > 1) cl.sync(); else __syncthreads();
+    // ---- owner: sum the S partials in rank order, all-gather the result into every CTA's G
+    {
+        const int ncol = 2 * nP * 8 + QMCD_TB;            // active columns: P | Q | D
+        for (int idx = tid; idx < RPO * ncol; idx += QMCD_THREADS) {
+            const int rl = idx / ncol, ci = idx - rl * ncol;
+            const int row = rl * S + w.r;
+            if (row >= QMCD_TB) continue;
+            const int col = (ci < nP * 8) ? ci : (ci < 2 * nP * 8) ? Kp + (ci - nP * 8) : 2 * Kp + (ci - 2 * nP * 8);
+            double v = 0.0;
+            for (int r = 0; r < S; ++r) v += x.recv[((size_t)r * RPO + rl) * RL + col];
+            for (int q = 0; q < S; ++q) {
+                double* gb = (S > 1) ? cl.map_shared_rank(x.G, q) : x.G;
+                gb[(size_t)row * RL + col] = v;
+            }
+        }
+    }
+    if (S > 1) cl.sync(); else __syncthreads();
+}
+
+// ---------------------------------------------------------------------------
+// The sweep loop in blocks (M in shared memory, replicated in every CTA).
+// Returns the queue length at the end.  Every CTA of the cluster runs the same
+// code on the same reduced numbers, so decisions agree without communication.
+// ---------------------------------------------------------------------------
+__device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group& cl,
+                                  const QmcdWalker& w, int m) {
+    const QmcdDev& P = A.P;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int N = P.N, K = P.K, Kp = qmcd_blk_Kp(K), RL = qmcd_blk_RL(K), ldM = qmcd_ldM(K);
+    const int len = w.khi - w.klo;
+    const QmcdBlk x = qmcd_blk_carve(s.rs, K);
+    int t = 0;
+    while (t < A.n_moves) {
+        const int j0 = (A.j_begin + t) % N;
+        int L = min(min(QMCD_TB, K - m), A.n_moves - t);
+        // an electron already queued may not be proposed inside a block (G7):
+        // cut the block before it, or flush first when it is the block's first move
+        {
+            bool hit = false;
+            for (int i = tid; i < m; i += QMCD_THREADS) { int dj = s.Js[i] - j0; if (dj < 0) dj += N; hit |= (dj < L); }
+            if (__syncthreads_or(hit)) {
+                if (tid == 0) {
+                    int lh = L;
+                    for (int i = 0; i < m; ++i) { int dj = s.Js[i] - j0; if (dj < 0) dj += N; lh = min(lh, dj); }
+                    s.iflag[0] = lh;
+                }
+                __syncthreads();
+                L = s.iflag[0];
+                __syncthreads();
+                if (L == 0) { qmcd_flush_phase<true>(P, s, cl, w, m); m = 0; continue; }
+            }
+        }
+        if (tid < L) {
+            const size_t tb = (size_t)(t + tid) * P.batch + w.b;
+            x.ub[tid] = A.uniforms ? A.uniforms[tb] : (A.mask[tb] ? 1.0 : 0.0);
+        }
+        // next block's operands: get them moving towards L2
+        for (int idx = tid; idx < QMCD_TB * ((len + 15) >> 4); idx += QMCD_THREADS) {
+            const int tl = idx / ((len + 15) >> 4), k = (idx - tl * ((len + 15) >> 4)) << 4;
+            const int tn = t + L + tl;
+            if (tn < A.n_moves) {
+                qmcd_prefetch_l2(A.v + ((size_t)tn * P.batch + w.b) * N + w.klo + k);
+                qmcd_prefetch_l2(w.B + (size_t)((A.j_begin + tn) % N) * N + w.klo + k);
+            }
+        }
+        qmcd_blk_strips(A, s, x, cl, w, t, L, m);
+
+        const int m0 = m;
+        unsigned accmask = 0;
+        int na = 0;
+        for (int tl = 0; tl < L; ++tl) {
+            const int mc = m0 + na;
+            const int j = (j0 + tl) % N;
+            const double* Grow = x.G + (size_t)tl * RL;
+            double* pf = x.pq + (size_t)(tl & 1) * 2 * Kp;
+            double* qf = pf + Kp;
+            // p, q of this move from the strips
+            for (int i = tid; i < mc; i += QMCD_THREADS) {
+                double p, q;
+                if (i < m0) { p = Grow[i]; q = Grow[Kp + i]; }
+                else {
+                    const int al = __fns(accmask, 0, i - m0 + 1);
+                    p = Grow[2 * Kp + al];
+                    q = x.G[(size_t)al * RL + 2 * Kp + tl];
+                }
+                pf[i] = p; qf[i] = q;
+            }
+            const double d = Grow[2 * Kp + tl];
+            __syncthreads();
+            // c = M q, r = M^T p
+            {
+                const int h = tid & 7;
+                for (int x0 = 0; x0 < mc; x0 += QMCD_THREADS / 8) {
+                    const int xx = x0 + (tid >> 3);
+                    double ca = 0, ra = 0;
+                    if (xx < mc) {
+                        for (int b = h; b < mc; b += 8) {
+                            ca += s.Ms[(size_t)xx * ldM + b] * qf[b];
+                            ra += pf[b] * s.Ms[(size_t)b * ldM + xx];
+                        }
+                    }
+#pragma unroll
+                    for (int o = 4; o > 0; o >>= 1) {
+                        ca += __shfl_xor_sync(0xffffffffu, ca, o);
+                        ra += __shfl_xor_sync(0xffffffffu, ra, o);
+                    }
+                    if (xx < mc && h == 0) { s.cf[xx] = ca; s.rf[xx] = ra; }
+                }
+            }
+            __syncthreads();
+            double sum = 0;
+            for (int a = lane; a < mc; a += 32) sum += pf[a] * s.cf[a];
+            sum = qmcd_warp_sum(sum);
+            const double R = d - sum;
+            bool acc;
+            if (A.uniforms) { const double pa = fmin(1.0, R * R); acc = x.ub[tl] < pa; }
+            else acc = x.ub[tl] != 0.0;
+            if (acc && (R == 0.0 || !isfinite(R))) {
+                if (w.r == 0 && tid == 0) qmcd_set_status(P, QMCD_DEV_ESINGULAR, w.b, t + tl);
+                acc = false;
+            }
+            if (w.r == 0 && tid == 0) {
+                const size_t tb = (size_t)(t + tl) * P.batch + w.b;
+                if (A.R_out) A.R_out[tb] = R;
+                if (A.acc_out) A.acc_out[tb] = acc ? 1 : 0;
+            }
+            if (acc) {
+                const double sigma = 1.0 / R;
+                for (int idx = tid; idx < mc * mc; idx += QMCD_THREADS) {
+                    const int a = idx / mc, bb = idx - a * mc;
+                    s.Ms[(size_t)a * ldM + bb] += sigma * s.cf[a] * s.rf[bb];
+                }
+                for (int a = tid; a < mc; a += QMCD_THREADS) {
+                    s.Ms[(size_t)a * ldM + mc] = -sigma * s.cf[a];
+                    s.Ms[(size_t)mc * ldM + a] = -sigma * s.rf[a];
+                }
+                if (tid == 0) { s.Ms[(size_t)mc * ldM + mc] = sigma; s.Js[mc] = j; }
+                accmask |= 1u << tl;
+                na += 1;
+            }
+        }
+        // ---- append the block's accepted moves to the queue: C[slot] = v, W[slot] = B0[j,:]
+        {
+            const int vpr = len >> 1;
+            for (int idx = tid; idx < na * vpr; idx += QMCD_THREADS) {
+                const int e = idx / vpr, k = (idx - e * vpr) * 2;
+                const int al = __fns(accmask, 0, e + 1);
+                const double2 vv = qmcd_ldcg128(A.v + ((size_t)(t + al) * P.batch + w.b) * N + w.klo + k);
+                const double2 bb = qmcd_ldcg128(w.B + (size_t)((j0 + al) % N) * N + w.klo + k);
+                qmcd_stg128(w.C + (size_t)(m0 + e) * N + w.klo + k, vv.x, vv.y);
+                qmcd_stg128(w.W + (size_t)(m0 + e) * N + w.klo + k, bb.x, bb.y);
+            }
+            if (w.r == 0) {
+                for (int e = tid; e < na; e += QMCD_THREADS) w.J[m0 + e] = (j0 + (int)__fns(accmask, 0, e + 1)) % N;
+                if (tid == 0) P.counters[(size_t)w.b * 2 + 0] += na;
+            }
+        }
+        m = m0 + na;
+        t += L;
+        __syncthreads();
+        if (m == K) { qmcd_flush_phase<true>(P, s, cl, w, m); m = 0; }
+    }
+    return m;
+}

@@ -36,6 +36,7 @@ struct QmcdDev {
     int flush_path;           // 0 auto, 1 CUDA-core, 2 DMMA
     int mma_smem_ok;          // host: the DMMA flush's shared memory fits
     int m_in_smem;            // host: every CTA keeps its own copy of M in shared memory
+    int blk_ok;               // host: qmcd_sweep may use the blocked look-ahead (qmcd_block.cuh)
 };
 
 enum QmcdMode { QMCD_MODE_RATIO = 0, QMCD_MODE_ACCEPT = 1, QMCD_MODE_FLUSH = 2, QMCD_MODE_SWEEP = 3 };
@@ -55,6 +56,7 @@ struct QmcdArgs {
     int accept_all;
     // SWEEP: v/mask/uniforms/R_out/acc_out are [n_moves][batch]...
     int j_begin, n_moves;
+    int blocked;                  // SWEEP: use the blocked look-ahead
 };
 
 // Shared-memory carving; every CTA of the cluster has the same layout: a small
@@ -84,36 +86,41 @@ __host__ __device__ inline int qmcd_ldM(int K) { return K | 1; }
 
 #define QMCD_SMEM_HEADER (40 * 8 + 16 * 4)      // red[40], iflag[16]; multiple of 16
 
-// Bytes of the look-ahead / accept arrays (after the header), without / with M.
-__host__ __device__ inline size_t qmcd_smem_base_bytes(int N, int K, int S, bool with_M) {
-    size_t ns = (size_t)(N + S - 1) / S + 1;
+// Bytes after the header: fixed arrays (pf qf cf rf Ts Js [Ms]) followed by a
+// union of the per-move look-ahead arrays (rs vs part) and the blocked
+// look-ahead's area (blk_bytes, 0 when unused).
+__host__ __device__ inline size_t qmcd_smem_fixed_bytes(int K, bool with_M) {
     size_t b = 0;
-    b += qmcd_align16(ns * 8) * 2;                             // rs, vs
-    b += qmcd_align16((size_t)2 * S * qmcd_PL(K) * 8);           // part
     b += qmcd_align16((size_t)K * 8) * 4;                      // pf qf cf rf
     b += qmcd_align16((size_t)QMCD_WARPS * K * 8);             // Ts
     b += qmcd_align16((size_t)K * 4);                          // Js
     if (with_M) b += qmcd_align16((size_t)K * qmcd_ldM(K) * 8);  // Ms
-    return qmcd_align16(b);
+    return b;
+}
+__host__ __device__ inline size_t qmcd_smem_base_bytes(int N, int K, int S, bool with_M, size_t blk_bytes) {
+    size_t ns = (size_t)(N + S - 1) / S + 1;
+    size_t u = qmcd_align16(ns * 8) * 2 + qmcd_align16((size_t)2 * S * qmcd_PL(K) * 8);   // rs, vs, part
+    if (blk_bytes > u) u = blk_bytes;
+    return qmcd_align16(qmcd_smem_fixed_bytes(K, with_M) + u);
 }
 
-__device__ inline QmcdSmem qmcd_carve(unsigned char* base, int N, int K, int S) {
+__device__ inline QmcdSmem qmcd_carve(unsigned char* base, int N, int K, int S, bool with_M) {
     QmcdSmem s;
     size_t ns = (size_t)(N + S - 1) / S + 1;
     unsigned char* p = base;
     s.red = (double*)p; p += 40 * 8;
     s.iflag = (int*)p; p += 16 * 4;
     s.dyn = p;
-    s.rs = (double*)p; p += qmcd_align16(ns * 8);
-    s.vs = (double*)p; p += qmcd_align16(ns * 8);
-    s.part = (double*)p; p += qmcd_align16((size_t)2 * S * qmcd_PL(K) * 8);
     s.pf = (double*)p; p += qmcd_align16((size_t)K * 8);
     s.qf = (double*)p; p += qmcd_align16((size_t)K * 8);
     s.cf = (double*)p; p += qmcd_align16((size_t)K * 8);
     s.rf = (double*)p; p += qmcd_align16((size_t)K * 8);
     s.Ts = (double*)p; p += qmcd_align16((size_t)QMCD_WARPS * K * 8);
     s.Js = (int*)p; p += qmcd_align16((size_t)K * 4);
-    s.Ms = (double*)p;
+    s.Ms = (double*)p; if (with_M) p += qmcd_align16((size_t)K * qmcd_ldM(K) * 8);
+    s.rs = (double*)p; p += qmcd_align16(ns * 8);          // union starts here (blocked area aliases it)
+    s.vs = (double*)p; p += qmcd_align16(ns * 8);
+    s.part = (double*)p;
     return s;
 }
 

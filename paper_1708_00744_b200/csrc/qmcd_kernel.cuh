@@ -22,6 +22,8 @@ __device__ void qmcd_flush_phase(const QmcdDev& P, const QmcdSmem& s, cg::cluste
     if (P.S > 1) cl.sync(); else __syncthreads();
 }
 
+#include "qmcd_block.cuh"
+
 // Accept path shared by ACCEPT and SWEEP.  Called by ALL CTAs with the same
 // (j, m, R, inq) and cf / rf valid in every CTA.  Returns the new m.
 template <bool MS>
@@ -104,6 +106,12 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
     // ---- QMCD_MODE_SWEEP: the whole move loop, no host round trip, one cluster
     // barrier per move (inside the look-ahead); every CTA decides for itself.
     qmcd_load_state<MS>(P, s, w, m);
+    if (MS && A.blocked) {
+        m = qmcd_sweep_blocked(A, s, cl, w, m);
+        qmcd_writeback_M<MS>(P, s, w, m);
+        if (r == 0 && tid == 0) { P.sj[b] = -1; P.m[b] = m; }
+        return;
+    }
     const int len = w.khi - w.klo;
     for (int t = 0; t < A.n_moves; ++t) {
         const int j = (A.j_begin + t) % P.N;
@@ -144,7 +152,7 @@ __global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel(const QmcdArgs A)
     const int S = P.S;
     const int r = (S > 1) ? (int)cl.block_rank() : 0;
     const int b = blockIdx.x / S;
-    const QmcdSmem s = qmcd_carve(qmcd_smem_raw, P.N, P.K, S);
+    const QmcdSmem s = qmcd_carve(qmcd_smem_raw, P.N, P.K, S, P.m_in_smem != 0);
     const QmcdWalker w = qmcd_walker(P, b, r);
     if (P.m_in_smem) qmcd_run<true>(A, s, cl, w);
     else qmcd_run<false>(A, s, cl, w);

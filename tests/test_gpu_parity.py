@@ -24,13 +24,16 @@ def _rel(a, b):
 
 
 def gpu_sweep(qmcd, wl, K, mask=None, uniforms=None, final_flush=True, cluster=None, j_begin=0,
-              flush_path=None):
+              flush_path=None, lookahead=None):
     import torch
     q = qmcd.Qmcd(wl.N, K, wl.batch)
     if cluster is not None:
         q.set_option("cluster", cluster)
     if flush_path is not None:
         q.set_option("flush_path", flush_path)
+    if lookahead is not None:
+        q.set_option("lookahead", lookahead)
+    blocked = bool(q.get_option("blocked_ok")) and q.get_option("lookahead") == 0
     B = _dev(wl.Ainv)
     q.set_inverse(B)
     P = _dev(wl.proposals)
@@ -44,7 +47,7 @@ def gpu_sweep(qmcd, wl, K, mask=None, uniforms=None, final_flush=True, cluster=N
     cnt = q.counters().cpu().numpy()
     pend = q.pending().cpu().numpy()
     out = dict(R=R.cpu().numpy(), acc=acc.cpu().numpy(), B=B.cpu().numpy(), status=st, info=info,
-               counters=cnt, pending=pend, S=q.get_option("cluster"))
+               counters=cnt, pending=pend, S=q.get_option("cluster"), blocked=blocked)
     q.close()
     return out
 
@@ -165,10 +168,50 @@ def test_sweep_equals_call_by_call(qmcd):
     """qmcd_sweep must reproduce the ratio -> accept(mask) sequence (include/qmcd.h)."""
     wl = inputs.make_workload(4, 128, 200, seed=3)
     mask = wl.bernoulli_mask(0.7)
-    a = gpu_sweep(qmcd, wl, 8, mask=mask)
+    a = gpu_sweep(qmcd, wl, 8, mask=mask, lookahead=1)      # per-move look-ahead: same arithmetic
     b = gpu_calls(qmcd, wl, 8, mask)
+    assert not a["blocked"]
     assert np.array_equal(a["R"], b["R"])
     assert np.array_equal(a["B"], b["B"])
+    c = gpu_sweep(qmcd, wl, 8, mask=mask)                   # blocked look-ahead: other summation order
+    assert c["blocked"]
+    assert _rel(c["R"], b["R"]) <= 1e-12
+    assert np.max(np.abs(c["B"] - b["B"])) <= 1e-12
+
+
+@pytest.mark.parametrize("N,K,batch,cluster,p,j_begin", [
+    (128, 16, 2, 1, 0.8, 0),       # one CTA per walker
+    (128, 5, 3, 2, 1.0, 3),        # K not a multiple of 8, every move accepted
+    (256, 40, 2, 4, 0.5, 250),     # wrap-around of the electron index inside a block
+    (512, 96, 2, 4, 0.9, 0),       # 26 output tiles per block
+    (64, 64, 2, 1, 0.3, 0),        # K = N with many rejections: electrons repeat inside a window
+    (48, 24, 2, 2, 0.4, 5),        # ragged chunk (24 columns per CTA), repeats
+    (1024, 32, 2, 16, 0.99, 0),    # 16 CTAs per walker, one strip row per owner
+])
+def test_blocked_lookahead_matches_oracle_and_per_move(qmcd, N, K, batch, cluster, p, j_begin):
+    """qmcd_sweep's blocked look-ahead (qmcd_block.cuh) against the oracle's delayed path and
+    against the per-move look-ahead of the same library."""
+    wl = inputs.make_workload(batch, N, n_moves=3 * N, seed=23)
+    # move t proposes electron (j_begin + t) % N: take the proposal the generator built around
+    # that column (keeps the matrices as well conditioned as in the BASELINE configs)
+    n_moves = 2 * N + 11
+    t = np.arange(n_moves)
+    pick = (t % N + j_begin) % N + N * (t // N)
+    wl.proposals = np.ascontiguousarray(wl.proposals[pick]); wl.uniforms = np.ascontiguousarray(wl.uniforms[pick])
+    wl.n_moves = n_moves
+    mask = wl.bernoulli_mask(p)
+    Bo = wl.Ainv.copy(); Ro, acco, _ = oracle.run(2, Bo, K, wl.proposals, j_begin=j_begin, mask=mask)
+    g = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, j_begin=j_begin)
+    assert g["status"] == 0 and g["S"] == cluster and g["blocked"]
+    assert np.array_equal(g["acc"], acco)
+    assert _rel(g["R"], Ro) <= RTOL_RATIO
+    assert np.max(np.abs(g["B"] - Bo)) <= 1e-10
+    assert np.array_equal(g["counters"][:, 0], mask.sum(axis=0))
+    assert np.all(g["pending"] == 0)
+    pm = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, j_begin=j_begin, lookahead=1)
+    assert not pm["blocked"]
+    assert np.max(np.abs(g["R"] - pm["R"])) <= 1e-11
+    assert np.max(np.abs(g["B"] - pm["B"])) <= 1e-11
 
 
 @pytest.mark.parametrize("K", [1, 16, 32])
