@@ -19,9 +19,11 @@
 __host__ __device__ inline int qmcd_mma_ldT(int K) { return ((K + 15) / 16) * 16 + 8; }
 // rows per tile: 128 (16 per warp) while T fits beside the two chunk buffers, else 64
 __host__ __device__ inline int qmcd_mma_rows(int K) { return (K <= 64) ? 128 : 64; }
+// operand chunks in flight: 3 (prefetch two chunks ahead) while they fit, else 2
+__host__ __device__ inline int qmcd_mma_stages(int K) { return (K <= 128) ? 3 : 2; }
 __host__ __device__ inline size_t qmcd_flush_mma_smem_bytes(int N, int K) {
     (void)N;
-    return (size_t)qmcd_mma_rows(K) * qmcd_mma_ldT(K) * 8 + 2 * (size_t)QMCD_MMA_CHUNK_DOUBLES * 8;
+    return (size_t)qmcd_mma_rows(K) * qmcd_mma_ldT(K) * 8 + qmcd_mma_stages(K) * (size_t)QMCD_MMA_CHUNK_DOUBLES * 8;
 }
 
 __device__ __forceinline__ void qmcd_dmma(double& d0, double& d1, double a, double b) {
@@ -61,6 +63,22 @@ __device__ __forceinline__ void qmcd_stage_chunk(double* __restrict__ dst, const
     }
 }
 
+// Same, but only the warps of group `half` (warps 4*half .. 4*half+3) stage, and only rows
+// [32*half, 32*half + 32): the two warps that share a scheduler stage at different
+// times (start / middle of a chunk's MMAs), so one's copies overlap the other's MMAs.
+template <int LD>
+__device__ __forceinline__ void qmcd_stage_half(double* __restrict__ dst, const double* __restrict__ src,
+                                                size_t ld, int row0, int nrows, int m_valid, int col0, int half) {
+    const int t = threadIdx.x & 127;
+    const int rlo = 32 * half, rhi = min(nrows, rlo + 32);
+    for (int idx = rlo * 32 + t; idx < rhi * 32; idx += 128) {
+        const int i = idx >> 5, c2 = (idx & 31) * 2;
+        double* d = dst + i * LD + c2;
+        if (row0 + i < m_valid) qmcd_cp_async16(d, src + (size_t)(row0 + i) * ld + col0 + c2);
+        else { d[0] = 0.0; d[1] = 0.0; }
+    }
+}
+
 __device__ __forceinline__ double2 qmcd_lds128(const double* p) { return *reinterpret_cast<const double2*>(p); }
 // coherent (never .nc) 16-byte global load / store of B: the same kernel rewrites B
 __device__ __forceinline__ double2 qmcd_ldg128(const double* p) {
@@ -79,7 +97,7 @@ __device__ __forceinline__ void qmcd_stg128(double* p, double x, double y) {
 // from global memory (16 B per lane, prefetched one k-group ahead), the C chunk
 // is staged once per CTA with cp.async and shared by the 8 warps.
 // ---------------------------------------------------------------------------
-template <int A_T, int NB>
+template <int A_T, int NB, int NS>
 __device__ void qmcd_mma_nt(const double* Bw, int N, int row0, int nvalid,
                             const double* __restrict__ Cq, const int* __restrict__ Jq, int m,
                             double* __restrict__ Ts, int ldT, double* __restrict__ cb) {
@@ -102,32 +120,38 @@ __device__ void qmcd_mma_nt(const double* Bw, int N, int row0, int nvalid,
         for (int a = 0; a < A_T; ++a)
 #pragma unroll
             for (int b = 0; b < NB; ++b) { acc[a][b][0] = 0.0; acc[a][b][1] = 0.0; }
-        qmcd_stage_chunk<QMCD_MMA_LDC>(cb, Cq, (size_t)N, col0, ncols, m, 0);
-        qmcd_cp_async_commit();
-        double2 a_next[A_T];
+        __syncthreads();                         // every warp is done with the chunk buffers
 #pragma unroll
-        for (int a = 0; a < A_T; ++a) a_next[a] = av[a] ? qmcd_ldg128(ap[a]) : make_double2(0.0, 0.0);
+        for (int i = 0; i < NS - 1; ++i) {
+            if (i < nchunks) qmcd_stage_chunk<QMCD_MMA_LDC>(cb + i * QMCD_MMA_CHUNK_DOUBLES, Cq, (size_t)N, col0, ncols, m, i * QMCD_MMA_KC);
+            qmcd_cp_async_commit();
+        }
+        // A fragments: a ring of 4 k-groups (32 columns) ahead of the MMAs
+        double2 ar[4][A_T];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int a = 0; a < A_T; ++a) ar[i][a] = av[a] ? qmcd_ldg128(ap[a] + 8 * i) : make_double2(0.0, 0.0);
         for (int kc = 0; kc < nchunks; ++kc) {
-            if (kc + 1 < nchunks) {
-                qmcd_stage_chunk<QMCD_MMA_LDC>(cb + ((kc + 1) & 1) * QMCD_MMA_CHUNK_DOUBLES, Cq, (size_t)N, col0, ncols, m,
-                                               (kc + 1) * QMCD_MMA_KC);
-                qmcd_cp_async_commit();
-                qmcd_cp_async_wait<1>();
-            } else {
-                qmcd_cp_async_wait<0>();
-            }
-            __syncthreads();
-            const double* cur = cb + (kc & 1) * QMCD_MMA_CHUNK_DOUBLES + g * QMCD_MMA_LDC + 2 * c;
+            qmcd_cp_async_wait<NS - 2>();
+            __syncthreads();                     // chunk kc landed; buffer (kc-1)%NS is free
+            const double* cur = cb + (kc % NS) * QMCD_MMA_CHUNK_DOUBLES + g * QMCD_MMA_LDC + 2 * c;
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
+                if (q == 4 * (wid >> 2)) {       // warps 0-3 stage at q = 0, warps 4-7 at q = 4
+                    if (kc + NS - 1 < nchunks)
+                        qmcd_stage_half<QMCD_MMA_LDC>(cb + ((kc + NS - 1) % NS) * QMCD_MMA_CHUNK_DOUBLES, Cq, (size_t)N, col0,
+                                                      ncols, m, (kc + NS - 1) * QMCD_MMA_KC, wid >> 2);
+                    qmcd_cp_async_commit();
+                }
                 double2 a_cur[A_T];
 #pragma unroll
-                for (int a = 0; a < A_T; ++a) a_cur[a] = a_next[a];
-                const int nk = kc * QMCD_MMA_KC + (q + 1) * 8;
+                for (int a = 0; a < A_T; ++a) a_cur[a] = ar[q & 3][a];
+                const int nk = kc * QMCD_MMA_KC + (q + 4) * 8;
                 if (nk < N) {
 #pragma unroll
                     for (int a = 0; a < A_T; ++a)
-                        if (av[a]) a_next[a] = qmcd_ldg128(ap[a] + nk);
+                        if (av[a]) ar[q & 3][a] = qmcd_ldg128(ap[a] + nk);
                 }
                 // all k-step-0 MMAs, then all k-step-1 MMAs: consecutive DMMAs are independent
                 double2 bv[NB];
@@ -142,8 +166,8 @@ __device__ void qmcd_mma_nt(const double* Bw, int N, int row0, int nvalid,
 #pragma unroll
                     for (int a = 0; a < A_T; ++a) qmcd_dmma(acc[a][b][0], acc[a][b][1], a_cur[a].y, bv[b].y);
             }
-            __syncthreads();
         }
+        qmcd_cp_async_wait<0>();
 #pragma unroll
         for (int a = 0; a < A_T; ++a)
 #pragma unroll
@@ -164,18 +188,25 @@ __device__ void qmcd_mma_nt(const double* Bw, int N, int row0, int nvalid,
 // NN stage:  D[row0+r][n] = (INIT ? D[row0+r][n] : 0) + sum_a Ts[r][a] X[a][n]
 // for tile rows r < nvalid and columns n in [c_lo, c_hi) (multiple of 64 wide),
 // a < kext (X rows >= m_valid read as zero).  X is staged in 64 x 64 chunks
-// (cp.async, double buffered over the linear (n-chunk, k-chunk) sequence); the
-// warp's 16 A_T/2... rows x 64 columns of D live in registers.
+// (cp.async ring of NS buffers, one __syncthreads per chunk).  A warp owns 8 A_T
+// rows and works in PASSES of 64 / A_T columns (16 accumulator registers pairs):
+// while pass p's MMAs run, the 8 vectors of pass p+1's initial D values are
+// loaded and the 8 result vectors of pass p-1 are stored, one of each per
+// k-group, so loads, MMAs and stores of three consecutive passes overlap and the
+// store queue never sees a burst.  A_T = 2 needs kext <= 64 (one k-chunk).
 // ---------------------------------------------------------------------------
-template <int A_T, bool INIT>
+template <int A_T, bool INIT, int NS>
 __device__ void qmcd_mma_nn(const double* __restrict__ Ts, int ldT, int kext,
                             const double* __restrict__ X, int m_valid, int N,
                             double* D, int row0, int nvalid, int c_lo, int c_hi,
                             double* __restrict__ cb) {
+    constexpr int GH = 4 / A_T;          // 16-column groups per pass
+    constexpr int NP = A_T;              // passes per 64-column chunk
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, g = lane >> 2, c = lane & 3;
     const int nk = (kext + 63) >> 6;
     const int nn = (c_hi - c_lo) >> 6;
     const int total = nn * nk;
+    const int npass = nn * NP;
     bool rv[A_T];
     double* dp[A_T];
     const double* tp[A_T];
@@ -186,82 +217,118 @@ __device__ void qmcd_mma_nn(const double* __restrict__ Ts, int ldT, int kext,
         dp[a] = D + (size_t)(row0 + (rv[a] ? r : 0)) * N + 4 * c;
         tp[a] = Ts + (size_t)r * ldT + 2 * c;
     }
-    qmcd_stage_chunk<QMCD_MMA_LDX>(cb, X, (size_t)N, 0, min(64, kext), m_valid, c_lo);
-    qmcd_cp_async_commit();
-    int ci = 0;
+    const bool warp_has_rows = wid * 8 * A_T < nvalid;       // warps without rows only help staging
+    __syncthreads();                                         // every warp is done with the chunk buffers
+#pragma unroll
+    for (int i = 0; i < NS - 1; ++i) {
+        if (i < total) {
+            const int ni = i / nk, kb = i - ni * nk;
+            qmcd_stage_chunk<QMCD_MMA_LDX>(cb + i * QMCD_MMA_CHUNK_DOUBLES, X, (size_t)N, kb * 64, min(64, kext - kb * 64),
+                                           m_valid, c_lo + ni * 64);
+        }
+        qmcd_cp_async_commit();
+    }
+    // vector v = (a, Gl, h) of a pass: rows a, columns 16 (hp GH + Gl) + 4 c + 2 h .. +1
+    double2 initn[8], outv[8];
+#pragma unroll
+    for (int v = 0; v < 8; ++v) {
+        const int a = v / (2 * GH), Gl = (v >> 1) % GH, h = v & 1;
+        initn[v] = (INIT && rv[a]) ? qmcd_ldg128(dp[a] + c_lo + 16 * Gl + 2 * h) : make_double2(0.0, 0.0);
+        outv[v] = make_double2(0.0, 0.0);
+    }
+    int ci = 0, pprev_col = -1;
     for (int ni = 0; ni < nn; ++ni) {
         const int n0 = c_lo + ni * 64;
-        double2 binit[A_T][4][2];
-        if (INIT) {
+#pragma unroll
+        for (int hp = 0; hp < NP; ++hp) {
+            const int pcol = n0 + 16 * GH * hp;                       // first column of this pass
+            const int pass = ni * NP + hp;
+            const int ncol = (hp + 1 < NP) ? pcol + 16 * GH : n0 + 64; // first column of the next pass
+            const bool has_next = pass + 1 < npass;
+            double acc[A_T][GH][2][2];
 #pragma unroll
             for (int a = 0; a < A_T; ++a)
 #pragma unroll
-                for (int G = 0; G < 4; ++G) {
-                    binit[a][G][0] = rv[a] ? qmcd_ldg128(dp[a] + n0 + 16 * G) : make_double2(0.0, 0.0);
-                    binit[a][G][1] = rv[a] ? qmcd_ldg128(dp[a] + n0 + 16 * G + 2) : make_double2(0.0, 0.0);
+                for (int Gl = 0; Gl < GH; ++Gl) {
+                    const int v = (a * GH + Gl) * 2;
+                    acc[a][Gl][0][0] = initn[v].x; acc[a][Gl][1][0] = initn[v].y;
+                    acc[a][Gl][0][1] = initn[v + 1].x; acc[a][Gl][1][1] = initn[v + 1].y;
                 }
-        }
-        double acc[A_T][4][2][2];
-#pragma unroll
-        for (int a = 0; a < A_T; ++a)
-#pragma unroll
-            for (int G = 0; G < 4; ++G) { acc[a][G][0][0] = acc[a][G][0][1] = acc[a][G][1][0] = acc[a][G][1][1] = 0.0; }
-        for (int kb = 0; kb < nk; ++kb, ++ci) {
-            if (ci + 1 < total) {
-                const int nci = ci + 1, nni = nci / nk, nkb = nci - nni * nk;
-                qmcd_stage_chunk<QMCD_MMA_LDX>(cb + (nci & 1) * QMCD_MMA_CHUNK_DOUBLES, X, (size_t)N, nkb * 64,
-                                               min(64, kext - nkb * 64), m_valid, c_lo + nni * 64);
-                qmcd_cp_async_commit();
-                qmcd_cp_async_wait<1>();
-            } else {
-                qmcd_cp_async_wait<0>();
-            }
-            __syncthreads();
-            const double* cur = cb + (ci & 1) * QMCD_MMA_CHUNK_DOUBLES + (2 * c) * QMCD_MMA_LDX + 2 * g;
-            const int nq = min(64, kext - kb * 64) >> 3;
-#pragma unroll 2
-            for (int q = 0; q < nq; ++q) {
-                double2 avv[A_T];
-#pragma unroll
-                for (int a = 0; a < A_T; ++a) avv[a] = qmcd_lds128(tp[a] + kb * 64 + 8 * q);
-                double2 x0[4], x1[4];
-#pragma unroll
-                for (int G = 0; G < 4; ++G) {
-                    x0[G] = qmcd_lds128(cur + (8 * q) * QMCD_MMA_LDX + 16 * G);
-                    x1[G] = qmcd_lds128(cur + (8 * q + 1) * QMCD_MMA_LDX + 16 * G);
+            for (int kb = 0; kb < nk; ++kb) {
+                if (hp == 0) {                   // a new chunk (with A_T = 2, nk == 1: both passes share it)
+                    qmcd_cp_async_wait<NS - 2>();
+                    __syncthreads();             // chunk ci landed; buffer (ci-1)%NS is free
                 }
+                const double* cur = cb + (ci % NS) * QMCD_MMA_CHUNK_DOUBLES + (2 * c) * QMCD_MMA_LDX + 2 * g + 16 * GH * hp;
+                const int nq = min(64, kext - kb * 64) >> 3;
 #pragma unroll
-                for (int G = 0; G < 4; ++G)
-#pragma unroll
-                    for (int a = 0; a < A_T; ++a) {
-                        qmcd_dmma(acc[a][G][0][0], acc[a][G][0][1], avv[a].x, x0[G].x);
-                        qmcd_dmma(acc[a][G][1][0], acc[a][G][1][1], avv[a].x, x0[G].y);
+                for (int q = 0; q < 8; ++q) {
+                    // warps 0-3 stage at the chunk's first k-group, warps 4-7 half way through it
+                    if ((wid < 4) ? (hp == 0 && q == 0) : (NP == 1 ? q == 4 : (hp == 1 && q == 0))) {
+                        if (ci + NS - 1 < total) {
+                            const int nci = ci + NS - 1, nni = nci / nk, nkb = nci - nni * nk;
+                            qmcd_stage_half<QMCD_MMA_LDX>(cb + (nci % NS) * QMCD_MMA_CHUNK_DOUBLES, X, (size_t)N, nkb * 64,
+                                                          min(64, kext - nkb * 64), m_valid, c_lo + nni * 64, wid >> 2);
+                        }
+                        qmcd_cp_async_commit();
                     }
-#pragma unroll
-                for (int G = 0; G < 4; ++G)
-#pragma unroll
-                    for (int a = 0; a < A_T; ++a) {
-                        qmcd_dmma(acc[a][G][0][0], acc[a][G][0][1], avv[a].y, x1[G].x);
-                        qmcd_dmma(acc[a][G][1][0], acc[a][G][1][1], avv[a].y, x1[G].y);
+                    if (kb == 0) {
+                        const int a = q / (2 * GH), Gl = (q >> 1) % GH, h = q & 1;
+                        if (rv[a]) {
+                            if (pprev_col >= 0) qmcd_stg128(dp[a] + pprev_col + 16 * Gl + 2 * h, outv[q].x, outv[q].y);
+                            if (INIT && has_next) initn[q] = qmcd_ldg128(dp[a] + ncol + 16 * Gl + 2 * h);
+                        }
                     }
-            }
-            __syncthreads();
-        }
+                    if (q < nq && warp_has_rows) {
+                        double2 avv[A_T];
 #pragma unroll
-        for (int a = 0; a < A_T; ++a) {
-            if (!rv[a]) continue;
+                        for (int a = 0; a < A_T; ++a) avv[a] = qmcd_lds128(tp[a] + kb * 64 + 8 * q);
+                        double2 x0[GH], x1[GH];
 #pragma unroll
-            for (int G = 0; G < 4; ++G) {
-                double o0 = acc[a][G][0][0], o1 = acc[a][G][1][0], o2 = acc[a][G][0][1], o3 = acc[a][G][1][1];
-                if (INIT) { o0 += binit[a][G][0].x; o1 += binit[a][G][0].y; o2 += binit[a][G][1].x; o3 += binit[a][G][1].y; }
-                qmcd_stg128(dp[a] + n0 + 16 * G, o0, o1);
-                qmcd_stg128(dp[a] + n0 + 16 * G + 2, o2, o3);
+                        for (int Gl = 0; Gl < GH; ++Gl) {
+                            x0[Gl] = qmcd_lds128(cur + (8 * q) * QMCD_MMA_LDX + 16 * Gl);
+                            x1[Gl] = qmcd_lds128(cur + (8 * q + 1) * QMCD_MMA_LDX + 16 * Gl);
+                        }
+#pragma unroll
+                        for (int Gl = 0; Gl < GH; ++Gl)
+#pragma unroll
+                            for (int a = 0; a < A_T; ++a) {
+                                qmcd_dmma(acc[a][Gl][0][0], acc[a][Gl][0][1], avv[a].x, x0[Gl].x);
+                                qmcd_dmma(acc[a][Gl][1][0], acc[a][Gl][1][1], avv[a].x, x0[Gl].y);
+                            }
+#pragma unroll
+                        for (int Gl = 0; Gl < GH; ++Gl)
+#pragma unroll
+                            for (int a = 0; a < A_T; ++a) {
+                                qmcd_dmma(acc[a][Gl][0][0], acc[a][Gl][0][1], avv[a].y, x1[Gl].x);
+                                qmcd_dmma(acc[a][Gl][1][0], acc[a][Gl][1][1], avv[a].y, x1[Gl].y);
+                            }
+                    }
+                }
+                if (hp == NP - 1) ++ci;
             }
+#pragma unroll
+            for (int a = 0; a < A_T; ++a)
+#pragma unroll
+                for (int Gl = 0; Gl < GH; ++Gl) {
+                    const int v = (a * GH + Gl) * 2;
+                    outv[v] = make_double2(acc[a][Gl][0][0], acc[a][Gl][1][0]);
+                    outv[v + 1] = make_double2(acc[a][Gl][0][1], acc[a][Gl][1][1]);
+                }
+            pprev_col = pcol;
         }
     }
+    if (pprev_col >= 0) {
+#pragma unroll
+        for (int v = 0; v < 8; ++v) {
+            const int a = v / (2 * GH), Gl = (v >> 1) % GH, h = v & 1;
+            if (rv[a]) qmcd_stg128(dp[a] + pprev_col + 16 * Gl + 2 * h, outv[v].x, outv[v].y);
+        }
+    }
+    qmcd_cp_async_wait<0>();
 }
 
-template <int A_T>
+template <int A_T, int NS>
 __device__ void qmcd_flush_mma_impl(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
                                     const QmcdWalker& w, int m) {
     constexpr int R = 64 * A_T;
@@ -277,22 +344,26 @@ __device__ void qmcd_flush_mma_impl(const QmcdDev& P, const QmcdSmem& s, cg::clu
             Ts[(size_t)r * ldT + a] = (r0 + r < m && a < m) ? __ldcg(w.M + (size_t)(r0 + r) * K + a) : 0.0;
         }
         __syncthreads();
-        qmcd_mma_nn<A_T, false>(Ts, ldT, mp8, w.W, m, N, w.Y, r0, min(R, m - r0), w.klo, w.khi, cb);
+        qmcd_mma_nn<A_T, false, NS>(Ts, ldT, mp8, w.W, m, N, w.Y, r0, min(R, m - r0), w.klo, w.khi, cb);
         __syncthreads();
     }
     if (P.S > 1) cl.sync(); else __syncthreads();
     // ---- my row slice, R rows at a time:  T = -(B C^T - E_J);  B += T Y
     for (int row0 = w.klo; row0 < w.khi; row0 += R) {
         const int nvalid = min(R, w.khi - row0);
-        if (mp8 <= 32) qmcd_mma_nt<A_T, 4>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
-        else qmcd_mma_nt<A_T, 8>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
-        qmcd_mma_nn<A_T, true>(Ts, ldT, mp8, w.Y, m, N, w.B, row0, nvalid, 0, N, cb);
+        if (mp8 <= 32) qmcd_mma_nt<A_T, 4, NS>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
+        else qmcd_mma_nt<A_T, 8, NS>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
+        qmcd_mma_nn<A_T, true, NS>(Ts, ldT, mp8, w.Y, m, N, w.B, row0, nvalid, 0, N, cb);
         __syncthreads();
     }
 }
 
 __device__ inline void qmcd_flush_mma(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
                                       const QmcdWalker& w, int m) {
-    if (qmcd_mma_rows(P.K) == 128 && (w.khi - w.klo) >= 128) qmcd_flush_mma_impl<2>(P, s, cl, w, m);
-    else qmcd_flush_mma_impl<1>(P, s, cl, w, m);
+    if (qmcd_mma_stages(P.K) == 3) {
+        if (qmcd_mma_rows(P.K) == 128 && (w.khi - w.klo) >= 128) qmcd_flush_mma_impl<2, 3>(P, s, cl, w, m);
+        else qmcd_flush_mma_impl<1, 3>(P, s, cl, w, m);
+    } else {
+        qmcd_flush_mma_impl<1, 2>(P, s, cl, w, m);
+    }
 }
