@@ -136,6 +136,9 @@ __device__ void qmcd_mma_nt(const double* Bw, int N, int row0, int nvalid,
             qmcd_cp_async_wait<NS - 2>();
             __syncthreads();                     // chunk kc landed; buffer (kc-1)%NS is free
             const double* cur = cb + (kc % NS) * QMCD_MMA_CHUNK_DOUBLES + g * QMCD_MMA_LDC + 2 * c;
+            double2 bn[NB];                      // C fragments of k-group q+1, loaded during k-group q
+#pragma unroll
+            for (int b = 0; b < NB; ++b) bn[b] = qmcd_lds128(cur + b * 8 * QMCD_MMA_LDC);
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
                 if (q == 4 * (wid >> 2)) {       // warps 0-3 stage at q = 0, warps 4-7 at q = 4
@@ -156,7 +159,11 @@ __device__ void qmcd_mma_nt(const double* Bw, int N, int row0, int nvalid,
                 // all k-step-0 MMAs, then all k-step-1 MMAs: consecutive DMMAs are independent
                 double2 bv[NB];
 #pragma unroll
-                for (int b = 0; b < NB; ++b) bv[b] = qmcd_lds128(cur + b * 8 * QMCD_MMA_LDC + 8 * q);
+                for (int b = 0; b < NB; ++b) bv[b] = bn[b];
+                if (q < 7) {
+#pragma unroll
+                    for (int b = 0; b < NB; ++b) bn[b] = qmcd_lds128(cur + b * 8 * QMCD_MMA_LDC + 8 * (q + 1));
+                }
 #pragma unroll
                 for (int b = 0; b < NB; ++b)
 #pragma unroll
@@ -261,6 +268,14 @@ __device__ void qmcd_mma_nn(const double* __restrict__ Ts, int ldT, int kext,
                 }
                 const double* cur = cb + (ci % NS) * QMCD_MMA_CHUNK_DOUBLES + (2 * c) * QMCD_MMA_LDX + 2 * g + 16 * GH * hp;
                 const int nq = min(64, kext - kb * 64) >> 3;
+                double2 fa[A_T], f0[GH], f1[GH];
+#pragma unroll
+                for (int a = 0; a < A_T; ++a) fa[a] = qmcd_lds128(tp[a] + kb * 64);
+#pragma unroll
+                for (int Gl = 0; Gl < GH; ++Gl) {
+                    f0[Gl] = qmcd_lds128(cur + 16 * Gl);
+                    f1[Gl] = qmcd_lds128(cur + QMCD_MMA_LDX + 16 * Gl);
+                }
 #pragma unroll
                 for (int q = 0; q < 8; ++q) {
                     // warps 0-3 stage at the chunk's first k-group, warps 4-7 half way through it
@@ -273,21 +288,33 @@ __device__ void qmcd_mma_nn(const double* __restrict__ Ts, int ldT, int kext,
                         qmcd_cp_async_commit();
                     }
                     if (kb == 0) {
-                        const int a = q / (2 * GH), Gl = (q >> 1) % GH, h = q & 1;
-                        if (rv[a]) {
-                            if (pprev_col >= 0) qmcd_stg128(dp[a] + pprev_col + 16 * Gl + 2 * h, outv[q].x, outv[q].y);
-                            if (INIT && has_next) initn[q] = qmcd_ldg128(dp[a] + ncol + 16 * Gl + 2 * h);
+                        // k-groups 0-3: the next pass's 8 initial vectors (two each, as early as
+                        // possible); k-groups 4-7: the previous pass's 8 result vectors
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            const int v = 2 * (q & 3) + e;
+                            const int a = v / (2 * GH), Gl = (v >> 1) % GH, h = v & 1;
+                            if (rv[a]) {
+                                if (q < 4) { if (INIT && has_next) initn[v] = qmcd_ldg128(dp[a] + ncol + 16 * Gl + 2 * h); }
+                                else if (pprev_col >= 0) qmcd_stg128(dp[a] + pprev_col + 16 * Gl + 2 * h, outv[v].x, outv[v].y);
+                            }
                         }
                     }
                     if (q < nq && warp_has_rows) {
-                        double2 avv[A_T];
+                        // fragments of k-group q were loaded during k-group q-1
+                        double2 avv[A_T], x0[GH], x1[GH];
 #pragma unroll
-                        for (int a = 0; a < A_T; ++a) avv[a] = qmcd_lds128(tp[a] + kb * 64 + 8 * q);
-                        double2 x0[GH], x1[GH];
+                        for (int a = 0; a < A_T; ++a) avv[a] = fa[a];
 #pragma unroll
-                        for (int Gl = 0; Gl < GH; ++Gl) {
-                            x0[Gl] = qmcd_lds128(cur + (8 * q) * QMCD_MMA_LDX + 16 * Gl);
-                            x1[Gl] = qmcd_lds128(cur + (8 * q + 1) * QMCD_MMA_LDX + 16 * Gl);
+                        for (int Gl = 0; Gl < GH; ++Gl) { x0[Gl] = f0[Gl]; x1[Gl] = f1[Gl]; }
+                        if (q + 1 < nq) {
+#pragma unroll
+                            for (int a = 0; a < A_T; ++a) fa[a] = qmcd_lds128(tp[a] + kb * 64 + 8 * (q + 1));
+#pragma unroll
+                            for (int Gl = 0; Gl < GH; ++Gl) {
+                                f0[Gl] = qmcd_lds128(cur + (8 * (q + 1)) * QMCD_MMA_LDX + 16 * Gl);
+                                f1[Gl] = qmcd_lds128(cur + (8 * (q + 1) + 1) * QMCD_MMA_LDX + 16 * Gl);
+                            }
                         }
 #pragma unroll
                         for (int Gl = 0; Gl < GH; ++Gl)
