@@ -143,10 +143,14 @@ int qmcd_sweep_host(qmcd_handle h, int j_begin, int n_moves,
                     void* staging_dev, size_t staging_bytes);
 size_t qmcd_sweep_host_min_staging(int N, int batch);
 
-/* Tuning / introspection.  set: "cluster" (CTAs per walker, 1..16), "flush_path"
+/* Tuning / introspection.  set: "cluster" (CTAs per cluster, 1..16; resets
+ * "clusters_per_walker" to 1), "clusters_per_walker" (1..4: cluster 0 of a walker
+ * runs the look-ahead, all of them share the rows of a flush; they must all fit
+ * on the device at once, else QMCD_EINVAL), "flush_path"
  * (0 auto, 1 CUDA-core, 2 DMMA), "lookahead" (qmcd_sweep: 0 auto = blocked
  * look-ahead when the shape allows, 1 = per move, the arithmetic of the per-call
- * API).  get: those plus "threads", "smem_bytes", "m_in_smem", "blocked_ok".
+ * API).  get: those plus "threads", "smem_bytes", "m_in_smem", "blocked_ok",
+ * "max_active_clusters".
  * get returns the value (>= 0) or a negative error. */
 int qmcd_set_option(qmcd_handle h, const char* key, int value);
 int qmcd_get_option(qmcd_handle h, const char* key);

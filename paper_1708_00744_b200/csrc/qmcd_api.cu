@@ -22,6 +22,7 @@ struct qmcd_ctx {
     size_t smem_bytes;
     int max_cluster;          // largest cluster size the device can co-schedule
     int lookahead;            // qmcd_sweep: 0 auto (blocked when possible), 1 per move
+    unsigned launch_seq;      // tags the leader/helper words of each launch
     char last_cuda_error[256];
 };
 
@@ -36,14 +37,15 @@ static int cuda_fail(qmcd_ctx* h, cudaError_t e, const char* what) {
 
 static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-struct WsLayout { size_t C, W, Y, M, J, m, sj, sR, sp, sc, sr, counters, status, total; };
+#define QMCD_GMAX 4        // clusters per walker (Y copies in the workspace)
+struct WsLayout { size_t C, W, Y, ybytes, M, J, m, sj, sR, sp, sc, sr, counters, status, go, done, total; };
 
 static WsLayout ws_layout(int N, int K, int batch) {
     WsLayout L; size_t o = 0;
     size_t kn = (size_t)batch * K * N * 8;
     L.C = o; o += al256(kn);
     L.W = o; o += al256(kn);
-    L.Y = o; o += al256(kn);
+    L.Y = o; L.ybytes = al256(kn); o += QMCD_GMAX * L.ybytes;     // one Y = M W per cluster of a walker
     L.M = o; o += al256((size_t)batch * K * K * 8);
     L.J = o; o += al256((size_t)batch * K * 4);
     L.m = o; o += al256((size_t)batch * 4);
@@ -54,6 +56,8 @@ static WsLayout ws_layout(int N, int K, int batch) {
     L.sr = o; o += al256((size_t)batch * K * 8);
     L.counters = o; o += al256((size_t)batch * 2 * 8);
     L.status = o; o += 256;
+    L.go = o; o += al256((size_t)batch * 8);
+    L.done = o; o += al256((size_t)batch * 8 * 8);
     L.total = o;
     return L;
 }
@@ -97,10 +101,36 @@ static int configure_kernel(qmcd_ctx* h, int S) {
     return QMCD_OK;
 }
 
-static int launch(qmcd_ctx* h, const QmcdArgs& a) {
+// Clusters of the current size the device can hold at once (0 on error).
+static int max_active_clusters(qmcd_ctx* h, int S, int nclusters) {
+    cudaLaunchConfig_t cfg; memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3((unsigned)(nclusters * S)); cfg.blockDim = dim3(QMCD_THREADS);
+    cfg.dynamicSmemBytes = h->smem_bytes;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)S; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, qmcd_kernel, &cfg) != cudaSuccess) { (void)cudaGetLastError(); return 0; }
+    return n;
+}
+
+// Largest G <= limit that keeps every CTA's flush row slice a multiple of 64 rows (1 otherwise).
+static int pick_G(int N, int S, int limit) {
+    if (limit > QMCD_GMAX) limit = QMCD_GMAX;
+    for (int G = limit; G > 1; --G)
+        if (N % (64 * S * G) == 0) return G;
+    return 1;
+}
+
+// with_helpers: the walker's helper clusters take part (launches that may flush many rows)
+static int launch(qmcd_ctx* h, QmcdArgs& a, bool with_helpers) {
+    const int G_act = with_helpers ? h->P.G : 1;
+    a.P.G_act = G_act;
+    a.P.launch_id = ++h->launch_seq;
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
-    cfg.gridDim = dim3((unsigned)(h->batch * h->P.S), 1, 1);
+    cfg.gridDim = dim3((unsigned)(h->batch * G_act * h->P.S), 1, 1);
     cfg.blockDim = dim3(QMCD_THREADS, 1, 1);
     cfg.dynamicSmemBytes = h->smem_bytes;
     cfg.stream = h->stream;
@@ -141,6 +171,8 @@ extern "C" int qmcd_create(qmcd_handle* out, int N, int K, int batch,
     P.sj = (int*)(ws + L.sj); P.sR = (double*)(ws + L.sR);
     P.sp = (double*)(ws + L.sp); P.sc = (double*)(ws + L.sc); P.sr = (double*)(ws + L.sr);
     P.counters = (long long*)(ws + L.counters); P.status = (int*)(ws + L.status);
+    P.go = (unsigned long long*)(ws + L.go); P.done = (unsigned long long*)(ws + L.done);
+    P.G = 1; P.G_act = 1; P.launch_id = 0; P.y_stride = L.ybytes / 8;
     P.flush_path = 0;
     int rc = QMCD_OK;
     do {
@@ -156,25 +188,22 @@ extern "C" int qmcd_create(qmcd_handle* out, int N, int K, int batch,
         }
         if (rc != QMCD_OK) break;
         h->max_cluster = 16;
-        int S = default_cluster(N, batch, prop.multiProcessorCount, h->max_cluster);
-        // shrink S until the device says a cluster of that size (with our smem) fits
-        for (;;) {
+        // Choose (S, G): S CTAs per cluster, G clusters per walker, maximising the SMs a walker
+        // gets (S*G) among the shapes the device can hold at once (a helper cluster spins on
+        // its leader, so all batch*G clusters must be co-resident); ties go to the larger S.
+        const int s_cap = default_cluster(N, batch, 16 * batch, h->max_cluster);   // N / 64 and 16 cap it
+        int bestS = 1, bestG = 1;
+        for (int S = s_cap; S >= 1; S /= 2) {
             rc = configure_kernel(h, S);
             if (rc != QMCD_OK) break;
-            cudaLaunchConfig_t cfg; memset(&cfg, 0, sizeof(cfg));
-            cfg.gridDim = dim3((unsigned)(batch * S)); cfg.blockDim = dim3(QMCD_THREADS);
-            cfg.dynamicSmemBytes = h->smem_bytes;
-            cudaLaunchAttribute attr[1];
-            attr[0].id = cudaLaunchAttributeClusterDimension;
-            attr[0].val.clusterDim.x = (unsigned)S; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-            cfg.attrs = attr; cfg.numAttrs = 1;
-            int nclusters = 0;
-            e = cudaOccupancyMaxActiveClusters(&nclusters, qmcd_kernel, &cfg);
-            if (e == cudaSuccess && nclusters >= 1 && (nclusters >= batch || S == 1)) break;
-            if (e != cudaSuccess) (void)cudaGetLastError();
-            if (S == 1) { if (e != cudaSuccess) rc = cuda_fail(h, e, "cudaOccupancyMaxActiveClusters"); break; }
-            S /= 2;
+            const int n = max_active_clusters(h, S, batch);
+            if (n < batch && S > 1) continue;
+            const int G = (n >= batch) ? pick_G(N, S, n / batch) : 1;
+            if (S * G > bestS * bestG) { bestS = S; bestG = G; }
         }
+        if (rc != QMCD_OK) break;
+        rc = configure_kernel(h, bestS);
+        h->P.G = bestG;
     } while (0);
     if (rc != QMCD_OK) {
         if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
@@ -221,7 +250,7 @@ extern "C" int qmcd_ratio(qmcd_handle h, int j, const double* v_dev, double* R_d
     if (!h->has_inverse) return QMCD_ESTATE;
     QmcdArgs a = base_args(h, QMCD_MODE_RATIO);
     a.j = j; a.v = v_dev; a.R_out = R_dev;
-    int rc = launch(h, a);
+    int rc = launch(h, a, false);
     if (rc == QMCD_OK) h->state = QMCD_PROPOSED;
     return rc;
 }
@@ -231,7 +260,7 @@ extern "C" int qmcd_ratio_jv(qmcd_handle h, const int* j_dev, const double* v_de
     if (!h->has_inverse) return QMCD_ESTATE;
     QmcdArgs a = base_args(h, QMCD_MODE_RATIO);
     a.jv = j_dev; a.v = v_dev; a.R_out = R_dev;
-    int rc = launch(h, a);
+    int rc = launch(h, a, false);
     if (rc == QMCD_OK) h->state = QMCD_PROPOSED;
     return rc;
 }
@@ -241,7 +270,7 @@ extern "C" int qmcd_accept(qmcd_handle h, const unsigned char* mask_dev) {
     if (h->state != QMCD_PROPOSED) return QMCD_ESTATE;
     QmcdArgs a = base_args(h, QMCD_MODE_ACCEPT);
     a.mask = mask_dev; a.accept_all = (mask_dev == nullptr);
-    int rc = launch(h, a);
+    int rc = launch(h, a, false);
     if (rc == QMCD_OK) h->state = QMCD_IDLE;
     return rc;
 }
@@ -251,7 +280,7 @@ extern "C" int qmcd_accept_metropolis(qmcd_handle h, const double* uniforms_dev,
     if (h->state != QMCD_PROPOSED) return QMCD_ESTATE;
     QmcdArgs a = base_args(h, QMCD_MODE_ACCEPT);
     a.uniforms = uniforms_dev; a.acc_out = acc_out_dev;
-    int rc = launch(h, a);
+    int rc = launch(h, a, false);
     if (rc == QMCD_OK) h->state = QMCD_IDLE;
     return rc;
 }
@@ -269,7 +298,7 @@ extern "C" int qmcd_flush(qmcd_handle h) {
     if (h->state != QMCD_IDLE) return QMCD_ESTATE;
     if (!h->has_inverse) return QMCD_OK;
     QmcdArgs a = base_args(h, QMCD_MODE_FLUSH);
-    return launch(h, a);
+    return launch(h, a, true);
 }
 
 extern "C" int qmcd_pending(qmcd_handle h, int* m_dev) {
@@ -306,7 +335,7 @@ extern "C" int qmcd_sweep(qmcd_handle h, int j_begin, int n_moves,
     a.j_begin = j_begin; a.n_moves = n_moves; a.v = proposals_dev;
     a.mask = mask_dev; a.uniforms = uniforms_dev; a.R_out = R_out_dev; a.acc_out = acc_out_dev;
     a.blocked = (h->lookahead != 1 && h->P.blk_ok && h->P.m_in_smem && (((uintptr_t)proposals_dev & 15) == 0)) ? 1 : 0;
-    return launch(h, a);
+    return launch(h, a, true);
 }
 
 extern "C" size_t qmcd_sweep_host_min_staging(int N, int batch) {
@@ -364,7 +393,14 @@ extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
     if (!strcmp(key, "cluster")) {
         if (value < 1 || value > 16 || value > h->N) return QMCD_EINVAL;
         CK(h, cudaStreamSynchronize(h->stream));
+        h->P.G = 1;
         return configure_kernel(h, value);
+    }
+    if (!strcmp(key, "clusters_per_walker")) {     // helper clusters spin on the leader: all must be co-resident
+        if (value < 1 || value > QMCD_GMAX) return QMCD_EINVAL;
+        if (value > 1 && (max_active_clusters(h, h->P.S, h->batch) < h->batch * value || h->N % (64 * h->P.S * value) != 0)) return QMCD_EINVAL;
+        h->P.G = value;
+        return QMCD_OK;
     }
     if (!strcmp(key, "flush_path")) {
         if (value < 0 || value > 2) return QMCD_EINVAL;
@@ -382,12 +418,14 @@ extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
 extern "C" int qmcd_get_option(qmcd_handle h, const char* key) {
     if (!h || !key) return QMCD_EINVAL;
     if (!strcmp(key, "cluster")) return h->P.S;
+    if (!strcmp(key, "clusters_per_walker")) return h->P.G;
     if (!strcmp(key, "flush_path")) return h->P.flush_path;
     if (!strcmp(key, "lookahead")) return h->lookahead;
     if (!strcmp(key, "blocked_ok")) return h->P.blk_ok && h->P.m_in_smem;
     if (!strcmp(key, "m_in_smem")) return h->P.m_in_smem;
     if (!strcmp(key, "threads")) return QMCD_THREADS;
     if (!strcmp(key, "smem_bytes")) return (int)h->smem_bytes;
+    if (!strcmp(key, "max_active_clusters")) return max_active_clusters(h, h->P.S, h->batch);
     return QMCD_EINVAL;
 }
 

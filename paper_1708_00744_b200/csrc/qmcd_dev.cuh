@@ -18,7 +18,13 @@ namespace cg = cooperative_groups;
 #define QMCD_DEV_ESINGULAR (-4)
 
 struct QmcdDev {
-    int N, K, batch, S;       // S = CTAs per walker (cluster size)
+    int N, K, batch, S;       // S = CTAs per cluster
+    int G;                    // clusters per walker: cluster 0 leads (look-ahead + flush), the rest help flushing
+    int G_act;                // clusters per walker taking part in THIS launch (1 or G), set per launch
+    unsigned launch_id;       // host counter, tags the go / done words of this launch
+    size_t y_stride;          // doubles between the Y copies of two clusters of one walker
+    unsigned long long* go;   // [batch]      leader -> helpers: (launch id << 32) | (flush no. << 12) | m
+    unsigned long long* done; // [batch][8]   helper g -> leader: (launch id << 32) | flush no.
     double* B;                // [batch][N][N]  inverse, borrowed, updated in place
     double* C;                // [batch][K][N]  queued new columns v_i (one per row)
     double* W;                // [batch][K][N]  rows j_i of the stale inverse B0
@@ -139,4 +145,15 @@ __device__ __forceinline__ void qmcd_set_status(const QmcdDev& P, int code, int 
         P.status[1] = walker;
         P.status[2] = (int)move;
     }
+}
+
+// ---- leader <-> helper clusters of one walker: words in global memory, release / acquire at gpu scope
+#define QMCD_GO_EXIT 0xFFFFFu
+__device__ __forceinline__ void qmcd_st_release(unsigned long long* p, unsigned long long v) {
+    asm volatile("st.release.gpu.global.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long qmcd_ld_acquire(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
 }

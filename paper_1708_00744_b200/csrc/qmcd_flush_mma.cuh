@@ -39,9 +39,9 @@ template <int N_> __device__ __forceinline__ void qmcd_cp_async_wait() {
     asm volatile("cp.async.wait_group %0;" :: "n"(N_) : "memory");
 }
 
-__device__ inline bool qmcd_flush_use_mma(const QmcdDev& P, int m) {
+__device__ inline bool qmcd_flush_use_mma(const QmcdDev& P, int m, int G_act) {
     if (P.flush_path == 1) return false;
-    const bool ok = (P.N % 64 == 0) && ((P.N / P.S) % 64 == 0) && P.mma_smem_ok;
+    const bool ok = (P.N % 64 == 0) && ((P.N / P.S) % 64 == 0) && ((P.N / (P.S * G_act)) % 64 == 0) && P.mma_smem_ok;
     if (!ok) return false;
     if (P.flush_path == 2) return true;
     return m >= 2;
@@ -376,8 +376,8 @@ __device__ void qmcd_flush_mma_impl(const QmcdDev& P, const QmcdSmem& s, cg::clu
     }
     if (P.S > 1) cl.sync(); else __syncthreads();
     // ---- my row slice, R rows at a time:  T = -(B C^T - E_J);  B += T Y
-    for (int row0 = w.klo; row0 < w.khi; row0 += R) {
-        const int nvalid = min(R, w.khi - row0);
+    for (int row0 = w.rlo; row0 < w.rhi; row0 += R) {
+        const int nvalid = min(R, w.rhi - row0);
         if (mp8 <= 32) qmcd_mma_nt<A_T, 4, NS>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
         else qmcd_mma_nt<A_T, 8, NS>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
         qmcd_mma_nn<A_T, true, NS>(Ts, ldT, mp8, w.Y, m, N, w.B, row0, nvalid, 0, N, cb);
@@ -388,7 +388,7 @@ __device__ void qmcd_flush_mma_impl(const QmcdDev& P, const QmcdSmem& s, cg::clu
 __device__ inline void qmcd_flush_mma(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
                                       const QmcdWalker& w, int m) {
     if (qmcd_mma_stages(P.K) == 3) {
-        if (qmcd_mma_rows(P.K) == 128 && (w.khi - w.klo) >= 128) qmcd_flush_mma_impl<2, 3>(P, s, cl, w, m);
+        if (qmcd_mma_rows(P.K) == 128 && (w.rhi - w.rlo) >= 128) qmcd_flush_mma_impl<2, 3>(P, s, cl, w, m);
         else qmcd_flush_mma_impl<1, 3>(P, s, cl, w, m);
     } else {
         qmcd_flush_mma_impl<1, 2>(P, s, cl, w, m);

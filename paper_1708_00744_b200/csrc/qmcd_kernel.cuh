@@ -4,22 +4,69 @@
 #include "qmcd_phases.cuh"
 #include "qmcd_flush_mma.cuh"
 
-// Flush wrapper: all CTAs of the cluster call it with the same m > 0.
-// M goes back to global memory first (the flush reads it from there).
+// Eq. 4 on this CTA's row slice (either path); ends with every CTA of the CLUSTER done.
+__device__ void qmcd_flush_rows(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
+                                const QmcdWalker& w, int m) {
+    if (qmcd_flush_use_mma(P, m, P.G_act)) qmcd_flush_mma(P, s, cl, w, m);
+    else qmcd_flush_simt(P, s, cl, w, m);
+}
+
+// Flush wrapper for the LEADER cluster: all its CTAs call it with the same m > 0.
+// M goes back to global memory first (the flush reads it from there).  With
+// G_act > 1 the walker's helper clusters are released through the `go` word
+// (they own the other row slices) and awaited through their `done` words.
 // Barriers: (entry) queue slots / M written by other CTAs become visible;
 // (exit) nobody restages slot 0 or reads B rows before every CTA is done.
+// s.iflag[8] counts the flushes of this launch (same value in every CTA).
 template <bool MS>
 __device__ void qmcd_flush_phase(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
                                  const QmcdWalker& w, int m) {
     qmcd_writeback_M<MS>(P, s, w, m);
     if (P.S > 1) cl.sync(); else __syncthreads();
-    if (qmcd_flush_use_mma(P, m)) qmcd_flush_mma(P, s, cl, w, m);
-    else qmcd_flush_simt(P, s, cl, w, m);
+    const int k = s.iflag[8] + 1;
+    if (P.G_act > 1 && w.r == 0 && threadIdx.x == 0) {
+        __threadfence();
+        qmcd_st_release(P.go + w.b, ((unsigned long long)P.launch_id << 32) | ((unsigned long long)k << 12) | (unsigned)m);
+    }
+    qmcd_flush_rows(P, s, cl, w, m);
+    __syncthreads();
+    if (threadIdx.x == 0) s.iflag[8] = k;
     if (w.r == 0 && threadIdx.x == 0) {
         P.m[w.b] = 0;
         P.counters[(size_t)w.b * 2 + 1] += 1;
+        const unsigned long long want = ((unsigned long long)P.launch_id << 32) | (unsigned)k;
+        for (int g = 1; g < P.G_act; ++g)
+            while (qmcd_ld_acquire(P.done + (size_t)w.b * 8 + g) != want) __nanosleep(64);
     }
     if (P.S > 1) cl.sync(); else __syncthreads();
+}
+
+// Helper cluster (w.g > 0): flush my row slices whenever the leader says so, until it says exit.
+__device__ void qmcd_helper_loop(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
+                                 const QmcdWalker& w) {
+    for (int k = 1;; ++k) {
+        if (threadIdx.x == 0) {
+            unsigned long long v;
+            for (;;) {
+                v = qmcd_ld_acquire(P.go + w.b);
+                if ((unsigned)(v >> 32) == P.launch_id) {
+                    const unsigned f = (unsigned)(v >> 12) & 0xFFFFFu;
+                    if (f == QMCD_GO_EXIT || f == (unsigned)k) break;
+                }
+                __nanosleep(64);
+            }
+            s.iflag[9] = (((unsigned)(v >> 12) & 0xFFFFFu) == QMCD_GO_EXIT) ? -1 : (int)(v & 0xFFFu);
+        }
+        __syncthreads();
+        const int m = s.iflag[9];
+        if (m < 0) return;
+        qmcd_flush_rows(P, s, cl, w, m);
+        if (P.S > 1) cl.sync(); else __syncthreads();      // the whole cluster is done with its rows
+        if (w.r == 0 && threadIdx.x == 0) {
+            __threadfence();
+            qmcd_st_release(P.done + (size_t)w.b * 8 + w.g, ((unsigned long long)P.launch_id << 32) | (unsigned)k);
+        }
+    }
 }
 
 #include "qmcd_block.cuh"
@@ -151,9 +198,18 @@ __global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel(const QmcdArgs A)
     cg::cluster_group cl = cg::this_cluster();
     const int S = P.S;
     const int r = (S > 1) ? (int)cl.block_rank() : 0;
-    const int b = blockIdx.x / S;
+    const int cidx = blockIdx.x / S;                 // cluster index
+    const int b = cidx / P.G_act, g = cidx - b * P.G_act;
     const QmcdSmem s = qmcd_carve(qmcd_smem_raw, P.N, P.K, S, P.m_in_smem != 0);
-    const QmcdWalker w = qmcd_walker(P, b, r);
+    const QmcdWalker w = qmcd_walker(P, b, r, g, P.G_act);
+    if (threadIdx.x == 0) s.iflag[8] = 0;
+    __syncthreads();
+    if (g > 0) { qmcd_helper_loop(P, s, cl, w); return; }
     if (P.m_in_smem) qmcd_run<true>(A, s, cl, w);
     else qmcd_run<false>(A, s, cl, w);
+    if (P.G_act > 1) {                               // release the helpers (every return path of qmcd_run lands here)
+        if (S > 1) cl.sync(); else __syncthreads();
+        if (r == 0 && threadIdx.x == 0)
+            qmcd_st_release(P.go + b, ((unsigned long long)P.launch_id << 32) | ((unsigned long long)QMCD_GO_EXIT << 12));
+    }
 }

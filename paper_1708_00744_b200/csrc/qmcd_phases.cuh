@@ -4,23 +4,27 @@
 #pragma once
 #include "qmcd_dev.cuh"
 
-struct QmcdWalker {          // per-CTA view of the walker this cluster owns
+struct QmcdWalker {          // per-CTA view of the walker this cluster works for
     int b;                   // walker index
     int r;                   // CTA rank in the cluster
-    int klo, khi;            // owned column slice (ratio) == owned row slice (flush)
+    int g;                   // cluster index within the walker (0 = leader)
+    int klo, khi;            // column slice of the look-ahead and of Y = M W (per cluster)
+    int rlo, rhi;            // row slice of B in the flush (over all G_act * S CTAs of the walker)
     double *B, *C, *W, *Y, *M;
     int* J;
 };
 
-__device__ inline QmcdWalker qmcd_walker(const QmcdDev& P, int b, int r) {
+__device__ inline QmcdWalker qmcd_walker(const QmcdDev& P, int b, int r, int g, int G_act) {
     QmcdWalker w;
-    w.b = b; w.r = r;
+    w.b = b; w.r = r; w.g = g;
     w.klo = qmcd_slice_lo(P.N, P.S, r);
     w.khi = qmcd_slice_lo(P.N, P.S, r + 1);
+    w.rlo = qmcd_slice_lo(P.N, P.S * G_act, g * P.S + r);
+    w.rhi = qmcd_slice_lo(P.N, P.S * G_act, g * P.S + r + 1);
     w.B = P.B + (size_t)b * P.N * P.N;
     w.C = P.C + (size_t)b * P.K * P.N;
     w.W = P.W + (size_t)b * P.K * P.N;
-    w.Y = P.Y + (size_t)b * P.K * P.N;
+    w.Y = P.Y + (size_t)b * P.K * P.N + (size_t)g * P.y_stride;   // every cluster forms its own Y = M W
     w.M = P.M + (size_t)b * P.K * P.K;
     w.J = P.J + (size_t)b * P.K;
     return w;
@@ -241,7 +245,7 @@ __device__ void qmcd_flush_simt(const QmcdDev& P, const QmcdSmem& s, cg::cluster
     if (S > 1) cl.sync(); else __syncthreads();
     // steps 2-3: rows of my slice, one warp per row
     double* Tw = s.Ts + (size_t)wid * K;
-    for (int r = w.klo + wid; r < w.khi; r += QMCD_WARPS) {
+    for (int r = w.rlo + wid; r < w.rhi; r += QMCD_WARPS) {
         double* Br = w.B + (size_t)r * N;
         for (int a0 = 0; a0 < m; a0 += 4) {
             double acc[4] = {0, 0, 0, 0};

@@ -38,9 +38,9 @@ def test_workspace_bytes_validation(lib):
     assert lib.qmcd_workspace_bytes(8, 0, 1) == 0
     assert lib.qmcd_workspace_bytes(8, 9, 1) == 0          # K > N (reading G16)
     assert lib.qmcd_workspace_bytes(8, 8, 0) == 0
-    # three K x N buffers per walker dominate
+    # K x N buffers per walker dominate: C, W and one Y per cluster of a walker (up to 4)
     big = lib.qmcd_workspace_bytes(4096, 256, 8)
-    assert 3 * 8 * 256 * 4096 * 8 <= big < 3 * 8 * 256 * 4096 * 8 + (8 << 20)
+    assert 6 * 8 * 256 * 4096 * 8 <= big < 6 * 8 * 256 * 4096 * 8 + (8 << 20)
 
 
 def test_strerror_and_version(lib):

@@ -164,6 +164,36 @@ def test_dmma_flush_matches_oracle(qmcd, N, K, batch, cluster, p):
     assert np.max(np.abs(g["B"] - s["B"])) <= 1e-11
 
 
+@pytest.mark.parametrize("N,K,batch,cluster,G", [(512, 32, 3, 4, 2), (512, 16, 2, 2, 4), (256, 8, 4, 1, 4),
+                                                 (1024, 64, 2, 4, 4), (384, 24, 2, 2, 3)])
+def test_helper_clusters_share_the_flush(qmcd, N, K, batch, cluster, G):
+    """clusters_per_walker > 1: cluster 0 of a walker runs the look-ahead, all G clusters split
+    the rows of every flush (leader/helper handshake through global memory)."""
+    wl = inputs.make_workload(batch, N, n_moves=N + 2 * K + 5, seed=31)
+    mask = wl.bernoulli_mask(0.9)
+    Bo = wl.Ainv.copy(); Ro, acco, _ = oracle.run(2, Bo, K, wl.proposals, mask=mask)
+    import torch
+    q = qmcd.Qmcd(N, K, batch)
+    q.set_option("cluster", cluster)
+    q.set_option("clusters_per_walker", G)
+    assert q.get_option("clusters_per_walker") == G
+    B = _dev(wl.Ainv); q.set_inverse(B)
+    R = torch.zeros((wl.n_moves, batch), dtype=torch.float64, device="cuda")
+    acc = torch.zeros((wl.n_moves, batch), dtype=torch.uint8, device="cuda")
+    half = wl.n_moves // 2
+    P, Md = _dev(wl.proposals), _dev(mask)
+    q.sweep(0, P[:half], mask=Md[:half], R_out=R[:half], acc_out=acc[:half])
+    q.flush()                                    # explicit flush launch with helpers, mid-run
+    q.sweep(half % N, P[half:], mask=Md[half:], R_out=R[half:], acc_out=acc[half:])
+    q.flush()
+    assert q.status()[0] == 0
+    assert np.array_equal(acc.cpu().numpy(), acco)
+    assert _rel(R.cpu().numpy(), Ro) <= RTOL_RATIO
+    assert np.max(np.abs(B.cpu().numpy() - Bo)) <= 1e-10
+    check_residuals(wl, mask, B.cpu().numpy())
+    q.close()
+
+
 def test_sweep_equals_call_by_call(qmcd):
     """qmcd_sweep must reproduce the ratio -> accept(mask) sequence (include/qmcd.h)."""
     wl = inputs.make_workload(4, 128, 200, seed=3)
