@@ -340,9 +340,14 @@ def run_ours(args):
     dfma = binding.probe_fp64(0, 20000)
     fl_final = 4.0 * N * N  # the final partial flush runs in the separate flush launch: negligible
     ach = work["flops"] / (sweep_ms * 1e-3) / 1e12
+    traffic = None
+    try:    # dram__bytes_read.sum + dram__bytes_write.sum of this kernel from the committed ncu capture
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(f"{args.config}:K{K}:{args.mode}")
+    except (OSError, ValueError):
+        pass
     roofline = {"kernel": "qmcd_kernel (sweep mode: ratio + accept + flush fused, one launch/step)",
                 "bound": "tensor", "achieved": ach, "peak": dmma, "unit": "TFLOP/s",
-                "frac": ach / dmma, "traffic": None,
+                "frac": ach / dmma, "traffic": traffic,
                 "peak_source": "measured live: register-resident DMMA.8x8x4 fp64 loop (qmcd_probe_fp64); "
                                f"DFMA loop {dfma:.1f} TFLOP/s; MEASURED_PEAKS.json has no fp64 figure",
                 "kernel_ms": sweep_ms, "algorithmic_flops_per_launch": work["flops"],
@@ -355,6 +360,9 @@ def run_ours(args):
            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": config_dict(args, cfg, wl, {"cluster": q.get_option("cluster"),
+                                                 "clusters_per_walker": q.get_option("clusters_per_walker"),
+                                                 "lookahead": "blocked" if (q.get_option("blocked_ok") and
+                                                                            q.get_option("lookahead") == 0) else "per-move",
                                                  "flush_path": q.get_option("flush_path"),
                                                  "accepted_per_step": accepted_all,
                                                  "flushes_per_step": work["flushes"]}),
