@@ -199,6 +199,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_1708_00744_b200 import binding, buildlib, inputs
+    from paper_1708_00744_b200 import dist as qdist
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -218,7 +219,7 @@ def run_ours(args):
 
     cfg = inputs.CONFIGS[args.config]
     wl = inputs.make_workload(cfg["batch"], cfg["N"], cfg["sweeps"] * cfg["N"],
-                              seed=cfg["seed"] + rank * cfg["batch"])     # per-rank walkers
+                              seed=qdist.rank_seed(cfg["seed"], rank, cfg["batch"]))     # per-rank walkers
     N, K, batch, n_moves = wl.N, args.K, wl.batch, wl.n_moves
     mask, uniforms = mode_inputs(wl, args.mode)
 
@@ -278,15 +279,9 @@ def run_ours(args):
         raise SystemExit(f"device status {st} {info}")
     acc_h = acc.cpu().numpy()
     accepted = int(acc_h.sum())
-    t = torch.tensor([ms_total, float(accepted)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        ms_total, accepted_all = float(tmax[0]), int(tsum[1])
-    else:
-        accepted_all = accepted
+    ms_total, accepted_all = qdist.combine(ms_total, accepted, device="cuda")    # max time, summed moves
     ms_per_step = ms_total / args.steps
-    value = accepted_all / (ms_per_step * 1e-3)
+    value = qdist.moves_per_second(ms_total, args.steps, accepted_all)
 
     # ---- end to end: host buffers through qmcd_sweep_host (H2D of Ainv + proposals + mask,
     #      D2H of R + acc inside the timed region)
