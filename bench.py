@@ -45,6 +45,7 @@ def parse_args():
     ap.add_argument("--mode", default="bern0.99")
     ap.add_argument("--cluster", type=int, default=0, help="CTAs per walker (0 = library default)")
     ap.add_argument("--flush-path", type=int, default=0, help="0 auto, 1 CUDA-core, 2 DMMA")
+    ap.add_argument("--opt", action="append", default=[], help="library option key=value (qmcd_set_option)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--phases", action="store_true",
@@ -228,6 +229,9 @@ def run_ours(args):
         q.set_option("cluster", args.cluster)
     if args.flush_path:
         q.set_option("flush_path", args.flush_path)
+    for kv in args.opt:
+        k_, v_ = kv.split("=")
+        q.set_option(k_, int(v_))
     B0 = torch.from_numpy(wl.Ainv).cuda()
     B = torch.empty_like(B0)
     P = torch.from_numpy(wl.proposals).cuda()
@@ -364,6 +368,14 @@ def run_ours(args):
            "clocks": clocks, "e2e": e2e, "gpu_launches": LAUNCHES_PER_STEP * args.steps,
            "roofline": roofline}
 
+    # time split inside the sweep kernel (SM cycles of each walker's leader CTA, summed over the
+    # steps since the last set_inverse = the last step): look-ahead products, per-move chain,
+    # queue append, flush
+    cyc = q.counters().cpu().numpy()[:, 2:7].astype(np.float64)
+    tot = np.maximum(cyc[:, 4], 1.0)
+    out["time_split"] = {k: float(np.mean(cyc[:, i] / tot)) for i, k in
+                         enumerate(["lookahead_products", "chain", "queue_append", "flush"])}
+    out["time_split"]["sweep_cycles_mean"] = float(np.mean(tot))
     if args.phases:
         out["phases"] = time_phases(binding, wl, K)
 

@@ -111,7 +111,9 @@ int qmcd_pending(qmcd_handle h, int* m_dev);
 int qmcd_status(qmcd_handle h, int* host_out, int* info_out);
 
 /* Per-walker counters since set_inverse, copied (enqueued) to
- * counters_dev: [batch][2] int64 = {accepted moves, flushes}. */
+ * counters_dev: [batch][8] int64 = {accepted moves, flushes, then SM clock cycles
+ * of the walker's leader CTA inside qmcd_sweep: look-ahead products (F1), per-move
+ * chain (F1 small part + F2), queue append, flush (F3), whole sweep, reserved}. */
 int qmcd_counters(qmcd_handle h, long long* counters_dev);
 
 /* Device-resident run of n_moves proposals with no host round trip (the same

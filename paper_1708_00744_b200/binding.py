@@ -175,7 +175,7 @@ class Qmcd:
 
     def counters(self):
         import torch
-        out = torch.empty((self.batch, 2), dtype=torch.int64, device="cuda")
+        out = torch.empty((self.batch, 8), dtype=torch.int64, device="cuda")
         _chk(self._L.qmcd_counters(self._h, _ptr(out, torch.int64)), "qmcd_counters")
         return out
 

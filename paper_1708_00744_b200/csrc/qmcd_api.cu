@@ -54,7 +54,7 @@ static WsLayout ws_layout(int N, int K, int batch) {
     L.sp = o; o += al256((size_t)batch * K * 8);
     L.sc = o; o += al256((size_t)batch * K * 8);
     L.sr = o; o += al256((size_t)batch * K * 8);
-    L.counters = o; o += al256((size_t)batch * 2 * 8);
+    L.counters = o; o += al256((size_t)batch * 8 * 8);
     L.status = o; o += 256;
     L.go = o; o += al256((size_t)batch * 8);
     L.done = o; o += al256((size_t)batch * 8 * 8);
@@ -172,7 +172,7 @@ extern "C" int qmcd_create(qmcd_handle* out, int N, int K, int batch,
     P.sp = (double*)(ws + L.sp); P.sc = (double*)(ws + L.sc); P.sr = (double*)(ws + L.sr);
     P.counters = (long long*)(ws + L.counters); P.status = (int*)(ws + L.status);
     P.go = (unsigned long long*)(ws + L.go); P.done = (unsigned long long*)(ws + L.done);
-    P.G = 1; P.G_act = 1; P.launch_id = 0; P.y_stride = L.ybytes / 8;
+    P.chain_regs = 1; P.G = 1; P.G_act = 1; P.launch_id = 0; P.y_stride = L.ybytes / 8;
     P.flush_path = 0;
     int rc = QMCD_OK;
     do {
@@ -231,7 +231,7 @@ extern "C" int qmcd_set_inverse(qmcd_handle h, double* Ainv_dev) {
     h->P.B = Ainv_dev;
     CK(h, cudaMemsetAsync(h->P.m, 0, (size_t)h->batch * 4, h->stream));
     CK(h, cudaMemsetAsync(h->P.sj, 0xff, (size_t)h->batch * 4, h->stream));
-    CK(h, cudaMemsetAsync(h->P.counters, 0, (size_t)h->batch * 16, h->stream));
+    CK(h, cudaMemsetAsync(h->P.counters, 0, (size_t)h->batch * 64, h->stream));
     CK(h, cudaMemsetAsync(h->P.status, 0, 16, h->stream));
     h->has_inverse = true;
     return QMCD_OK;
@@ -309,7 +309,7 @@ extern "C" int qmcd_pending(qmcd_handle h, int* m_dev) {
 
 extern "C" int qmcd_counters(qmcd_handle h, long long* counters_dev) {
     if (!h || !counters_dev) return QMCD_EINVAL;
-    CK(h, cudaMemcpyAsync(counters_dev, h->P.counters, (size_t)h->batch * 16, cudaMemcpyDeviceToDevice, h->stream));
+    CK(h, cudaMemcpyAsync(counters_dev, h->P.counters, (size_t)h->batch * 64, cudaMemcpyDeviceToDevice, h->stream));
     return QMCD_OK;
 }
 
@@ -410,6 +410,11 @@ extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
     if (!strcmp(key, "lookahead")) {
         if (value < 0 || value > 1) return QMCD_EINVAL;
         h->lookahead = value;
+        return QMCD_OK;
+    }
+    if (!strcmp(key, "chain_regs")) {
+        if (value < 0 || value > 1) return QMCD_EINVAL;
+        h->P.chain_regs = value;
         return QMCD_OK;
     }
     return QMCD_EINVAL;

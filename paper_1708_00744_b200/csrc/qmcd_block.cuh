@@ -24,17 +24,22 @@
 
 __host__ __device__ inline int qmcd_blk_Kp(int K) { return (K + 7) & ~7; }
 __host__ __device__ inline int qmcd_blk_RL(int K) { return 2 * qmcd_blk_Kp(K) + QMCD_TB; }
-// As[2][32][LDA] | recv[16][RL] | G[16][RL] | pq[2][2][Kp] | ub[16]
+// As[2][32][LDA] | recv[16][RL] | G[16][RL] | ub[16] | Rb[16] | Z[2][16][16] | Xm[Kp][16] | Ym[16][Kp] | Um[Kp][16]
 __host__ __device__ inline size_t qmcd_blk_smem_bytes(int K) {
-    return ((size_t)2 * 32 * QMCD_BLK_LDA + (size_t)2 * QMCD_TB * qmcd_blk_RL(K) + 4 * (size_t)qmcd_blk_Kp(K) + 16) * 8;
+    return ((size_t)2 * 32 * QMCD_BLK_LDA + (size_t)2 * QMCD_TB * qmcd_blk_RL(K) + 32 + 2 * QMCD_TB * QMCD_TB + 3 * (size_t)QMCD_TB * qmcd_blk_Kp(K) + 8) * 8;
 }
 
 struct QmcdBlk {
     double* As;     // [2][32][LDA]  rows 0..15: B0[j_tl, chunk], rows 16..31: v_tl[chunk]
     double* recv;   // [S][RPO][RL]  partial strips of the rows this CTA reduces
     double* G;      // [16][RL]      reduced strips: P | Q | D
-    double* pq;     // [2][2][Kp]    p, q of the current move, double buffered by move parity
+    double* Z;      // [2][16][16]   e_jt^T A_cur^-1 v_s of the block, ping-pong over accepted moves
+    double* Xm;     // [Kp][16]      M0 Q^T
+    double* Ym;     // [16][Kp]      P M0
+    double* Um;     // [Kp][16]      X Zc^-1
+    int* al;        // [16]          block index of the e-th accepted move
     double* ub;     // [16]          decision inputs of the block (uniform or mask as 0/1)
+    double* Rb;     // [16]          ratios of the block (written to R_out at the block's end)
 };
 
 __device__ inline QmcdBlk qmcd_blk_carve(double* base, int K) {
@@ -43,8 +48,13 @@ __device__ inline QmcdBlk qmcd_blk_carve(double* base, int K) {
     x.As = base; base += 2 * 32 * QMCD_BLK_LDA;
     x.recv = base; base += QMCD_TB * RL;
     x.G = base; base += QMCD_TB * RL;
-    x.pq = base; base += 4 * qmcd_blk_Kp(K);
-    x.ub = base;
+    x.ub = base; base += 16;
+    x.Rb = base; base += 16;
+    x.Z = base; base += 2 * QMCD_TB * QMCD_TB;
+    x.Xm = base; base += QMCD_TB * qmcd_blk_Kp(K);
+    x.Ym = base; base += QMCD_TB * qmcd_blk_Kp(K);
+    x.Um = base; base += QMCD_TB * qmcd_blk_Kp(K);
+    x.al = reinterpret_cast<int*>(base);
     return x;
 }
 
@@ -95,7 +105,7 @@ __device__ __forceinline__ const double* qmcd_blk_right(const QmcdArgs& A, const
 //   G[tl][Kp + i]       = Q[tl][i]   i < m0
 //   G[tl][2 Kp + sl]    = D[tl][sl] = B0[j_tl,:] . v_sl
 // ---------------------------------------------------------------------------
-__device__ void qmcd_blk_strips(const QmcdArgs& A, const QmcdSmem& s, const QmcdBlk& x, cg::cluster_group& cl,
+__device__ __noinline__ void qmcd_blk_strips(const QmcdArgs& A, const QmcdSmem& s, const QmcdBlk& x, cg::cluster_group& cl,
                                 const QmcdWalker& w, int t0, int L, int m0) {
     const QmcdDev& P = A.P;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, g = lane >> 2, c = lane & 3;
@@ -204,14 +214,32 @@ __device__ void qmcd_blk_strips(const QmcdArgs& A, const QmcdSmem& s, const Qmcd
 // The sweep loop in blocks (M in shared memory, replicated in every CTA).
 // Returns the queue length at the end.  Every CTA of the cluster runs the same
 // code on the same reduced numbers, so decisions agree without communication.
+//
+// Inside a block the look-ahead of Eq. 3 is a 16 x 16 elimination.  With M0 the
+// inverse of S at the block's start,
+//     Z[t][s] = D[t][s] - P[t,:] M0 Q[s,:]^T  =  e_{j_t}^T A_cur^-1 v_s     (t, s < L)
+// is formed for ALL moves of the block at once; the ratio of move t is Z[t][t]
+// (the Schur complement of the bordered S), and accepting move e
+// applies the sweep operator on index e:
+//     Z[i][j] -= Z[i][e] Z[e][j] / Z[e][e],  Z[e][j] /= Z[e][e],  Z[i][e] /= -Z[e][e],  Z[e][e] = 1/Z[e][e]
+// -- one element per thread, one barrier per ACCEPTED move, nothing for a rejected
+// one.  After the block the swept part of Z is Zc^-1 (Zc = Z0 on the accepted
+// moves), and M = S^-1 for the grown queue follows from the block-bordering
+// identity  M11 = M0 + X Zc^-1 Y,  M12 = -X Zc^-1,  M21 = -Zc^-1 Y,  M22 = Zc^-1
+// with X = M0 Q_acc^T, Y = P_acc M0 (formed with Z0, in parallel, at the start).
+// In exact arithmetic this is the move-by-move bordering of qmcd_accept_update.
 // ---------------------------------------------------------------------------
 __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group& cl,
                                   const QmcdWalker& w, int m) {
     const QmcdDev& P = A.P;
-    const int tid = threadIdx.x, lane = tid & 31;
+    const int tid = threadIdx.x;
     const int N = P.N, K = P.K, Kp = qmcd_blk_Kp(K), RL = qmcd_blk_RL(K), ldM = qmcd_ldM(K);
     const int len = w.khi - w.klo;
     const QmcdBlk x = qmcd_blk_carve(s.rs, K);
+    // cycle accounting by one thread of the leader CTA (every phase boundary is a barrier)
+    const bool prof = (w.r == 0 && tid == 0);
+    long long cy_la = 0, cy_chain = 0, cy_app = 0, cy_fl = 0, c0 = prof ? clock64() : 0, c_start = c0;
+#define QMCD_TICK(acc_) do { if (prof) { const long long c1_ = clock64(); (acc_) += c1_ - c0; c0 = c1_; } } while (0)
     int t = 0;
     while (t < A.n_moves) {
         const int j0 = (A.j_begin + t) % N;
@@ -230,7 +258,13 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
                 __syncthreads();
                 L = s.iflag[0];
                 __syncthreads();
-                if (L == 0) { qmcd_flush_phase<true>(P, s, cl, w, m); m = 0; continue; }
+                if (L == 0) {
+                    QMCD_TICK(cy_la);
+                    qmcd_flush_phase<true>(P, s, cl, w, m);
+                    QMCD_TICK(cy_fl);
+                    m = 0;
+                    continue;
+                }
             }
         }
         if (tid < L) {
@@ -247,54 +281,43 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
             }
         }
         qmcd_blk_strips(A, s, x, cl, w, t, L, m);
+        QMCD_TICK(cy_la);
 
         const int m0 = m;
+        // ---- X = M0 Q^T (Xm[i][t]) and Y = P M0 (Ym[t][b]) for every move of the block
+        for (int idx = tid; idx < m0 * QMCD_TB; idx += QMCD_THREADS) {
+            const int i = idx >> 4, tl = idx & 15;
+            double xa = 0.0, ya = 0.0;
+            if (tl < L) {
+                const double* Gq = x.G + (size_t)tl * RL + Kp;      // Q[tl][:]
+                const double* Gp = x.G + (size_t)tl * RL;           // P[tl][:]
+                for (int b = 0; b < m0; ++b) {
+                    xa += s.Ms[(size_t)i * ldM + b] * Gq[b];
+                    ya += Gp[b] * s.Ms[(size_t)b * ldM + i];
+                }
+            }
+            x.Xm[i * QMCD_TB + tl] = xa;
+            x.Ym[tl * Kp + i] = ya;
+        }
+        __syncthreads();
+        // ---- Z0 = D - P X : one element per thread
+        double* Zc = x.Z;                                  // current / next buffer (ping-pong)
+        double* Zn = x.Z + QMCD_TB * QMCD_TB;
+        {
+            const int ti = tid >> 4, sj = tid & 15;
+            double z = 0.0;
+            if (ti < L && sj < L) {
+                z = x.G[(size_t)ti * RL + 2 * Kp + sj];
+                const double* Gp = x.G + (size_t)ti * RL;
+                for (int i = 0; i < m0; ++i) z -= Gp[i] * x.Xm[i * QMCD_TB + sj];
+            }
+            Zc[tid] = z;
+        }
+        __syncthreads();
         unsigned accmask = 0;
         int na = 0;
         for (int tl = 0; tl < L; ++tl) {
-            const int mc = m0 + na;
-            const int j = (j0 + tl) % N;
-            const double* Grow = x.G + (size_t)tl * RL;
-            double* pf = x.pq + (size_t)(tl & 1) * 2 * Kp;
-            double* qf = pf + Kp;
-            // p, q of this move from the strips
-            for (int i = tid; i < mc; i += QMCD_THREADS) {
-                double p, q;
-                if (i < m0) { p = Grow[i]; q = Grow[Kp + i]; }
-                else {
-                    const int al = __fns(accmask, 0, i - m0 + 1);
-                    p = Grow[2 * Kp + al];
-                    q = x.G[(size_t)al * RL + 2 * Kp + tl];
-                }
-                pf[i] = p; qf[i] = q;
-            }
-            const double d = Grow[2 * Kp + tl];
-            __syncthreads();
-            // c = M q, r = M^T p
-            {
-                const int h = tid & 7;
-                for (int x0 = 0; x0 < mc; x0 += QMCD_THREADS / 8) {
-                    const int xx = x0 + (tid >> 3);
-                    double ca = 0, ra = 0;
-                    if (xx < mc) {
-                        for (int b = h; b < mc; b += 8) {
-                            ca += s.Ms[(size_t)xx * ldM + b] * qf[b];
-                            ra += pf[b] * s.Ms[(size_t)b * ldM + xx];
-                        }
-                    }
-#pragma unroll
-                    for (int o = 4; o > 0; o >>= 1) {
-                        ca += __shfl_xor_sync(0xffffffffu, ca, o);
-                        ra += __shfl_xor_sync(0xffffffffu, ra, o);
-                    }
-                    if (xx < mc && h == 0) { s.cf[xx] = ca; s.rf[xx] = ra; }
-                }
-            }
-            __syncthreads();
-            double sum = 0;
-            for (int a = lane; a < mc; a += 32) sum += pf[a] * s.cf[a];
-            sum = qmcd_warp_sum(sum);
-            const double R = d - sum;
+            const double R = Zc[tl * QMCD_TB + tl];
             bool acc;
             if (A.uniforms) { const double pa = fmin(1.0, R * R); acc = x.ub[tl] < pa; }
             else acc = x.ub[tl] != 0.0;
@@ -302,26 +325,56 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
                 if (w.r == 0 && tid == 0) qmcd_set_status(P, QMCD_DEV_ESINGULAR, w.b, t + tl);
                 acc = false;
             }
-            if (w.r == 0 && tid == 0) {
-                const size_t tb = (size_t)(t + tl) * P.batch + w.b;
-                if (A.R_out) A.R_out[tb] = R;
-                if (A.acc_out) A.acc_out[tb] = acc ? 1 : 0;
-            }
+            if (tid == 0) x.Rb[tl] = R;
             if (acc) {
-                const double sigma = 1.0 / R;
-                for (int idx = tid; idx < mc * mc; idx += QMCD_THREADS) {
-                    const int a = idx / mc, bb = idx - a * mc;
-                    s.Ms[(size_t)a * ldM + bb] += sigma * s.cf[a] * s.rf[bb];
-                }
-                for (int a = tid; a < mc; a += QMCD_THREADS) {
-                    s.Ms[(size_t)a * ldM + mc] = -sigma * s.cf[a];
-                    s.Ms[(size_t)mc * ldM + a] = -sigma * s.rf[a];
-                }
-                if (tid == 0) { s.Ms[(size_t)mc * ldM + mc] = sigma; s.Js[mc] = j; }
+                // sweep operator on index tl: thread (i, jj) owns Z[i][jj]
+                const int i = tid >> 4, jj = tid & 15;
+                const double rp = 1.0 / R;
+                const double zie = Zc[i * QMCD_TB + tl], zej = Zc[tl * QMCD_TB + jj], zij = Zc[tid];
+                double zn;
+                if (i == tl) zn = (jj == tl) ? rp : zej * rp;
+                else zn = (jj == tl) ? -zie * rp : zij - zie * (zej * rp);
+                Zn[tid] = zn;
+                __syncthreads();
+                double* tmp = Zc; Zc = Zn; Zn = tmp;
                 accmask |= 1u << tl;
                 na += 1;
             }
         }
+        // ---- M for the grown queue (block bordering); al(e) = block index of the e-th accepted move
+        if (na > 0) {
+            int* al_s = x.al;
+            if (tid < na) al_s[tid] = __fns(accmask, 0, tid + 1);
+            __syncthreads();
+            // U = X Zc^-1 restricted to accepted moves: U[i][f] = sum_e Xm[i][al_e] W1[e][f], W1 = Z[al_e][al_f]
+            for (int idx = tid; idx < m0 * na; idx += QMCD_THREADS) {
+                const int i = idx / na, f = idx - i * na;
+                double u = 0.0;
+                for (int e = 0; e < na; ++e) u += x.Xm[i * QMCD_TB + al_s[e]] * Zc[al_s[e] * QMCD_TB + al_s[f]];
+                x.Um[i * QMCD_TB + f] = u;
+            }
+            __syncthreads();
+            // M11 += U Y_acc ; M12 = -U ; M21 = -W1 Y_acc ; M22 = W1
+            const int mn = m0 + na;
+            for (int idx = tid; idx < mn * mn; idx += QMCD_THREADS) {
+                const int a = idx / mn, b = idx - a * mn;
+                double v;
+                if (a < m0 && b < m0) {
+                    v = s.Ms[(size_t)a * ldM + b];
+                    for (int f = 0; f < na; ++f) v += x.Um[a * QMCD_TB + f] * x.Ym[al_s[f] * Kp + b];
+                } else if (a < m0) {
+                    v = -x.Um[a * QMCD_TB + (b - m0)];
+                } else if (b < m0) {
+                    v = 0.0;
+                    for (int f = 0; f < na; ++f) v -= Zc[al_s[a - m0] * QMCD_TB + al_s[f]] * x.Ym[al_s[f] * Kp + b];
+                } else {
+                    v = Zc[al_s[a - m0] * QMCD_TB + al_s[b - m0]];
+                }
+                s.Ms[(size_t)a * ldM + b] = v;
+            }
+            if (tid < na) s.Js[m0 + tid] = (j0 + al_s[tid]) % N;
+        }
+        QMCD_TICK(cy_chain);
         // ---- append the block's accepted moves to the queue: C[slot] = v, W[slot] = B0[j,:]
         {
             const int vpr = len >> 1;
@@ -333,15 +386,27 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
                 qmcd_stg128(w.C + (size_t)(m0 + e) * N + w.klo + k, vv.x, vv.y);
                 qmcd_stg128(w.W + (size_t)(m0 + e) * N + w.klo + k, bb.x, bb.y);
             }
+            __syncthreads();                       // Rb of the last move
+            if (w.r == 0 && tid < L) {
+                const size_t tb = (size_t)(t + tid) * P.batch + w.b;
+                if (A.R_out) A.R_out[tb] = x.Rb[tid];
+                if (A.acc_out) A.acc_out[tb] = (accmask >> tid) & 1u;
+            }
             if (w.r == 0) {
                 for (int e = tid; e < na; e += QMCD_THREADS) w.J[m0 + e] = (j0 + (int)__fns(accmask, 0, e + 1)) % N;
-                if (tid == 0) P.counters[(size_t)w.b * 2 + 0] += na;
+                if (tid == 0) P.counters[(size_t)w.b * 8 + 0] += na;
             }
         }
         m = m0 + na;
         t += L;
         __syncthreads();
-        if (m == K) { qmcd_flush_phase<true>(P, s, cl, w, m); m = 0; }
+        QMCD_TICK(cy_app);
+        if (m == K) { qmcd_flush_phase<true>(P, s, cl, w, m); m = 0; QMCD_TICK(cy_fl); }
     }
+    if (prof) {
+        long long* pc = P.counters + (size_t)w.b * 8;
+        pc[2] += cy_la; pc[3] += cy_chain; pc[4] += cy_app; pc[5] += cy_fl; pc[6] += clock64() - c_start;
+    }
+#undef QMCD_TICK
     return m;
 }

@@ -37,11 +37,12 @@ struct QmcdDev {
     double* sp;               // [batch][K]     staged p (delta term applied)
     double* sc;               // [batch][K]     staged c = M q
     double* sr;               // [batch][K]     staged r = M^T p
-    long long* counters;      // [batch][2]     accepted, flushes
+    long long* counters;      // [batch][8]     accepted, flushes, cycles: look-ahead, chain, queue append, flush, total
     int* status;              // [4]            sticky: code, walker, move counter
     int flush_path;           // 0 auto, 1 CUDA-core, 2 DMMA
     int mma_smem_ok;          // host: the DMMA flush's shared memory fits
     int m_in_smem;            // host: every CTA keeps its own copy of M in shared memory
+    int chain_regs;           // option: blocked look-ahead keeps M in registers when K <= 32
     int blk_ok;               // host: qmcd_sweep may use the blocked look-ahead (qmcd_block.cuh)
 };
 

@@ -20,8 +20,8 @@ __device__ void qmcd_flush_rows(const QmcdDev& P, const QmcdSmem& s, cg::cluster
 // s.iflag[8] counts the flushes of this launch (same value in every CTA).
 template <bool MS>
 __device__ void qmcd_flush_phase(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
-                                 const QmcdWalker& w, int m) {
-    qmcd_writeback_M<MS>(P, s, w, m);
+                                 const QmcdWalker& w, int m, bool writeback = true) {
+    if (writeback) qmcd_writeback_M<MS>(P, s, w, m);
     if (P.S > 1) cl.sync(); else __syncthreads();
     const int k = s.iflag[8] + 1;
     if (P.G_act > 1 && w.r == 0 && threadIdx.x == 0) {
@@ -33,7 +33,7 @@ __device__ void qmcd_flush_phase(const QmcdDev& P, const QmcdSmem& s, cg::cluste
     if (threadIdx.x == 0) s.iflag[8] = k;
     if (w.r == 0 && threadIdx.x == 0) {
         P.m[w.b] = 0;
-        P.counters[(size_t)w.b * 2 + 1] += 1;
+        P.counters[(size_t)w.b * 8 + 1] += 1;
         const unsigned long long want = ((unsigned long long)P.launch_id << 32) | (unsigned)k;
         for (int g = 1; g < P.G_act; ++g)
             while (qmcd_ld_acquire(P.done + (size_t)w.b * 8 + g) != want) __nanosleep(64);
@@ -102,7 +102,7 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
     if (A.mode == QMCD_MODE_RATIO) {
         int j = A.jv ? A.jv[b] : A.j;
         if (j < 0 || j >= P.N) {
-            if (r == 0 && tid == 0) { qmcd_set_status(P, QMCD_DEV_EINVAL, b, P.counters[(size_t)b * 2]); P.sj[b] = -1; A.R_out[b] = 0.0; }
+            if (r == 0 && tid == 0) { qmcd_set_status(P, QMCD_DEV_EINVAL, b, P.counters[(size_t)b * 8]); P.sj[b] = -1; A.R_out[b] = 0.0; }
             return;   // uniform over the cluster
         }
         qmcd_load_state<MS>(P, s, w, m);
@@ -124,7 +124,7 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
         if (A.uniforms) { double pa = fmin(1.0, R * R); acc = A.uniforms[b] < pa; }
         else acc = A.accept_all || (A.mask[b] != 0);
         if (acc && (R == 0.0 || !isfinite(R))) {
-            if (r == 0 && tid == 0) qmcd_set_status(P, QMCD_DEV_ESINGULAR, b, P.counters[(size_t)b * 2]);
+            if (r == 0 && tid == 0) qmcd_set_status(P, QMCD_DEV_ESINGULAR, b, P.counters[(size_t)b * 8]);
             acc = false;
         }
         if (r == 0 && tid == 0) {
@@ -160,6 +160,8 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
         return;
     }
     const int len = w.khi - w.klo;
+    const bool prof = (r == 0 && tid == 0);
+    long long cy_la = 0, cy_acc = 0, c0 = prof ? clock64() : 0, c_start = c0;
     for (int t = 0; t < A.n_moves; ++t) {
         const int j = (A.j_begin + t) % P.N;
         const size_t tb = (size_t)t * P.batch + b;
@@ -175,6 +177,7 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
         }
         bool inq;
         double R = qmcd_lookahead<MS>(P, s, cl, w, j, m, A.v + tb * P.N, pbuf, &inq);
+        if (prof) { const long long c1 = clock64(); cy_la += c1 - c0; c0 = c1; }
         bool acc;
         if (A.uniforms) { double pa = fmin(1.0, R * R); acc = u < pa; }
         else acc = mk != 0;
@@ -187,8 +190,13 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
             if (A.acc_out) A.acc_out[tb] = acc ? 1 : 0;
         }
         if (acc) m = qmcd_do_accept<MS>(P, s, cl, w, j, m, R, inq, pbuf);
+        if (prof) { const long long c1 = clock64(); cy_acc += c1 - c0; c0 = c1; }   // accept + flush (per-move path)
     }
     qmcd_writeback_M<MS>(P, s, w, m);
+    if (prof) {
+        long long* pc = P.counters + (size_t)b * 8;
+        pc[2] += cy_la; pc[5] += cy_acc; pc[6] += clock64() - c_start;
+    }
     if (r == 0 && tid == 0) { P.sj[b] = -1; P.m[b] = m; }
 }
 

@@ -193,7 +193,7 @@ __device__ void qmcd_accept_update(const QmcdDev& P, const QmcdSmem& s, const Qm
         s.Js[m] = j;
         if (w.r == 0) {
             w.J[m] = j;
-            P.counters[(size_t)w.b * 2 + 0] += 1;
+            P.counters[(size_t)w.b * 8 + 0] += 1;
         }
     }
     __syncthreads();

@@ -414,7 +414,8 @@ def test_sweep_host_matches_device_sweep(qmcd):
     need = qmcd.load().qmcd_sweep_host_min_staging(wl.N, wl.batch)
     staging = torch.empty(need * 7 + 256, dtype=torch.uint8, device="cuda")   # forces many chunks
     q.sweep_host(0, Ph, mask=Mh, R_out=Rh, acc_out=Ah, staging=staging)
-    assert np.array_equal(Rh.numpy(), ref["R"])
+    # chunk boundaries cut the look-ahead blocks elsewhere: same numbers to rounding
+    assert _rel(Rh.numpy(), ref["R"]) <= 1e-12
     assert np.array_equal(Ah.numpy(), ref["acc"])
-    assert np.array_equal(B.cpu().numpy(), ref["B"])
+    assert np.max(np.abs(B.cpu().numpy() - ref["B"])) <= 1e-12
     q.close()
