@@ -146,7 +146,7 @@ int qmcd_sweep_host(qmcd_handle h, int j_begin, int n_moves,
 size_t qmcd_sweep_host_min_staging(int N, int batch);
 
 /* Tuning / introspection.  set: "cluster" (CTAs per cluster, 1..16; resets
- * "clusters_per_walker" to 1), "clusters_per_walker" (1..4: cluster 0 of a walker
+ * "clusters_per_walker" to 1), "clusters_per_walker" (1..16, 1..4 when K > 64: cluster 0 of a walker
  * runs the look-ahead, all of them share the rows of a flush; they must all fit
  * on the device at once, else QMCD_EINVAL), "flush_path"
  * (0 auto, 1 CUDA-core, 2 DMMA), "lookahead" (qmcd_sweep: 0 auto = blocked

@@ -57,7 +57,7 @@ static WsLayout ws_layout(int N, int K, int batch) {
     L.counters = o; o += al256((size_t)batch * 8 * 8);
     L.status = o; o += 256;
     L.go = o; o += al256((size_t)batch * 8);
-    L.done = o; o += al256((size_t)batch * 8 * 8);
+    L.done = o; o += al256((size_t)batch * 16 * 8);
     L.total = o;
     return L;
 }
@@ -115,12 +115,15 @@ static int max_active_clusters(qmcd_ctx* h, int S, int nclusters) {
     return n;
 }
 
-// Largest G <= limit that keeps every CTA's flush row slice a multiple of 64 rows (1 otherwise).
-static int pick_G(int N, int S, int limit) {
-    if (limit > QMCD_GMAX) limit = QMCD_GMAX;
-    for (int G = limit; G > 1; --G)
-        if (N % (64 * S * G) == 0) return G;
-    return 1;
+// Clusters per walker: as many as fit, but no more workers (S*G CTAs) than 64-row tiles of B,
+// and at most QMCD_GMAX when the flush keeps one Y = M W per cluster (K > 64).
+static int pick_G(int N, int K, int S, int limit) {
+    const int gmax = (K <= 64) ? 16 : QMCD_GMAX;
+    if (limit > gmax) limit = gmax;
+    int by_tiles = (N / 64) / S;
+    if (N % 64 != 0 || by_tiles < 1) by_tiles = 1;
+    if (limit > by_tiles) limit = by_tiles;
+    return limit < 1 ? 1 : limit;
 }
 
 // with_helpers: the walker's helper clusters take part (launches that may flush many rows)
@@ -198,7 +201,7 @@ extern "C" int qmcd_create(qmcd_handle* out, int N, int K, int batch,
             if (rc != QMCD_OK) break;
             const int n = max_active_clusters(h, S, batch);
             if (n < batch && S > 1) continue;
-            const int G = (n >= batch) ? pick_G(N, S, n / batch) : 1;
+            const int G = (n >= batch) ? pick_G(N, K, S, n / batch) : 1;
             if (S * G > bestS * bestG) { bestS = S; bestG = G; }
         }
         if (rc != QMCD_OK) break;
@@ -397,8 +400,8 @@ extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
         return configure_kernel(h, value);
     }
     if (!strcmp(key, "clusters_per_walker")) {     // helper clusters spin on the leader: all must be co-resident
-        if (value < 1 || value > QMCD_GMAX) return QMCD_EINVAL;
-        if (value > 1 && (max_active_clusters(h, h->P.S, h->batch) < h->batch * value || h->N % (64 * h->P.S * value) != 0)) return QMCD_EINVAL;
+        if (value < 1 || value > ((h->K <= 64) ? 16 : QMCD_GMAX)) return QMCD_EINVAL;
+        if (value > 1 && max_active_clusters(h, h->P.S, h->batch) < h->batch * value) return QMCD_EINVAL;
         h->P.G = value;
         return QMCD_OK;
     }

@@ -64,24 +64,34 @@ __device__ __forceinline__ double2 qmcd_ldcg128(const double* p) {
     return v;
 }
 
-// Stage chunk kc (columns [klo + 64 kc, + cw)) of the block's left operands:
-// rows 0..15 = B0[j_tl, :], rows 16..31 = v_tl, tl < L (rows >= L are zeroed).
-__device__ __forceinline__ void qmcd_blk_stage(double* dst, const QmcdArgs& A, const QmcdWalker& w,
-                                               int t0, int L, int kc, int cw) {
+// Left operands of a block, staged chunk by chunk (64 columns): rows 0..15 = B0[j_tl, :],
+// rows 16..31 = v_tl, tl < L (rows >= L are zeroed).  Thread t copies vector (t & 31) of rows
+// (t >> 5) + 8 i, i < 4; the four source row pointers are computed once per block.
+struct QmcdBlkSrc { const double* p[4]; };
+__device__ __forceinline__ QmcdBlkSrc qmcd_blk_src(const QmcdArgs& A, const QmcdWalker& w, int t0, int L) {
+    QmcdBlkSrc r;
     const QmcdDev& P = A.P;
     const int N = P.N;
-    const int vpr = cw >> 1;                       // 16-byte vectors per row
-    for (int idx = threadIdx.x; idx < 32 * vpr; idx += QMCD_THREADS) {
-        const int row = idx / vpr, c2 = (idx - row * vpr) * 2;
-        const int tl = row & 15;
-        double* d = dst + row * QMCD_BLK_LDA + c2;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int row = (threadIdx.x >> 5) + 8 * i, tl = row & 15;
+        r.p[i] = nullptr;
         if (tl < L) {
-            const int col = w.klo + kc * QMCD_BLK_KC + c2;
-            const double* src;
-            if (row < 16) { int j = A.j_begin + t0 + tl; j %= N; src = w.B + (size_t)j * N + col; }
-            else src = A.v + ((size_t)(t0 + tl) * P.batch + w.b) * N + col;
-            qmcd_cp_async16(d, src);
-        } else { d[0] = 0.0; d[1] = 0.0; }
+            if (row < 16) { int j = A.j_begin + t0 + tl; j %= N; r.p[i] = w.B + (size_t)j * N + w.klo; }
+            else r.p[i] = A.v + ((size_t)(t0 + tl) * P.batch + w.b) * N + w.klo;
+        }
+    }
+    return r;
+}
+__device__ __forceinline__ void qmcd_blk_stage(double* dst, const QmcdBlkSrc& src, int kc, int cw) {
+    const int c2 = (threadIdx.x & 31) * 2;
+    if (c2 >= cw) return;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int row = (threadIdx.x >> 5) + 8 * i;
+        double* d = dst + row * QMCD_BLK_LDA + c2;
+        if (src.p[i]) qmcd_cp_async16(d, src.p[i] + kc * QMCD_BLK_KC + c2);
+        else { d[0] = 0.0; d[1] = 0.0; }
     }
 }
 
@@ -126,12 +136,13 @@ __device__ __noinline__ void qmcd_blk_strips(const QmcdArgs& A, const QmcdSmem& 
 #pragma unroll
     for (int i = 0; i < QMCD_BLK_MAXU; ++i) { acc[i][0][0] = acc[i][0][1] = acc[i][1][0] = acc[i][1][1] = 0.0; }
 
-    qmcd_blk_stage(x.As, A, w, t0, L, 0, min(QMCD_BLK_KC, len));
+    const QmcdBlkSrc src = qmcd_blk_src(A, w, t0, L);
+    qmcd_blk_stage(x.As, src, 0, min(QMCD_BLK_KC, len));
     qmcd_cp_async_commit();
     for (int kc = 0; kc < nchunks; ++kc) {
         const int cw = min(QMCD_BLK_KC, len - kc * QMCD_BLK_KC);
         if (kc + 1 < nchunks) {
-            qmcd_blk_stage(x.As + ((kc + 1) & 1) * 32 * QMCD_BLK_LDA, A, w, t0, L, kc + 1,
+            qmcd_blk_stage(x.As + ((kc + 1) & 1) * 32 * QMCD_BLK_LDA, src, kc + 1,
                            min(QMCD_BLK_KC, len - (kc + 1) * QMCD_BLK_KC));
             qmcd_cp_async_commit();
         }

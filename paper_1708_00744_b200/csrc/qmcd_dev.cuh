@@ -24,7 +24,7 @@ struct QmcdDev {
     unsigned launch_id;       // host counter, tags the go / done words of this launch
     size_t y_stride;          // doubles between the Y copies of two clusters of one walker
     unsigned long long* go;   // [batch]      leader -> helpers: (launch id << 32) | (flush no. << 12) | m
-    unsigned long long* done; // [batch][8]   helper g -> leader: (launch id << 32) | flush no.
+    unsigned long long* done; // [batch][16]   helper g -> leader: (launch id << 32) | flush no.
     double* B;                // [batch][N][N]  inverse, borrowed, updated in place
     double* C;                // [batch][K][N]  queued new columns v_i (one per row)
     double* W;                // [batch][K][N]  rows j_i of the stale inverse B0

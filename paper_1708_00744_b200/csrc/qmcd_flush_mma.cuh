@@ -23,7 +23,8 @@ __host__ __device__ inline int qmcd_mma_rows(int K) { return (K <= 64) ? 128 : 6
 __host__ __device__ inline int qmcd_mma_stages(int K) { return (K <= 128) ? 3 : 2; }
 __host__ __device__ inline size_t qmcd_flush_mma_smem_bytes(int N, int K) {
     (void)N;
-    return (size_t)qmcd_mma_rows(K) * qmcd_mma_ldT(K) * 8 + qmcd_mma_stages(K) * (size_t)QMCD_MMA_CHUNK_DOUBLES * 8;
+    return (size_t)qmcd_mma_rows(K) * qmcd_mma_ldT(K) * 8 + qmcd_mma_stages(K) * (size_t)QMCD_MMA_CHUNK_DOUBLES * 8 +
+           (K <= 64 ? (size_t)64 * QMCD_MMA_LDX * 8 : 0);      // + M for the local T M stage
 }
 
 __device__ __forceinline__ void qmcd_dmma(double& d0, double& d1, double a, double b) {
@@ -41,7 +42,8 @@ template <int N_> __device__ __forceinline__ void qmcd_cp_async_wait() {
 
 __device__ inline bool qmcd_flush_use_mma(const QmcdDev& P, int m, int G_act) {
     if (P.flush_path == 1) return false;
-    const bool ok = (P.N % 64 == 0) && ((P.N / P.S) % 64 == 0) && ((P.N / (P.S * G_act)) % 64 == 0) && P.mma_smem_ok;
+    (void)G_act;
+    const bool ok = (P.N % 64 == 0) && ((P.N / P.S) % 64 == 0 || P.K <= 64) && P.mma_smem_ok;
     if (!ok) return false;
     if (P.flush_path == 2) return true;
     return m >= 2;
@@ -355,6 +357,61 @@ __device__ void qmcd_mma_nn(const double* __restrict__ Ts, int ldT, int kext,
     qmcd_cp_async_wait<0>();
 }
 
+// ---------------------------------------------------------------------------
+// TM stage (m <= 64):  Ts <- Ts M  in place, warp-local (a warp owns its rows of Ts
+// over all columns).  Mf: M staged in shared memory, [64][LDX], zero outside m x m.
+// With it B <- B0 + Ts W needs neither Y = M W nor a barrier across the cluster.
+// ---------------------------------------------------------------------------
+template <int A_T>
+__device__ void qmcd_mma_tm(double* __restrict__ Ts, int ldT, int mp8, const double* __restrict__ Mf) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
+    const int nq = mp8 >> 3, nG = (mp8 + 15) >> 4;
+    double* tp[A_T];
+#pragma unroll
+    for (int a = 0; a < A_T; ++a) tp[a] = Ts + (size_t)(wid * 8 * A_T + a * 8 + g) * ldT;
+    double acc[A_T][4][2][2];
+#pragma unroll
+    for (int a = 0; a < A_T; ++a)
+#pragma unroll
+        for (int G = 0; G < 4; ++G) { acc[a][G][0][0] = acc[a][G][0][1] = acc[a][G][1][0] = acc[a][G][1][1] = 0.0; }
+    const double* xb = Mf + (2 * c) * QMCD_MMA_LDX + 2 * g;
+    for (int q = 0; q < nq; ++q) {
+        double2 avv[A_T];
+#pragma unroll
+        for (int a = 0; a < A_T; ++a) avv[a] = qmcd_lds128(tp[a] + 2 * c + 8 * q);
+#pragma unroll
+        for (int G = 0; G < 4; ++G) {
+            if (G < nG) {
+                const double2 x0 = qmcd_lds128(xb + (8 * q) * QMCD_MMA_LDX + 16 * G);
+                const double2 x1 = qmcd_lds128(xb + (8 * q + 1) * QMCD_MMA_LDX + 16 * G);
+#pragma unroll
+                for (int a = 0; a < A_T; ++a) {
+                    qmcd_dmma(acc[a][G][0][0], acc[a][G][0][1], avv[a].x, x0.x);
+                    qmcd_dmma(acc[a][G][1][0], acc[a][G][1][1], avv[a].x, x0.y);
+                    qmcd_dmma(acc[a][G][0][0], acc[a][G][0][1], avv[a].y, x1.x);
+                    qmcd_dmma(acc[a][G][1][0], acc[a][G][1][1], avv[a].y, x1.y);
+                }
+            }
+        }
+    }
+    __syncwarp();                                    // all lanes have read this warp's rows of Ts
+#pragma unroll
+    for (int a = 0; a < A_T; ++a)
+#pragma unroll
+        for (int G = 0; G < 4; ++G)
+            if (G < nG) {                            // columns 16 G + 4 c .. + 3 (may reach into the row's padding: ldT >= mp8 + 8)
+                *reinterpret_cast<double2*>(tp[a] + 16 * G + 4 * c) = make_double2(acc[a][G][0][0], acc[a][G][1][0]);
+                *reinterpret_cast<double2*>(tp[a] + 16 * G + 4 * c + 2) = make_double2(acc[a][G][0][1], acc[a][G][1][1]);
+            }
+    __syncwarp();
+}
+
+// Tiles of R rows of B are dealt round-robin to the walker's workers (every CTA of
+// every participating cluster; helper clusters first, the leader cluster last).
+__device__ __forceinline__ int qmcd_worker_id(const QmcdDev& P, const QmcdWalker& w) {
+    return (w.g == 0) ? (P.G_act - 1) * P.S + w.r : (w.g - 1) * P.S + w.r;
+}
+
 template <int A_T, int NS>
 __device__ void qmcd_flush_mma_impl(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
                                     const QmcdWalker& w, int m) {
@@ -364,6 +421,25 @@ __device__ void qmcd_flush_mma_impl(const QmcdDev& P, const QmcdSmem& s, cg::clu
     const int mp8 = (m + 7) & ~7;
     double* Ts = reinterpret_cast<double*>(s.dyn);
     double* cb = Ts + (size_t)qmcd_mma_rows(K) * ldT;
+    const int NW = P.G_act * P.S, wf = qmcd_worker_id(P, w);
+    const int ntiles = (N + R - 1) / R;
+    if (K <= 64) {
+        // ---- local path: T = -(B C^T - E_J); T <- T M; B += T W.  No Y, no cluster barrier.
+        double* Mf = cb + (size_t)NS * QMCD_MMA_CHUNK_DOUBLES;
+        for (int idx = tid; idx < 64 * 64; idx += QMCD_THREADS) {
+            const int a = idx >> 6, b = idx & 63;
+            Mf[a * QMCD_MMA_LDX + b] = (a < m && b < m) ? __ldcg(w.M + (size_t)a * K + b) : 0.0;
+        }
+        for (int tile = wf; tile < ntiles; tile += NW) {
+            const int row0 = tile * R, nvalid = min(R, N - row0);
+            if (mp8 <= 32) qmcd_mma_nt<A_T, 4, NS>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
+            else qmcd_mma_nt<A_T, 8, NS>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
+            qmcd_mma_tm<A_T>(Ts, ldT, mp8, Mf);      // (the NT stage ended with a barrier: Mf and Ts are visible)
+            qmcd_mma_nn<A_T, true, NS>(Ts, ldT, mp8, w.W, m, N, w.B, row0, nvalid, 0, N, cb);
+            __syncthreads();
+        }
+        return;
+    }
     // ---- Y = M W on my column slice, M taken R rows at a time as the A operand
     for (int r0 = 0; r0 < m; r0 += R) {
         for (int idx = tid; idx < R * mp8; idx += QMCD_THREADS) {
@@ -375,9 +451,9 @@ __device__ void qmcd_flush_mma_impl(const QmcdDev& P, const QmcdSmem& s, cg::clu
         __syncthreads();
     }
     if (P.S > 1) cl.sync(); else __syncthreads();
-    // ---- my row slice, R rows at a time:  T = -(B C^T - E_J);  B += T Y
-    for (int row0 = w.rlo; row0 < w.rhi; row0 += R) {
-        const int nvalid = min(R, w.rhi - row0);
+    // ---- my tiles:  T = -(B C^T - E_J);  B += T Y
+    for (int tile = wf; tile < ntiles; tile += NW) {
+        const int row0 = tile * R, nvalid = min(R, N - row0);
         if (mp8 <= 32) qmcd_mma_nt<A_T, 4, NS>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
         else qmcd_mma_nt<A_T, 8, NS>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
         qmcd_mma_nn<A_T, true, NS>(Ts, ldT, mp8, w.Y, m, N, w.B, row0, nvalid, 0, N, cb);
@@ -385,10 +461,12 @@ __device__ void qmcd_flush_mma_impl(const QmcdDev& P, const QmcdSmem& s, cg::clu
     }
 }
 
+// 128-row tiles when there are enough of them for every worker, else 64-row tiles
 __device__ inline void qmcd_flush_mma(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
                                       const QmcdWalker& w, int m) {
+    const int NW = P.G_act * P.S;
     if (qmcd_mma_stages(P.K) == 3) {
-        if (qmcd_mma_rows(P.K) == 128 && (w.rhi - w.rlo) >= 128) qmcd_flush_mma_impl<2, 3>(P, s, cl, w, m);
+        if (qmcd_mma_rows(P.K) == 128 && P.N / 128 >= NW) qmcd_flush_mma_impl<2, 3>(P, s, cl, w, m);
         else qmcd_flush_mma_impl<1, 3>(P, s, cl, w, m);
     } else {
         qmcd_flush_mma_impl<1, 2>(P, s, cl, w, m);

@@ -36,7 +36,7 @@ __device__ void qmcd_flush_phase(const QmcdDev& P, const QmcdSmem& s, cg::cluste
         P.counters[(size_t)w.b * 8 + 1] += 1;
         const unsigned long long want = ((unsigned long long)P.launch_id << 32) | (unsigned)k;
         for (int g = 1; g < P.G_act; ++g)
-            while (qmcd_ld_acquire(P.done + (size_t)w.b * 8 + g) != want) __nanosleep(64);
+            while (qmcd_ld_acquire(P.done + (size_t)w.b * 16 + g) != want) __nanosleep(64);
     }
     if (P.S > 1) cl.sync(); else __syncthreads();
 }
@@ -64,7 +64,7 @@ __device__ void qmcd_helper_loop(const QmcdDev& P, const QmcdSmem& s, cg::cluste
         if (P.S > 1) cl.sync(); else __syncthreads();      // the whole cluster is done with its rows
         if (w.r == 0 && threadIdx.x == 0) {
             __threadfence();
-            qmcd_st_release(P.done + (size_t)w.b * 8 + w.g, ((unsigned long long)P.launch_id << 32) | (unsigned)k);
+            qmcd_st_release(P.done + (size_t)w.b * 16 + w.g, ((unsigned long long)P.launch_id << 32) | (unsigned)k);
         }
     }
 }
