@@ -196,13 +196,17 @@ extern "C" int qmcd_create(qmcd_handle* out, int N, int K, int batch,
         // its leader, so all batch*G clusters must be co-resident); ties go to the larger S.
         const int s_cap = default_cluster(N, batch, 16 * batch, h->max_cluster);   // N / 64 and 16 cap it
         int bestS = 1, bestG = 1;
+        double best_score = 0.0;
         for (int S = s_cap; S >= 1; S /= 2) {
             rc = configure_kernel(h, S);
             if (rc != QMCD_OK) break;
             const int n = max_active_clusters(h, S, batch);
             if (n < batch && S > 1) continue;
             const int G = (n >= batch) ? pick_G(N, K, S, n / batch) : 1;
-            if (S * G > bestS * bestG) { bestS = S; bestG = G; }
+            // SMs per walker, with a bonus for clusters of >= 4: the look-ahead products run on the
+            // leader cluster only and cost ~N/S per CTA (measured: c4 with S=2,G=9 is slower than S=4,G=4)
+            const double score = (double)(S * G) * (S >= 4 ? 1.25 : 1.0);
+            if (score > best_score) { best_score = score; bestS = S; bestG = G; }
         }
         if (rc != QMCD_OK) break;
         rc = configure_kernel(h, bestS);
