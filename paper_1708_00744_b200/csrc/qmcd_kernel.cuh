@@ -36,7 +36,7 @@ __device__ void qmcd_flush_phase(const QmcdDev& P, const QmcdSmem& s, cg::cluste
         P.counters[(size_t)w.b * 8 + 1] += 1;
         const unsigned long long want = ((unsigned long long)P.launch_id << 32) | (unsigned)k;
         for (int g = 1; g < P.G_act; ++g)
-            while (qmcd_ld_acquire(P.done + (size_t)w.b * 16 + g) != want) __nanosleep(64);
+            while (qmcd_ld_acquire(P.done + (size_t)w.b * 16 + g) != want) __nanosleep(20);
     }
     if (P.S > 1) cl.sync(); else __syncthreads();
 }
@@ -53,7 +53,7 @@ __device__ void qmcd_helper_loop(const QmcdDev& P, const QmcdSmem& s, cg::cluste
                     const unsigned f = (unsigned)(v >> 12) & 0xFFFFFu;
                     if (f == QMCD_GO_EXIT || f == (unsigned)k) break;
                 }
-                __nanosleep(64);
+                __nanosleep(20);
             }
             s.iflag[9] = (((unsigned)(v >> 12) & 0xFFFFFu) == QMCD_GO_EXIT) ? -1 : (int)(v & 0xFFFu);
         }
