@@ -96,6 +96,8 @@ static int configure_kernel(qmcd_ctx* h, int S) {
     // the attribute is per function, not per handle: always allow the device maximum
     CK(h, cudaFuncSetAttribute(qmcd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     CK(h, cudaFuncSetAttribute(qmcd_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    CK(h, cudaFuncSetAttribute(qmcd_kernel_sweep, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    CK(h, cudaFuncSetAttribute(qmcd_kernel_sweep, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     h->smem_bytes = smem;
     h->P.S = S;
     return QMCD_OK;
@@ -144,7 +146,8 @@ static int launch(qmcd_ctx* h, QmcdArgs& a, bool with_helpers) {
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    CK(h, cudaLaunchKernelEx(&cfg, qmcd_kernel, a));
+    if (a.mode == QMCD_MODE_SWEEP && a.blocked && h->P.m_in_smem) CK(h, cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep, a));
+    else CK(h, cudaLaunchKernelEx(&cfg, qmcd_kernel, a));
     return QMCD_OK;
 }
 

@@ -200,7 +200,10 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
     if (r == 0 && tid == 0) { P.sj[b] = -1; P.m[b] = m; }
 }
 
-__global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel(const QmcdArgs A) {
+// Common prologue / epilogue of both entry points.  BLOCKED = true: the blocked sweep only (its
+// own register allocation: the per-move look-ahead of the generic entry is not compiled in).
+template <bool BLOCKED>
+__device__ __forceinline__ void qmcd_kernel_body(const QmcdArgs& A) {
     extern __shared__ __align__(1024) unsigned char qmcd_smem_raw[];
     const QmcdDev& P = A.P;
     cg::cluster_group cl = cg::this_cluster();
@@ -213,11 +216,22 @@ __global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel(const QmcdArgs A)
     if (threadIdx.x == 0) s.iflag[8] = 0;
     __syncthreads();
     if (g > 0) { qmcd_helper_loop(P, s, cl, w); return; }
-    if (P.m_in_smem) qmcd_run<true>(A, s, cl, w);
-    else qmcd_run<false>(A, s, cl, w);
-    if (P.G_act > 1) {                               // release the helpers (every return path of qmcd_run lands here)
+    if (BLOCKED) {
+        int m = __ldcg(P.m + b);
+        qmcd_load_state<true>(P, s, w, m);
+        m = qmcd_sweep_blocked(A, s, cl, w, m);
+        qmcd_writeback_M<true>(P, s, w, m);
+        if (r == 0 && threadIdx.x == 0) { P.sj[b] = -1; P.m[b] = m; }
+    } else {
+        if (P.m_in_smem) qmcd_run<true>(A, s, cl, w);
+        else qmcd_run<false>(A, s, cl, w);
+    }
+    if (P.G_act > 1) {                               // release the helpers (every return path lands here)
         if (S > 1) cl.sync(); else __syncthreads();
         if (r == 0 && threadIdx.x == 0)
             qmcd_st_release(P.go + b, ((unsigned long long)P.launch_id << 32) | ((unsigned long long)QMCD_GO_EXIT << 12));
     }
 }
+
+__global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel(const QmcdArgs A) { qmcd_kernel_body<false>(A); }
+__global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel_sweep(const QmcdArgs A) { qmcd_kernel_body<true>(A); }
