@@ -419,3 +419,65 @@ def test_sweep_host_matches_device_sweep(qmcd):
     assert np.array_equal(Ah.numpy(), ref["acc"])
     assert np.max(np.abs(B.cpu().numpy() - ref["B"])) <= 1e-12
     q.close()
+
+
+# ------------------------------------------------------------------ full-size configs, bench launch configuration
+def _residuals_numpy(wl, acc, B, walkers):
+    worst = 0.0
+    for w in walkers:
+        A_cur = inputs.current_matrix(wl.A[w], wl.proposals[:, w, :], acc[:, w], wl.n_moves)
+        worst = max(worst, float(np.max(np.abs(A_cur @ B[w] - np.eye(wl.N)))))
+    return worst
+
+
+def test_c2_full_size_sampled_walkers_vs_oracle_and_residuals(qmcd):
+    """BASELINE.json configs[2] at FULL size (64 walkers, N = 1024, 4 sweeps) in bench.py's launch
+    configuration (qmcd_sweep + qmcd_flush, library-chosen clusters), K = 64 and 32.
+    Sampled outputs: walkers 0 and 63 against the oracle's rank-1 path run on exactly those walkers
+    (a walker's data depend only on its seed); every walker: max|A.Ainv - I| <= 1e-8 after the run;
+    K-independence of all ratios.  Bernoulli(0.99) and the Metropolis rule."""
+    wl = inputs.make_config("c2")
+    sample = [0, wl.batch - 1]
+    for mode in ("bern0.99", "metropolis"):
+        mask = wl.bernoulli_mask(0.99) if mode == "bern0.99" else None
+        uni = wl.uniforms if mode == "metropolis" else None
+        g64 = gpu_sweep(qmcd, wl, 64, mask=mask, uniforms=uni)
+        assert g64["status"] == 0 and g64["blocked"]
+        Bs = np.ascontiguousarray(wl.Ainv[sample])
+        Ro, acco, _ = oracle.run(1, Bs, 1, np.ascontiguousarray(wl.proposals[:, sample, :]),
+                                 mask=None if mask is None else np.ascontiguousarray(mask[:, sample]),
+                                 uniforms=None if uni is None else np.ascontiguousarray(uni[:, sample]))
+        assert np.array_equal(g64["acc"][:, sample], acco)
+        assert _rel(g64["R"][:, sample], Ro) <= RTOL_RATIO
+        assert np.max(np.abs(g64["B"][sample] - Bs)) <= 1e-9
+        assert _residuals_numpy(wl, g64["acc"], g64["B"], range(0, wl.batch, 7)) <= TOL_RESID
+        assert 0.97 < g64["acc"].mean() < 1.0
+        if mode == "bern0.99":
+            g32 = gpu_sweep(qmcd, wl, 32, mask=mask)
+            assert np.array_equal(g32["acc"], g64["acc"])
+            assert _rel(g32["R"], g64["R"]) <= RTOL_RATIO
+            assert np.max(np.abs(g32["B"] - g64["B"])) <= 1e-9
+
+
+def test_c4_full_size_properties(qmcd):
+    """BASELINE.json configs[4] at FULL size (8 walkers, N = 4096, 1 sweep), bench launch
+    configuration, K = 64 (helper clusters) against K = 32: identical accept sequence, ratios
+    K-independent to 1e-10, max|A.Ainv - I| <= 1e-8 for every walker, and the
+    ratios of sampled moves against the plain definition det(A_new)/det(A_cur) by library LU."""
+    wl = inputs.make_config("c4")
+    mask = wl.bernoulli_mask(0.99)
+    g64 = gpu_sweep(qmcd, wl, 64, mask=mask)
+    assert g64["status"] == 0 and g64["blocked"]
+    g32 = gpu_sweep(qmcd, wl, 32, mask=mask)
+    assert np.array_equal(g64["acc"], mask) and np.array_equal(g32["acc"], mask)
+    assert _rel(g64["R"], g32["R"]) <= RTOL_RATIO
+    assert np.max(np.abs(g64["B"] - g32["B"])) <= 1e-9
+    assert _residuals_numpy(wl, mask, g64["B"], range(wl.batch)) <= TOL_RESID
+    # plain definition at sampled moves of walker 3 (explicit LU determinants, numpy/LAPACK)
+    w = 3
+    for t in (0, 70, 1500):
+        A_cur = inputs.current_matrix(wl.A[w], wl.proposals[:, w, :], mask[:, w], t)
+        A_new = A_cur.copy(); A_new[:, t % wl.N] = wl.proposals[t, w]
+        s0, l0 = np.linalg.slogdet(A_cur); s1, l1 = np.linalg.slogdet(A_new)
+        Rdef = s1 * s0 * np.exp(l1 - l0)
+        assert abs(g64["R"][t, w] - Rdef) <= 1e-9 * abs(Rdef)
