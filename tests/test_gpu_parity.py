@@ -481,3 +481,24 @@ def test_c4_full_size_properties(qmcd):
         s0, l0 = np.linalg.slogdet(A_cur); s1, l1 = np.linalg.slogdet(A_new)
         Rdef = s1 * s0 * np.exp(l1 - l0)
         assert abs(g64["R"][t, w] - Rdef) <= 1e-9 * abs(Rdef)
+
+
+def test_c3_full_size_properties(qmcd):
+    """BASELINE.json configs[3] at FULL size (32 walkers, N = 2048, 2 sweeps), bench launch
+    configuration: K = 64 against K = 128 (the Y = M W flush path): identical accept sequence,
+    K-independent ratios, residuals of sampled walkers, walker 5 against the oracle's
+    rank-1 path for the first 300 proposals."""
+    wl = inputs.make_config("c3")
+    mask = wl.bernoulli_mask(0.99)
+    g64 = gpu_sweep(qmcd, wl, 64, mask=mask)
+    g128 = gpu_sweep(qmcd, wl, 128, mask=mask)
+    assert g64["status"] == 0 and g128["status"] == 0
+    assert np.array_equal(g64["acc"], mask) and np.array_equal(g128["acc"], mask)
+    assert _rel(g64["R"], g128["R"]) <= RTOL_RATIO
+    assert np.max(np.abs(g64["B"] - g128["B"])) <= 1e-9
+    assert _residuals_numpy(wl, mask, g64["B"], (0, 13, 31)) <= TOL_RESID
+    w, nt = 5, 300
+    Bs = np.ascontiguousarray(wl.Ainv[w:w + 1])
+    Ro, acco, _ = oracle.run(1, Bs, 1, np.ascontiguousarray(wl.proposals[:nt, w:w + 1, :]),
+                             mask=np.ascontiguousarray(mask[:nt, w:w + 1]))
+    assert _rel(g64["R"][:nt, w:w + 1], Ro) <= RTOL_RATIO
