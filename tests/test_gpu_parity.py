@@ -502,3 +502,49 @@ def test_c3_full_size_properties(qmcd):
     Ro, acco, _ = oracle.run(1, Bs, 1, np.ascontiguousarray(wl.proposals[:nt, w:w + 1, :]),
                              mask=np.ascontiguousarray(mask[:nt, w:w + 1]))
     assert _rel(g64["R"][:nt, w:w + 1], Ro) <= RTOL_RATIO
+
+
+def test_blocked_sweep_singular_move_is_dropped_and_reported(qmcd):
+    """Reading G13 inside qmcd_sweep (blocked look-ahead): a proposal with R == 0 that the mask
+    accepts sets the sticky status, is NOT queued, and the rest of the run is unaffected."""
+    import torch
+    wl = inputs.make_workload(2, 128, 200, seed=41)
+    mask = wl.bernoulli_mask(0.9)
+    t_bad, w_bad = 37, 1
+    wl.proposals[t_bad, w_bad, :] = 0.0               # zero column: det(A_new) = 0 exactly
+    mask[t_bad, w_bad] = 1
+    ref_mask = mask.copy(); ref_mask[t_bad, w_bad] = 0  # what must effectively happen
+    Bo = wl.Ainv.copy(); Ro, acco, _ = oracle.run(2, Bo, 16, wl.proposals, mask=ref_mask)
+    g = gpu_sweep(qmcd, wl, 16, mask=mask)
+    assert g["blocked"] and g["status"] == qmcd.ESINGULAR and g["info"][0] == w_bad
+    assert g["R"][t_bad, w_bad] == 0.0 and g["acc"][t_bad, w_bad] == 0
+    assert np.array_equal(g["acc"], ref_mask)
+    ok = np.ones_like(mask, dtype=bool); ok[t_bad, w_bad] = False
+    assert _rel(g["R"][ok], Ro[ok]) <= RTOL_RATIO
+    assert np.max(np.abs(g["B"] - Bo)) <= 1e-10
+
+
+def test_helper_clusters_with_metropolis_and_single_moves(qmcd):
+    """Helper clusters under the Metropolis rule, driven by sweeps of 1, 2, 3, ... proposals
+    (blocks and windows cut at every launch boundary; M, J, m live in global memory in between)."""
+    import torch
+    N, K, batch = 256, 8, 3
+    wl = inputs.make_workload(batch, N, 120, seed=43)
+    Bo = wl.Ainv.copy(); Ro, acco, _ = oracle.run(2, Bo, K, wl.proposals, uniforms=wl.uniforms)
+    q = qmcd.Qmcd(N, K, batch)
+    q.set_option("cluster", 2); q.set_option("clusters_per_walker", 2)
+    B = _dev(wl.Ainv); q.set_inverse(B)
+    P, U = _dev(wl.proposals), _dev(wl.uniforms)
+    R = torch.zeros((wl.n_moves, batch), dtype=torch.float64, device="cuda")
+    acc = torch.zeros((wl.n_moves, batch), dtype=torch.uint8, device="cuda")
+    t, step = 0, 1
+    while t < wl.n_moves:
+        n = min(step, wl.n_moves - t)
+        q.sweep(t % N, P[t:t + n], uniforms=U[t:t + n], R_out=R[t:t + n], acc_out=acc[t:t + n])
+        t += n; step += 1
+    q.flush()
+    assert q.status()[0] == 0
+    assert np.array_equal(acc.cpu().numpy(), acco)
+    assert _rel(R.cpu().numpy(), Ro) <= RTOL_RATIO
+    assert np.max(np.abs(B.cpu().numpy() - Bo)) <= 1e-10
+    q.close()
