@@ -139,13 +139,20 @@ static int launch(qmcd_ctx* h, QmcdArgs& a, bool with_helpers) {
     cfg.blockDim = dim3(QMCD_THREADS, 1, 1);
     cfg.dynamicSmemBytes = h->smem_bytes;
     cfg.stream = h->stream;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = (unsigned)h->P.S;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
+    if (G_act > 1) {
+        // helper clusters spin on their leader: ask the driver to guarantee co-residency of the
+        // whole grid (the launch fails instead of dead-locking when the device is shared)
+        attr[1].id = cudaLaunchAttributeCooperative;
+        attr[1].val.cooperative = 1;
+        cfg.numAttrs = 2;
+    }
     if (a.mode == QMCD_MODE_SWEEP && a.blocked && h->P.m_in_smem) CK(h, cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep, a));
     else CK(h, cudaLaunchKernelEx(&cfg, qmcd_kernel, a));
     return QMCD_OK;
