@@ -341,10 +341,13 @@ def run_ours(args):
     ach = work["flops"] / (sweep_ms * 1e-3) / 1e12
     traffic = None
     try:    # dram__bytes_read.sum + dram__bytes_write.sum of this kernel from the committed ncu capture
-        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(f"{args.config}:K{K}:{args.mode}")
-    except (OSError, ValueError):
+        for line in open(os.path.join(ROOT, "profiles", "r1_traffic.csv")).read().splitlines()[1:]:
+            f = line.split(",")
+            if f[0] == f"{args.config}:K{K}:{args.mode}":
+                traffic = int(f[1])
+    except (OSError, ValueError, IndexError):
         pass
-    roofline = {"kernel": "qmcd_kernel (sweep mode: ratio + accept + flush fused, one launch/step)",
+    roofline = {"kernel": "qmcd_kernel_sweep (look-ahead + accept + flush fused, persistent, one launch/step)",
                 "bound": "tensor", "achieved": ach, "peak": dmma, "unit": "TFLOP/s",
                 "frac": ach / dmma, "traffic": traffic,
                 "peak_source": "measured live: register-resident DMMA.8x8x4 fp64 loop (qmcd_probe_fp64); "
