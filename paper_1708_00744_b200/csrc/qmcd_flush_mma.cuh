@@ -1,7 +1,9 @@
-// qmcd_flush_mma.cuh -- FP64 tensor-core (DMMA) flush of Eq. 4:
-//     Y = M W            (m x N,  by column slice, one cluster sync after it)
+// qmcd_flush_mma.cuh -- FP64 tensor-core (DMMA) flush of Eq. 4, per tile of
+// 128 / 64 rows of B (tiles dealt round-robin to the walker's CTAs):
 //     T = B0 C^T - E_J   (row tile x m, reduction over N)          "NT stage"
-//     B <- B0 - T Y      (row tile x N, reduction over m)          "NN stage"
+//     K <= 64:  T <- T M (warp-local)                              "TM stage"
+//               B <- B0 - T W                                      "NN stage"
+//     K >  64:  Y = M W first (m x N, by column slice, one cluster barrier), B <- B0 - T Y
 // sm_100a has no tcgen05 f64 kind; its FP64 tensor instruction is DMMA.8x8x4
 // (mma.sync.m8n8k4.f64), measured at 37 TFLOP/s against 34 for DFMA.  Operand
 // fragments are loaded as 16-byte vectors by permuting the contraction index

@@ -1,5 +1,6 @@
-// qmcd_kernel.cuh -- the one __global__ entry: a cluster per walker runs either
-// one phase (per-call API) or the whole move loop (qmcd_sweep, persistent).
+// qmcd_kernel.cuh -- the two __global__ entries over one body: clusters of S CTAs, G clusters
+// per walker.  qmcd_kernel runs one phase (per-call API) or the per-move sweep, qmcd_kernel_sweep
+// the blocked sweep (persistent: the whole move loop); helper clusters serve the flushes.
 #pragma once
 #include "qmcd_phases.cuh"
 #include "qmcd_flush_mma.cuh"
