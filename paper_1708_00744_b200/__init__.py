@@ -9,4 +9,4 @@ for NVIDIA B200 (sm_100a).
 
 There is no CPU fallback: using ``binding`` without the built CUDA library raises.
 """
-__all__ = ["inputs", "binding", "buildlib", "dist"]
+__all__ = ["inputs", "binding", "buildlib", "dist", "autotune"]

@@ -548,3 +548,13 @@ def test_helper_clusters_with_metropolis_and_single_moves(qmcd):
     assert _rel(R.cpu().numpy(), Ro) <= RTOL_RATIO
     assert np.max(np.abs(B.cpu().numpy() - Bo)) <= 1e-10
     q.close()
+
+
+def test_autotune_K_picks_a_tensor_bound_delay(qmcd):
+    """the autotuner times the real sweep per candidate K.  On a c2-shaped problem
+    the classic K = 1 path must lose by a wide margin and the winner must be a delay >= 16."""
+    from paper_1708_00744_b200 import autotune
+    r = autotune.autotune_K(1024, 16, Ks=(1, 16, 32, 64), n_moves=256, reps=1)
+    assert set(r["moves_per_s"]) == {1, 16, 32, 64}
+    assert r["best_K"] in (16, 32, 64)
+    assert r["moves_per_s"][r["best_K"]] > 5 * r["moves_per_s"][1]
