@@ -46,11 +46,25 @@ def parse_args():
     ap.add_argument("--cluster", type=int, default=0, help="CTAs per walker (0 = library default)")
     ap.add_argument("--flush-path", type=int, default=0, help="0 auto, 1 CUDA-core, 2 DMMA")
     ap.add_argument("--opt", action="append", default=[], help="library option key=value (qmcd_set_option)")
+    ap.add_argument("--N", type=int, default=0, help="with --config custom: matrix order")
+    ap.add_argument("--batch", type=int, default=1, help="with --config custom: walkers")
+    ap.add_argument("--sweeps", type=int, default=1, help="with --config custom: sweeps over the electrons")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--phases", action="store_true",
                     help="also time the ratio and flush kernels in isolation (per-call API)")
     return ap.parse_args()
+
+
+def get_config(args):
+    """BASELINE.json config c0..c4, or a custom shape (the paper's own grid, PAPER.md:103-113:
+    one walker, N = 256 ... 8192, 100 % acceptance = --mode bern1.0)."""
+    from paper_1708_00744_b200 import inputs
+    if args.config == "custom":
+        if args.N < 1:
+            raise SystemExit("--config custom needs --N")
+        return dict(batch=args.batch, N=args.N, sweeps=args.sweeps, Ks=(args.K,), modes=(args.mode,), seed=1)
+    return inputs.CONFIGS[args.config]
 
 
 def mode_inputs(wl, mode):
@@ -172,8 +186,8 @@ def run_reference(args):
         return
     import oracle
     from paper_1708_00744_b200 import inputs
-    cfg = inputs.CONFIGS[args.config]
-    wl = inputs.make_config(args.config)
+    cfg = get_config(args)
+    wl = inputs.make_workload(cfg["batch"], cfg["N"], cfg["sweeps"] * cfg["N"], seed=cfg["seed"])
     mask, uniforms = mode_inputs(wl, args.mode)
     for _ in range(min(args.warmup, 1)):
         oracle_step(oracle, wl, args.K, mask, uniforms)
@@ -218,7 +232,7 @@ def run_ours(args):
         dist.barrier()
     binding.load()
 
-    cfg = inputs.CONFIGS[args.config]
+    cfg = get_config(args)
     wl = inputs.make_workload(cfg["batch"], cfg["N"], cfg["sweeps"] * cfg["N"],
                               seed=qdist.rank_seed(cfg["seed"], rank, cfg["batch"]))     # per-rank walkers
     N, K, batch, n_moves = wl.N, args.K, wl.batch, wl.n_moves
