@@ -121,7 +121,9 @@ int qmcd_counters(qmcd_handle h, long long* counters_dev);
  * equal the call-by-call sequence -- bit for bit with option "lookahead" = 1,
  * to rounding (another summation order, and an already-queued electron is
  * flushed before its block instead of at its accept) with the default blocked
- * look-ahead, which needs proposals_dev 16-byte aligned).  Move t proposes electron
+ * look-ahead, which needs proposals_dev 16-byte aligned; the blocked sweep also
+ * flushes a walker's queue up to min(8, K/4) - 1 moves before it is full when the
+ * next block would not fit -- neutral).  Move t proposes electron
  * (j_begin + t) mod N with new column proposals_dev[t][b][:].  Exactly one of
  * mask_dev ([n_moves][batch] uint8) / uniforms_dev ([n_moves][batch] fp64,
  * Metropolis u < min(1,R^2)) is non-NULL.  Outputs R_out_dev [n_moves][batch]

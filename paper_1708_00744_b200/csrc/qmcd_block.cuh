@@ -412,7 +412,9 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
         t += L;
         __syncthreads();
         QMCD_TICK(cy_app);
-        if (m == K) { qmcd_flush_phase<true>(P, s, cl, w, m); m = 0; QMCD_TICK(cy_fl); }
+        // flush when the queue is full -- or nearly full: a few moves early is neutral
+        // and avoids a tail of 4-, 2-, 1-move blocks (several blocks per window at 50 % acceptance)
+        if (K - m < max(1, min(QMCD_TB / 2, K / 4))) { qmcd_flush_phase<true>(P, s, cl, w, m); m = 0; QMCD_TICK(cy_fl); }
     }
     if (prof) {
         long long* pc = P.counters + (size_t)w.b * 8;
