@@ -88,6 +88,10 @@ def _load():
                           ctypes.c_int, _dp, _dp, _up, _dp, ctypes.c_int, ctypes.c_int,
                           _dp, _up, _ip]
     L.orc_run.restype = ctypes.c_int
+    L.orc_run_lockstep.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                   _dp, _dp, _dp, _up, _dp, ctypes.c_int, ctypes.c_int,
+                                   _dp, _up, ctypes.POINTER(ctypes.c_long), _ip]
+    L.orc_run_lockstep.restype = ctypes.c_int
     L.orc_residual.argtypes = [ctypes.c_int, _dp, _dp]
     L.orc_residual.restype = ctypes.c_double
     L.orc_max_threads.argtypes = []
@@ -268,6 +272,43 @@ def run(path, B, K, proposals, j_begin=0, mask=None, uniforms=None, final_flush=
                          ctypes.byref(thr))
     _chk(rc, "run")
     return R, acc, thr.value
+
+
+def run_lockstep(A, B, K, proposals, j_begin=0, mask=None, uniforms=None, final_flush=True):
+    """Path 3, the lock-step variant: every proposal takes a queue slot
+    (a rejected one with the unchanged column of A), Eq. 4 every K proposals.
+
+    A, B       [batch][N][N] float64, C-contiguous, both updated IN PLACE
+    other arguments as in run().  Returns (R, acc, flushes [batch], threads_used).
+    """
+    for X in (A, B):
+        if not (isinstance(X, np.ndarray) and X.dtype == np.float64 and X.flags.c_contiguous and X.ndim == 3):
+            raise ValueError("A and B must be C-contiguous float64 [batch][N][N] ndarrays")
+    if A.shape != B.shape:
+        raise ValueError("A and B differ in shape")
+    batch, n, _ = B.shape
+    proposals = _f64(proposals)
+    n_moves = proposals.shape[0]
+    if proposals.shape != (n_moves, batch, n):
+        raise ValueError("proposals must be [n_moves][batch][N]")
+    if (mask is None) == (uniforms is None):
+        raise ValueError("exactly one of mask / uniforms")
+    R = np.zeros((n_moves, batch), dtype=np.float64)
+    acc = np.zeros((n_moves, batch), dtype=np.uint8)
+    fl = (ctypes.c_long * batch)()
+    thr = ctypes.c_int()
+    if mask is not None:
+        mask = np.ascontiguousarray(mask, dtype=np.uint8)
+        assert mask.shape == (n_moves, batch)
+        mp, up, mode = mask.ctypes.data_as(_up), None, 0
+    else:
+        uniforms = _f64(uniforms, (n_moves, batch))
+        mp, up, mode = None, _p(uniforms), 1
+    rc = _load().orc_run_lockstep(batch, n, int(K), n_moves, int(j_begin), _p(A), _p(B), _p(proposals),
+                                  mp, up, mode, int(bool(final_flush)), _p(R), acc.ctypes.data_as(_up),
+                                  fl, ctypes.byref(thr))
+    _chk(rc, "run_lockstep")
+    return R, acc, np.array(list(fl), dtype=np.int64), thr.value
 
 
 def max_threads() -> int:

@@ -24,7 +24,8 @@
  *          and the rows J of the STALE inverse B0 (one per row of W)
  *   S      = I_m + V'A^-1 U of Eq. 3 = W C^T  (derived below)
  *
- * Three independent paths:
+ * Three independent paths (plus path 3, the lock-step variant of PAPER.md:97-99,
+ * which is path 2 with every proposal occupying a queue slot):
  *   path 0  the plain definition: explicit LU determinants / inverse
  *           (PAPER.md:55,57 -- "p ~ det(A_new)/det(A)").
  *   path 1  classic rank-1 Sherman-Morrison, Eqs. 1-2.
@@ -32,7 +33,7 @@
  *           (PAPER.md:78-93).
  * The method is exact, so path 0 is the definition of truth and
  * paths 1-2 must agree with it to rounding.  Pins: tests/test_oracle_pins.py.
- * Parity unpinned: nothing (every function below has a pin there).
+ * Parity unpinned: nothing (every function below has a pin there; path 3: P11).
  *
  * No blocking, fusion or reordering beyond what the formulas state; the only
  * parallelism is an OpenMP "parallel for" over independent walkers in the
@@ -484,6 +485,86 @@ int orc_run(int path, int batch, int n, int K, int n_moves, int j_begin,
             if (rc == ORC_OK && final_flush) rc = orc_delayed_flush(h);
             orc_delayed_destroy(h);
         }
+        if (rc != ORC_OK) {
+#pragma omp critical
+            { if (err == ORC_OK) err = rc; }
+        }
+    }
+    return err;
+}
+
+/* ------------------------------------------------------------------ */
+/* Path 3: the lock-step variant of PAPER.md:97-99.  */
+/* "Rejected moves can be treated similarly to an accepted move, only  */
+/* substituting the unchanged matrix columns": EVERY     */
+/* proposal occupies a slot of the queue.  An accepted proposal queues */
+/* its new column v; a rejected one queues the column the electron     */
+/* already has, A_cur[:,j] (a zero column of the paper's U, so it      */
+/* changes neither the determinant nor the inverse).  The queue is     */
+/* therefore full after exactly K proposals for every walker, and all  */
+/* walkers apply Eq. 4 at the same time ("the number of   */
+/* operations is fixed").  Written literally: it needs the current     */
+/* Slater matrix A (row-major, [batch][n][n], updated in place with    */
+/* the accepted columns) to know the unchanged column.                 */
+/* mode / mask / uniforms / outputs / final_flush as in orc_run.       */
+/* ------------------------------------------------------------------ */
+int orc_run_lockstep(int batch, int n, int K, int n_moves, int j_begin,
+                     double *A, double *B, const double *proposals,
+                     const unsigned char *mask, const double *uniforms, int mode,
+                     int final_flush, double *R_out, unsigned char *acc_out,
+                     long *flushes_out, int *threads_used)
+{
+    if (batch < 1 || n < 1 || n_moves < 0 || !A || !B) return ORC_EINVAL;
+    if (mode == 0 && !mask) return ORC_EINVAL;
+    if (mode == 1 && !uniforms) return ORC_EINVAL;
+    int err = ORC_OK;
+    int nthreads = 1;
+#ifdef _OPENMP
+    nthreads = omp_get_max_threads();
+    if (nthreads > batch) nthreads = batch;
+#endif
+    if (threads_used) *threads_used = nthreads;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads)
+    for (int b = 0; b < batch; ++b) {
+        double *Ab = A + (size_t)b * n * n;
+        double *Bb = B + (size_t)b * n * n;
+        double *col = (double *)malloc((size_t)n * sizeof(double));
+        orc_delayed *h = orc_delayed_create(n, K, Bb);
+        int rc = (h && col) ? ORC_OK : ORC_EINVAL;
+        for (int t = 0; t < n_moves && rc == ORC_OK; ++t) {
+            int j = (j_begin + t) % n;
+            const double *v = proposals + ((size_t)t * batch + b) * n;
+            double R;
+            rc = orc_delayed_ratio(h, j, v, &R);
+            if (rc != ORC_OK) break;
+            int acc;
+            if (mode == 0) {
+                acc = mask[(size_t)t * batch + b] != 0;
+            } else {
+                double pacc = R * R;
+                if (pacc > 1.0) pacc = 1.0;
+                acc = uniforms[(size_t)t * batch + b] < pacc;
+            }
+            R_out[(size_t)t * batch + b] = R;
+            acc_out[(size_t)t * batch + b] = (unsigned char)acc;
+            if (acc) {
+                for (int i = 0; i < n; ++i) Ab[(size_t)i * n + j] = v[i];
+            } else {
+                /* the slot takes the unchanged column */
+                double R1;
+                for (int i = 0; i < n; ++i) col[i] = Ab[(size_t)i * n + j];
+                rc = orc_delayed_ratio(h, j, col, &R1);
+                if (rc != ORC_OK) break;
+            }
+            rc = orc_delayed_accept(h);      /* flushes when all K slots are taken */
+            if (rc > 0) rc = ORC_OK;
+        }
+        if (h) {
+            if (rc == ORC_OK && final_flush) rc = orc_delayed_flush(h);
+            if (flushes_out) flushes_out[b] = orc_delayed_flush_count(h);
+            orc_delayed_destroy(h);
+        }
+        free(col);
         if (rc != ORC_OK) {
 #pragma omp critical
             { if (err == ORC_OK) err = rc; }

@@ -293,6 +293,47 @@ def test_P6_flush_neutrality_and_no_final_flush():
     assert np.array_equal(B3, wl.Ainv)                     # K > moves and no flush: untouched
 
 
+# ------------------------------------------------------------------ P11: lock-step variant (path 3)
+@pytest.mark.parametrize("p", [0.99, 0.5, 0.0])
+def test_P11_lockstep_equals_rank1_and_fresh_inverse(p):
+    """a rejected move takes a slot with the unchanged column; the result is
+    still that of the classical method, the tracked A is the walked matrix, and
+    every walker applies Eq. 4 exactly once per K proposals."""
+    wl = inputs.make_workload(batch=3, N=40, n_moves=100, seed=11)
+    mask = wl.bernoulli_mask(p)
+    B1 = wl.Ainv.copy()
+    R1, acc1, _ = oracle.run(1, B1, 1, wl.proposals, mask=mask)
+    for K in (1, 3, 16, 40):
+        A3, B3 = wl.A.copy(), wl.Ainv.copy()
+        R3, acc3, fl, _ = oracle.run_lockstep(A3, B3, K, wl.proposals, mask=mask)
+        assert np.array_equal(acc1, acc3)
+        assert np.abs(R3 / R1 - 1).max() < 1e-11
+        assert np.abs(B3 - B1).max() < 1e-11
+        # K | 100 -> the final flush finds an empty queue; else one more partial flush
+        assert np.all(fl == -(-100 // K))
+        for w in range(wl.batch):
+            Af = _walk(wl.A[w], wl.proposals[:, w], acc1[:, w], wl.n_moves)
+            assert np.array_equal(A3[w], Af)
+            assert np.abs(B3[w] - np.linalg.inv(Af)).max() < 1e-11
+    if p == 0.0:                                           # nothing accepted: nothing moves
+        assert np.abs(B3 - wl.Ainv).max() < 1e-12
+
+
+def test_P11_lockstep_metropolis_and_window_boundaries():
+    """Without a final flush the inverse is stale exactly by the last n_moves mod K proposals."""
+    wl = inputs.make_workload(batch=2, N=24, n_moves=50, seed=12)
+    u = wl.uniforms
+    B1 = wl.Ainv.copy()
+    R1, acc1, _ = oracle.run(1, B1, 1, wl.proposals, uniforms=u)
+    A3, B3 = wl.A.copy(), wl.Ainv.copy()
+    R3, acc3, fl, _ = oracle.run_lockstep(A3, B3, 8, wl.proposals, uniforms=u, final_flush=False)
+    assert np.array_equal(acc1, acc3) and np.abs(R3 / R1 - 1).max() < 1e-11
+    assert np.all(fl == 50 // 8)
+    for w in range(wl.batch):
+        A48 = _walk(wl.A[w], wl.proposals[:48, w], acc1[:48, w], 48)
+        assert np.abs(B3[w] - np.linalg.inv(A48)).max() < 1e-11
+
+
 # ------------------------------------------------------------------ P10: repeated electron (G7)
 def test_P10_same_electron_twice_in_one_window():
     rng = np.random.default_rng(77)
