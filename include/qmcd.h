@@ -94,7 +94,8 @@ int qmcd_accept(qmcd_handle h, const unsigned char* mask_dev);
 int qmcd_accept_metropolis(qmcd_handle h, const double* uniforms_dev,
                            unsigned char* acc_out_dev);
 
-/* Drop the staged proposal for every walker (== accept with an all-zero mask). */
+/* Drop the staged proposal for every walker (== accept with an all-zero mask).
+ * Under option "lockstep" the proposal still counts towards the window of K. */
 int qmcd_reject(qmcd_handle h);
 
 /* Apply the queue of every walker with m > 0 (Eq. 4):
@@ -113,7 +114,8 @@ int qmcd_status(qmcd_handle h, int* host_out, int* info_out);
 /* Per-walker counters since set_inverse, copied (enqueued) to
  * counters_dev: [batch][8] int64 = {accepted moves, flushes, then SM clock cycles
  * of the walker's leader CTA inside qmcd_sweep: look-ahead products (F1), per-move
- * chain (F1 small part + F2), queue append, flush (F3), whole sweep, reserved}. */
+ * chain (F1 small part + F2), queue append, flush (F3), whole sweep, proposals in
+ * the current window (option "lockstep", else 0)}. */
 int qmcd_counters(qmcd_handle h, long long* counters_dev);
 
 /* Device-resident run of n_moves proposals with no host round trip (the same
@@ -153,7 +155,13 @@ size_t qmcd_sweep_host_min_staging(int N, int batch);
  * on the device at once, else QMCD_EINVAL), "flush_path"
  * (0 auto, 1 CUDA-core, 2 DMMA), "lookahead" (qmcd_sweep: 0 auto = blocked
  * look-ahead when the shape allows, 1 = per move, the arithmetic of the per-call
- * API).  get: those plus "threads", "smem_bytes", "m_in_smem", "blocked_ok",
+ * API), "lockstep" (0/1, IDLE only: the lock-step variant of PAPER.md:97-99 --
+ * every proposal, accepted or not, takes one of the K slots of the window (a rejected
+ * one stands for the unchanged column, a zero column of U in Eq. 4, so it adds no
+ * arithmetic), and Eq. 4 is applied after every K-th PROPOSAL with rank m = the
+ * moves accepted in the window, 0 <= m <= K: all walkers flush in the same move.
+ * Holds for qmcd_accept* / qmcd_reject and both sweeps; qmcd_flush and
+ * qmcd_set_inverse open a new window).  get: those plus "threads", "smem_bytes", "m_in_smem", "blocked_ok",
  * "max_active_clusters".
  * get returns the value (>= 0) or a negative error. */
 int qmcd_set_option(qmcd_handle h, const char* key, int value);

@@ -305,6 +305,13 @@ extern "C" int qmcd_accept_metropolis(qmcd_handle h, const double* uniforms_dev,
 extern "C" int qmcd_reject(qmcd_handle h) {
     if (!h) return QMCD_EINVAL;
     if (h->state != QMCD_PROPOSED) return QMCD_ESTATE;
+    if (h->P.lockstep) {                       // the rejected proposal still takes a slot of the window
+        QmcdArgs a = base_args(h, QMCD_MODE_ACCEPT);
+        a.reject_all = 1;
+        int rc = launch(h, a, false);
+        if (rc == QMCD_OK) h->state = QMCD_IDLE;
+        return rc;
+    }
     CK(h, cudaMemsetAsync(h->P.sj, 0xff, (size_t)h->batch * 4, h->stream));
     h->state = QMCD_IDLE;
     return QMCD_OK;
@@ -429,6 +436,12 @@ extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
         h->lookahead = value;
         return QMCD_OK;
     }
+    if (!strcmp(key, "lockstep")) {                // legal between windows only (IDLE); starts a fresh window count
+        if (value < 0 || value > 1) return QMCD_EINVAL;
+        if (h->state != QMCD_IDLE) return QMCD_ESTATE;
+        h->P.lockstep = value;
+        return QMCD_OK;
+    }
     if (!strcmp(key, "chain_regs")) {
         if (value < 0 || value > 1) return QMCD_EINVAL;
         h->P.chain_regs = value;
@@ -443,6 +456,7 @@ extern "C" int qmcd_get_option(qmcd_handle h, const char* key) {
     if (!strcmp(key, "clusters_per_walker")) return h->P.G;
     if (!strcmp(key, "flush_path")) return h->P.flush_path;
     if (!strcmp(key, "lookahead")) return h->lookahead;
+    if (!strcmp(key, "lockstep")) return h->P.lockstep;
     if (!strcmp(key, "blocked_ok")) return h->P.blk_ok && h->P.m_in_smem;
     if (!strcmp(key, "m_in_smem")) return h->P.m_in_smem;
     if (!strcmp(key, "threads")) return QMCD_THREADS;

@@ -37,13 +37,14 @@ struct QmcdDev {
     double* sp;               // [batch][K]     staged p (delta term applied)
     double* sc;               // [batch][K]     staged c = M q
     double* sr;               // [batch][K]     staged r = M^T p
-    long long* counters;      // [batch][8]     accepted, flushes, cycles: look-ahead, chain, queue append, flush, total
+    long long* counters;      // [batch][8]     accepted, flushes, cycles: look-ahead, chain, queue append, flush, total; [7] = proposals since the last flush (lock-step)
     int* status;              // [4]            sticky: code, walker, move counter
     int flush_path;           // 0 auto, 1 CUDA-core, 2 DMMA
     int mma_smem_ok;          // host: the DMMA flush's shared memory fits
     int m_in_smem;            // host: every CTA keeps its own copy of M in shared memory
     int chain_regs;           // option: blocked look-ahead keeps M in registers when K <= 32
     int blk_ok;               // host: qmcd_sweep may use the blocked look-ahead (qmcd_block.cuh)
+    int lockstep;             // option: lock-step variant: Eq. 4 every K PROPOSALS; counters[7] = proposals in the window
 };
 
 enum QmcdMode { QMCD_MODE_RATIO = 0, QMCD_MODE_ACCEPT = 1, QMCD_MODE_FLUSH = 2, QMCD_MODE_SWEEP = 3 };
@@ -61,6 +62,7 @@ struct QmcdArgs {
     const double* uniforms;       // [batch] or nullptr (Metropolis)
     unsigned char* acc_out;       // [batch] or nullptr
     int accept_all;
+    int reject_all;               // qmcd_reject under "lockstep": the proposal still takes a slot
     // SWEEP: v/mask/uniforms/R_out/acc_out are [n_moves][batch]...
     int j_begin, n_moves;
     int blocked;                  // SWEEP: use the blocked look-ahead

@@ -35,6 +35,7 @@ __device__ void qmcd_flush_phase(const QmcdDev& P, const QmcdSmem& s, cg::cluste
     if (w.r == 0 && threadIdx.x == 0) {
         P.m[w.b] = 0;
         P.counters[(size_t)w.b * 8 + 1] += 1;
+        P.counters[(size_t)w.b * 8 + 7] = 0;          // a new window starts (lock-step proposal count)
         const unsigned long long want = ((unsigned long long)P.launch_id << 32) | (unsigned)k;
         for (int g = 1; g < P.G_act; ++g)
             while (qmcd_ld_acquire(P.done + (size_t)w.b * 16 + g) != want) __nanosleep(20);
@@ -119,10 +120,13 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
         const int j = __ldcg(P.sj + b);
         if (j < 0) return;
         const double R = __ldcg(P.sR + b);
+        // lock-step: this proposal takes a slot of the window whatever the decision
+        int pw = P.lockstep ? (int)__ldcg(P.counters + (size_t)b * 8 + 7) + 1 : 0;
         // every CTA has read the staged proposal before the leader clears it
         if (S > 1) cl.sync();
         bool acc;
-        if (A.uniforms) { double pa = fmin(1.0, R * R); acc = A.uniforms[b] < pa; }
+        if (A.reject_all) acc = false;
+        else if (A.uniforms) { double pa = fmin(1.0, R * R); acc = A.uniforms[b] < pa; }
         else acc = A.accept_all || (A.mask[b] != 0);
         if (acc && (R == 0.0 || !isfinite(R))) {
             if (r == 0 && tid == 0) qmcd_set_status(P, QMCD_DEV_ESINGULAR, b, P.counters[(size_t)b * 8]);
@@ -132,7 +136,16 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
             if (A.acc_out) A.acc_out[b] = acc ? 1 : 0;
             P.sj[b] = -1;
         }
-        if (!acc) return;
+        if (!acc) {
+            if (P.lockstep) {
+                if (pw >= P.K) {                       // the window is full: Eq. 4 for whatever was accepted in it
+                    if (m > 0) qmcd_flush_phase<false>(P, s, cl, w, m);   // M is in global memory between launches
+                    pw = 0;
+                }
+                if (r == 0 && tid == 0) P.counters[(size_t)b * 8 + 7] = pw;
+            }
+            return;
+        }
         qmcd_load_state<MS>(P, s, w, m);
         bool inq = false;
         for (int i = tid; i < m; i += QMCD_THREADS) {
@@ -141,13 +154,21 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
         for (int i = 0; i < m; ++i) inq |= (s.Js[i] == j);
         __syncthreads();
         m = qmcd_do_accept<MS>(P, s, cl, w, j, m, R, inq, pbuf);
+        if (P.lockstep) {
+            if (inq) pw = 1;                           // G7 flushed first: this move opens the new window
+            if (pw >= P.K) {
+                if (m > 0) { qmcd_flush_phase<MS>(P, s, cl, w, m); m = 0; }
+                pw = 0;
+            }
+        }
         qmcd_writeback_M<MS>(P, s, w, m);
-        if (r == 0 && tid == 0) P.m[b] = m;
+        if (r == 0 && tid == 0) { P.m[b] = m; if (P.lockstep) P.counters[(size_t)b * 8 + 7] = pw; }
         return;
     }
 
     if (A.mode == QMCD_MODE_FLUSH) {
         if (m > 0) qmcd_flush_phase<false>(P, s, cl, w, m);   // M is in global memory between launches
+        else if (r == 0 && tid == 0) P.counters[(size_t)b * 8 + 7] = 0;
         return;
     }
 
@@ -162,6 +183,7 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
     }
     const int len = w.khi - w.klo;
     const bool prof = (r == 0 && tid == 0);
+    int pw = P.lockstep ? (int)__ldcg(P.counters + (size_t)b * 8 + 7) : 0;   // proposals in the window (lock-step)
     long long cy_la = 0, cy_acc = 0, c0 = prof ? clock64() : 0, c_start = c0;
     for (int t = 0; t < A.n_moves; ++t) {
         const int j = (A.j_begin + t) % P.N;
@@ -191,8 +213,18 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
             if (A.acc_out) A.acc_out[tb] = acc ? 1 : 0;
         }
         if (acc) m = qmcd_do_accept<MS>(P, s, cl, w, j, m, R, inq, pbuf);
+        if (P.lockstep) {
+            // every proposal takes a slot (a rejected one adds a zero column of U,
+            // i.e. nothing), so the window closes after K proposals for every walker at once
+            pw = (acc && inq) ? 1 : pw + 1;
+            if (pw >= P.K) {
+                if (m > 0) { qmcd_flush_phase<MS>(P, s, cl, w, m); m = 0; }
+                pw = 0;
+            }
+        }
         if (prof) { const long long c1 = clock64(); cy_acc += c1 - c0; c0 = c1; }   // accept + flush (per-move path)
     }
+    if (P.lockstep && r == 0 && tid == 0) P.counters[(size_t)b * 8 + 7] = pw;
     qmcd_writeback_M<MS>(P, s, w, m);
     if (prof) {
         long long* pc = P.counters + (size_t)b * 8;

@@ -24,23 +24,31 @@ def _rel(a, b):
 
 
 def gpu_sweep(qmcd, wl, K, mask=None, uniforms=None, final_flush=True, cluster=None, j_begin=0,
-              flush_path=None, lookahead=None):
+              flush_path=None, lookahead=None, lockstep=None, G=None, split=None):
     import torch
     q = qmcd.Qmcd(wl.N, K, wl.batch)
+    if lockstep is not None:
+        q.set_option("lockstep", lockstep)
     if cluster is not None:
         q.set_option("cluster", cluster)
     if flush_path is not None:
         q.set_option("flush_path", flush_path)
     if lookahead is not None:
         q.set_option("lookahead", lookahead)
+    if G is not None:
+        q.set_option("clusters_per_walker", G)
     blocked = bool(q.get_option("blocked_ok")) and q.get_option("lookahead") == 0
     B = _dev(wl.Ainv)
     q.set_inverse(B)
     P = _dev(wl.proposals)
     R = torch.zeros((wl.n_moves, wl.batch), dtype=torch.float64, device="cuda")
     acc = torch.zeros((wl.n_moves, wl.batch), dtype=torch.uint8, device="cuda")
-    q.sweep(j_begin, P, mask=None if mask is None else _dev(mask),
-            uniforms=None if uniforms is None else _dev(uniforms), R_out=R, acc_out=acc)
+    Md = None if mask is None else _dev(mask)
+    Ud = None if uniforms is None else _dev(uniforms)
+    cuts = [0] + list(split or []) + [wl.n_moves]
+    for a, b in zip(cuts[:-1], cuts[1:]):          # one launch per piece
+        q.sweep((j_begin + a) % wl.N, P[a:b], mask=None if Md is None else Md[a:b],
+                uniforms=None if Ud is None else Ud[a:b], R_out=R[a:b], acc_out=acc[a:b])
     if final_flush:
         q.flush()
     st, info = q.status()
@@ -598,3 +606,87 @@ def test_randomized_shapes_seeds_modes_and_launch_splits(qmcd):
         assert np.array_equal(acc.cpu().numpy(), acco), ctx
         assert _rel(R.cpu().numpy(), Ro) <= RTOL_RATIO, ctx
         assert np.max(np.abs(B.cpu().numpy() - Bo)) <= 1e-10, ctx
+
+
+# ------------------------------------------------------------------ lock-step variant
+def _windows_with_accepts(acc, K):
+    n = (acc.shape[0] // K) * K
+    return acc[:n].reshape(-1, K, acc.shape[1]).any(axis=1).sum(axis=0)
+
+
+@pytest.mark.parametrize("N,K,batch,cluster,G,p,lookahead,split", [
+    (128, 16, 3, 1, None, 0.5, 0, None),        # blocked look-ahead, one block per window
+    (128, 16, 3, 2, None, 0.5, 1, None),        # per-move look-ahead
+    (256, 40, 2, 4, None, 0.5, 0, [37, 301]),   # windows of 16 + 16 + 8 proposals, launches cut mid-window
+    (512, 32, 3, 4, 2, 0.99, 0, None),          # helper clusters share the flushes
+    (512, 64, 2, 4, None, 0.3, 0, [5]),         # DMMA flush of low, varying rank
+    (96, 7, 2, 1, None, 0.1, 0, None),          # windows with no accepted move at all
+    (64, 1, 2, 1, None, 0.5, 0, None),          # K = 1
+])
+def test_lockstep_sweep_matches_oracle_path3(qmcd, N, K, batch, cluster, G, p, lookahead, split):
+    """Option "lockstep" against the oracle's literal path 3 (a rejected move
+    queues the unchanged column): same ratios, decisions and inverse; every walker flushes in
+    the same move, once per K proposals."""
+    n_moves = 2 * N + 13
+    wl = inputs.make_workload(batch, N, n_moves=n_moves, seed=41)
+    mask = wl.bernoulli_mask(p)
+    Ao, Bo = wl.A.copy(), wl.Ainv.copy()
+    Ro, acco, flo, _ = oracle.run_lockstep(Ao, Bo, K, wl.proposals, mask=mask, final_flush=False)
+    g = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, G=G, lookahead=lookahead, lockstep=1,
+                  split=split, final_flush=False)
+    assert g["status"] == 0
+    if lookahead == 1:
+        assert not g["blocked"]
+    assert np.array_equal(g["acc"], acco)
+    assert _rel(g["R"], Ro) <= RTOL_RATIO
+    assert np.max(np.abs(g["B"] - Bo)) <= 1e-10
+    assert np.all(flo == n_moves // K)
+    assert np.array_equal(g["counters"][:, 1], _windows_with_accepts(mask, K))   # empty windows cost nothing
+    assert np.all(g["counters"][:, 7] == n_moves % K)
+    assert np.array_equal(g["pending"], mask[(n_moves // K) * K:].sum(axis=0))
+    # the other reading (only accepted moves take slots) reaches the same inverse (PAPER.md:95)
+    g2 = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, lookahead=lookahead)
+    g1 = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, G=G, lookahead=lookahead, lockstep=1, split=split)
+    assert np.max(np.abs(g1["B"] - g2["B"])) <= 1e-10
+    check_residuals(wl, acco, g1["B"])
+
+
+def test_lockstep_metropolis_and_per_call_api(qmcd):
+    """Lock-step through ratio / accept / accept_metropolis / reject, and a Metropolis sweep."""
+    import torch
+    N, K, batch, n_moves = 64, 6, 3, 100
+    wl = inputs.make_workload(batch, N, n_moves=n_moves, seed=42)
+    u = wl.uniforms
+    Ao, Bo = wl.A.copy(), wl.Ainv.copy()
+    Ro, acco, flo, _ = oracle.run_lockstep(Ao, Bo, K, wl.proposals, uniforms=u, final_flush=False)
+    g = gpu_sweep(qmcd, wl, K, uniforms=u, lockstep=1, final_flush=False)
+    assert g["status"] == 0 and np.array_equal(g["acc"], acco) and _rel(g["R"], Ro) <= RTOL_RATIO
+    assert np.max(np.abs(g["B"] - Bo)) <= 1e-10
+    # per-call: every third proposal is dropped with qmcd_reject, the others decided by Metropolis
+    u2 = u.copy(); u2[::3] = 2.0                     # u >= 1 > min(1, R^2): rejected
+    Ao, Bo = wl.A.copy(), wl.Ainv.copy()
+    Ro, acco, flo, _ = oracle.run_lockstep(Ao, Bo, K, wl.proposals, uniforms=u2, final_flush=False)
+    q = qmcd.Qmcd(N, K, batch)
+    q.set_option("lockstep", 1)
+    B = _dev(wl.Ainv); q.set_inverse(B)
+    P = _dev(wl.proposals); Ud = _dev(u2)
+    R = torch.zeros((n_moves, batch), dtype=torch.float64, device="cuda")
+    acc = torch.zeros((n_moves, batch), dtype=torch.uint8, device="cuda")
+    for t in range(n_moves):
+        q.ratio(t % N, P[t], R[t])
+        if t % 3 == 0:
+            q.reject()
+        else:
+            q.accept_metropolis(Ud[t], acc[t])
+        if (t + 1) % K == 0:
+            assert np.all(q.pending().cpu().numpy() == 0), t      # the window closed in this move
+    st, _ = q.status()
+    cnt = q.counters().cpu().numpy()
+    assert st == 0
+    assert np.array_equal(acc.cpu().numpy(), acco)
+    assert _rel(R.cpu().numpy(), Ro) <= RTOL_RATIO
+    assert np.max(np.abs(B.cpu().numpy() - Bo)) <= 1e-10
+    assert np.all(cnt[:, 7] == n_moves % K)
+    q.flush()
+    assert np.all(q.counters().cpu().numpy()[:, 7] == 0)
+    q.close()
