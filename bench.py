@@ -141,11 +141,13 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------------------- accounting
-def algorithmic_work(acc, N, K):
+def algorithmic_work(acc, N, K, lockstep=False):
     """Algorithmic flops / bytes of one step from the accept sequence acc [n_moves][batch]
     (SURVEY.md 8(d) / DESIGN.md 'Kernels'): F1 per proposal at queue length m:
     2N(2m+1)+2m^2 flops, 8N(2m+2)+8m^2 bytes; F2 per accept 4m^2 flops; F3 per rank-m
-    flush 4N^2 m + 2 m^2 N flops, 16N^2 + 24mN bytes (final partial flush included)."""
+    flush 4N^2 m + 2 m^2 N flops, 16N^2 + 24mN bytes (final partial flush included).
+    lockstep: the window closes after every K-th PROPOSAL with the rank m
+    accepted in it; a rejected slot is a zero column of U and counts no work."""
     n_moves, batch = acc.shape
     f1f = f1b = f2f = f3f = f3b = 0.0
     flushes = 0
@@ -158,11 +160,11 @@ def algorithmic_work(acc, N, K):
             if a[t]:
                 f2f += 4.0 * m * m
                 m += 1
-                if m == K:
-                    f3f += 4.0 * N * N * m + 2.0 * m * m * N
-                    f3b += 16.0 * N * N + 24.0 * m * N
-                    flushes += 1
-                    m = 0
+            if (m > 0 and (t + 1) % K == 0) if lockstep else (m == K):
+                f3f += 4.0 * N * N * m + 2.0 * m * m * N
+                f3b += 16.0 * N * N + 24.0 * m * N
+                flushes += 1
+                m = 0
         if m > 0:
             f3f += 4.0 * N * N * m + 2.0 * m * m * N
             f3b += 16.0 * N * N + 24.0 * m * N
@@ -343,7 +345,7 @@ def run_ours(args):
         return
 
     # ---- roofline of the dominant kernel (the persistent sweep kernel: F1+F2+F3 fused)
-    work = algorithmic_work(acc_h, N, K)
+    work = algorithmic_work(acc_h, N, K, lockstep=bool(q.get_option("lockstep")))
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -380,6 +382,7 @@ def run_ours(args):
                                                  "lookahead": "blocked" if (q.get_option("blocked_ok") and
                                                                             q.get_option("lookahead") == 0) else "per-move",
                                                  "flush_path": q.get_option("flush_path"),
+                                                 "lockstep": q.get_option("lockstep"),
                                                  "accepted_per_step": accepted_all,
                                                  "flushes_per_step": work["flushes"]}),
            "clocks": clocks, "e2e": e2e, "gpu_launches": LAUNCHES_PER_STEP * args.steps,

@@ -54,3 +54,14 @@ def test_mode_inputs_and_config_names():
     m, u = bench.mode_inputs(wl, "metropolis")
     assert m is None and u is wl.uniforms
     assert set(inputs.CONFIGS) == {"c0", "c1", "c2", "c3", "c4"}
+
+
+def test_lockstep_accounting_flushes_every_K_proposals():
+    """one flush per window of K proposals, rank = accepts in it; none if empty."""
+    N, K = 16, 4
+    acc = np.array([[1, 0, 0, 0,  0, 0, 0, 0,  1, 1, 1, 1,  1, 0]], dtype=np.uint8).T
+    w = bench.algorithmic_work(acc, N, K, lockstep=True)
+    assert w["flushes"] == 3                      # ranks 1, (empty), 4, and the final partial 1
+    assert w["flush_flops"] == sum(4.0 * N * N * m + 2.0 * m * m * N for m in (1, 4, 1))
+    w2 = bench.algorithmic_work(acc, N, K, lockstep=False)
+    assert w2["flushes"] == 2                     # ranks 4 and 2
