@@ -149,6 +149,19 @@ int qmcd_sweep_host(qmcd_handle h, int j_begin, int n_moves,
                     void* staging_dev, size_t staging_bytes);
 size_t qmcd_sweep_host_min_staging(int N, int batch);
 
+/* Batched on-device inversion (the "explicit copy of the matrix inverse" the
+ * method starts from and may refresh): Ainv_dev[b] <- A_dev[b]^-1 for every walker, by
+ * Gauss-Jordan elimination with partial pivoting in one cooperative launch.  A_dev, Ainv_dev:
+ * [batch][N][N] row-major fp64 (A: row = orbital, column = electron; may be the same buffer).
+ * scratch_dev: caller-owned, 256-byte aligned, >= qmcd_invert_scratch_bytes(N, batch) bytes
+ * (0 = N too large for the kernel's shared memory, N <= 11600).  info_dev: [batch] int32, 0 or
+ * k+1 of the first zero / non-finite pivot (that walker's result is then garbage); may be NULL.
+ * Does not adopt the result: call qmcd_set_inverse(Ainv_dev) afterwards.  Enqueued on the
+ * handle's stream.  Errors: QMCD_EINVAL, QMCD_ESTATE (PROPOSED), QMCD_ECUDA. */
+size_t qmcd_invert_scratch_bytes(int N, int batch);
+int qmcd_invert(qmcd_handle h, const double* A_dev, double* Ainv_dev,
+                void* scratch_dev, size_t scratch_bytes, int* info_dev);
+
 /* Tuning / introspection.  set: "cluster" (CTAs per cluster, 1..16; resets
  * "clusters_per_walker" to 1), "clusters_per_walker" (1..16, 1..4 when K > 64: cluster 0 of a walker
  * runs the look-ahead, all of them share the rows of a flush; they must all fit

@@ -31,6 +31,8 @@ SYMBOLS = {
     "qmcd_sweep": (_ci, [_vp, _ci, _ci, _vp, _vp, _vp, _vp, _vp]),
     "qmcd_sweep_host": (_ci, [_vp, _ci, _ci, _vp, _vp, _vp, _vp, _vp, _vp, _sz]),
     "qmcd_sweep_host_min_staging": (_sz, [_ci, _ci]),
+    "qmcd_invert_scratch_bytes": (_sz, [_ci, _ci]),
+    "qmcd_invert": (_ci, [_vp, _vp, _vp, _vp, _sz, _vp]),
     "qmcd_set_option": (_ci, [_vp, ctypes.c_char_p, _ci]),
     "qmcd_get_option": (_ci, [_vp, ctypes.c_char_p]),
     "qmcd_probe_fp64": (_ci, [_ci, _ci, _vp, ctypes.POINTER(ctypes.c_double)]),
@@ -207,6 +209,26 @@ class Qmcd:
                                      _ptr(uniforms, torch.float64, "cpu"), _ptr(R_out, torch.float64, "cpu"),
                                      _ptr(acc_out, torch.uint8, "cpu"),
                                      staging.data_ptr() + off, staging.numel() - off), "qmcd_sweep_host")
+
+    def invert(self, A, Ainv=None, info=None):
+        """Ainv[b] <- A[b]^-1 on the device (qmcd_invert); returns (Ainv, info [batch] int32).
+        Does not adopt the result: call set_inverse(Ainv)."""
+        import torch
+        if tuple(A.shape) != (self.batch, self.N, self.N):
+            raise ValueError("A must be [batch][N][N]")
+        if Ainv is None:
+            Ainv = torch.empty_like(A)
+        if info is None:
+            info = torch.empty(self.batch, dtype=torch.int32, device="cuda")
+        need = self._L.qmcd_invert_scratch_bytes(self.N, self.batch)
+        if need == 0:
+            raise ValueError("qmcd_invert: N too large")
+        scratch = torch.empty(need + 256, dtype=torch.uint8, device="cuda")
+        off = (-scratch.data_ptr()) % 256
+        _chk(self._L.qmcd_invert(self._h, _ptr(A, torch.float64), _ptr(Ainv, torch.float64),
+                                 scratch.data_ptr() + off, need, _ptr(info, torch.int32)), "qmcd_invert")
+        self._keep = scratch          # alive until the next call (the work is only enqueued)
+        return Ainv, info
 
     def set_option(self, key: str, value: int):
         _chk(self._L.qmcd_set_option(self._h, key.encode(), int(value)), f"qmcd_set_option({key})")

@@ -8,6 +8,7 @@
 
 #include "../../include/qmcd.h"
 #include "qmcd_kernel.cuh"
+#include "qmcd_invert.cuh"
 
 enum { QMCD_IDLE = 0, QMCD_PROPOSED = 1 };
 
@@ -360,6 +361,57 @@ extern "C" int qmcd_sweep(qmcd_handle h, int j_begin, int n_moves,
     a.mask = mask_dev; a.uniforms = uniforms_dev; a.R_out = R_out_dev; a.acc_out = acc_out_dev;
     a.blocked = (h->lookahead != 1 && h->P.blk_ok && h->P.m_in_smem && (((uintptr_t)proposals_dev & 15) == 0)) ? 1 : 0;
     return launch(h, a, true);
+}
+
+// ---- batched on-device inversion (qmcd_invert.cuh)
+static size_t inv_smem_bytes(int N) { return (size_t)N * 20; }
+
+extern "C" size_t qmcd_invert_scratch_bytes(int N, int batch) {
+    if (N < 1 || batch < 1 || inv_smem_bytes(N) > 227 * 1024) return 0;
+    return al256((size_t)batch * N * 4) + al256((size_t)batch * QMCD_INV_CMAX * 8) +
+           al256((size_t)batch * QMCD_INV_CMAX * 4) + al256((size_t)batch * 4);
+}
+
+extern "C" int qmcd_invert(qmcd_handle h, const double* A_dev, double* Ainv_dev,
+                           void* scratch_dev, size_t scratch_bytes, int* info_dev) {
+    if (!h || !A_dev || !Ainv_dev || !scratch_dev) return QMCD_EINVAL;
+    const int N = h->N, batch = h->batch;
+    const size_t need = qmcd_invert_scratch_bytes(N, batch);
+    if (need == 0 || scratch_bytes < need || ((uintptr_t)scratch_dev & 255)) return QMCD_EINVAL;
+    if (h->state != QMCD_IDLE) return QMCD_ESTATE;
+    const size_t smem = inv_smem_bytes(N);
+    CK(h, cudaFuncSetAttribute(qmcd_invert_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int dev = 0, sms = 0, per_sm = 0;
+    CK(h, cudaGetDevice(&dev));
+    CK(h, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CK(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, qmcd_invert_kernel, QMCD_INV_THREADS, smem));
+    const int max_blocks = sms * per_sm;
+    if (max_blocks < 1) return QMCD_EINVAL;
+    // C CTAs per walker (row slots interleaved), as many walkers per cooperative launch as fit
+    int C = max_blocks / batch;
+    if (C < 1) C = 1;
+    if (C > QMCD_INV_CMAX) C = QMCD_INV_CMAX;
+    if (C > (N + 7) / 8) C = (N + 7) / 8;          // at least one row per warp
+    const int per_launch = (max_blocks / C < batch) ? max_blocks / C : batch;
+    unsigned char* sc = (unsigned char*)scratch_dev;
+    QmcdInvArgs a;
+    a.N = N; a.C = C;
+    int* piv = (int*)sc; sc += al256((size_t)batch * N * 4);
+    double* cval = (double*)sc; sc += al256((size_t)batch * QMCD_INV_CMAX * 8);
+    int* cidx = (int*)sc; sc += al256((size_t)batch * QMCD_INV_CMAX * 4);
+    int* info = info_dev ? info_dev : (int*)sc;
+    CK(h, cudaMemsetAsync(info, 0, (size_t)batch * 4, h->stream));
+    for (int b0 = 0; b0 < batch; b0 += per_launch) {
+        const int nb = (batch - b0 < per_launch) ? batch - b0 : per_launch;
+        a.batch = nb;
+        a.A = A_dev + (size_t)b0 * N * N; a.X = Ainv_dev + (size_t)b0 * N * N;
+        a.piv = piv + (size_t)b0 * N; a.cand_val = cval + (size_t)b0 * QMCD_INV_CMAX;
+        a.cand_idx = cidx + (size_t)b0 * QMCD_INV_CMAX; a.info = info + b0;
+        void* kargs[] = {(void*)&a};
+        CK(h, cudaLaunchCooperativeKernel((void*)qmcd_invert_kernel, dim3((unsigned)(nb * C)), dim3(QMCD_INV_THREADS),
+                                          kargs, smem, h->stream));
+    }
+    return QMCD_OK;
 }
 
 extern "C" size_t qmcd_sweep_host_min_staging(int N, int batch) {

@@ -32,6 +32,13 @@ def test_header_symbols_all_exported_and_bound(lib):
     assert sorted(binding.SYMBOLS) == names
 
 
+def test_invert_scratch_bytes_validation(lib):
+    assert lib.qmcd_invert_scratch_bytes(512, 16) >= 16 * 512 * 4
+    assert lib.qmcd_invert_scratch_bytes(0, 1) == 0
+    assert lib.qmcd_invert_scratch_bytes(8, 0) == 0
+    assert lib.qmcd_invert_scratch_bytes(20000, 1) == 0     # two rows + the gather no longer fit in shared memory
+
+
 def test_workspace_bytes_validation(lib):
     assert lib.qmcd_workspace_bytes(64, 4, 1) > 2 * 4 * 64 * 8
     assert lib.qmcd_workspace_bytes(0, 1, 1) == 0

@@ -690,3 +690,63 @@ def test_lockstep_metropolis_and_per_call_api(qmcd):
     q.flush()
     assert np.all(q.counters().cpu().numpy()[:, 7] == 0)
     q.close()
+
+
+# ------------------------------------------------------------------ on-device inversion
+@pytest.mark.parametrize("N,batch,seed", [(1, 2, 3), (7, 3, 4), (64, 1, 1), (130, 5, 6), (512, 16, 7), (1024, 3, 8)])
+def test_invert_matches_oracle_lu_inverse(qmcd, N, batch, seed):
+    """qmcd_invert (Gauss-Jordan, partial pivoting) against the oracle's LU inverse and the
+    north_star residual; a leading zero forces a row exchange in walker 0."""
+    import torch
+    wl = inputs.make_workload(batch, N, n_moves=1, seed=seed)
+    A = wl.A.copy()
+    if N > 1:
+        A[0, 0, 0] = 0.0
+    q = qmcd.Qmcd(N, 1, batch)
+    Ad = _dev(A)
+    X, info = q.invert(Ad)
+    torch.cuda.synchronize()
+    assert np.all(info.cpu().numpy() == 0)
+    assert torch.equal(Ad, _dev(A))                       # the input is left alone
+    Xh = X.cpu().numpy()
+    for w in range(min(batch, 4)):
+        Xo = oracle.inverse(A[w])
+        assert np.max(np.abs(Xh[w] - Xo)) <= 1e-10 * max(1.0, np.abs(Xo).max())
+        assert np.max(np.abs(A[w] @ Xh[w] - np.eye(N))) <= TOL_RESID
+    # in place, then adopted: the ratios of a sweep agree with the oracle started from ITS inverse
+    q.invert(Ad, Ainv=Ad)
+    torch.cuda.synchronize()
+    assert np.array_equal(Ad.cpu().numpy(), Xh)
+    q.close()
+
+
+def test_invert_permutation_singular_and_pipeline(qmcd):
+    import torch
+    N, batch, K = 96, 3, 8
+    rng = np.random.default_rng(5)
+    A = np.zeros((batch, N, N))
+    perm = rng.permutation(N)
+    A[0, np.arange(N), perm] = 2.0                         # scaled permutation: every step pivots
+    A[1] = np.eye(N); A[1, 5, 5] = 0.0                     # exactly singular
+    wl = inputs.make_workload(1, N, n_moves=2 * N, seed=9)
+    A[2] = wl.A[0]
+    q = qmcd.Qmcd(N, K, batch)
+    X, info = q.invert(_dev(A))
+    torch.cuda.synchronize()
+    info = info.cpu().numpy(); Xh = X.cpu().numpy()
+    assert info[0] == 0 and info[2] == 0 and info[1] == 6  # first zero pivot at step k = 5
+    assert np.array_equal(Xh[0], A[0].T / 4.0)             # closed form, exact in fp64
+    # walker 2: invert -> set_inverse -> sweep, against the oracle run from its own LU inverse
+    q.close()
+    q = qmcd.Qmcd(N, K, 1)
+    Bd, _ = q.invert(_dev(wl.A))
+    q.set_inverse(Bd)
+    mask = wl.bernoulli_mask(0.7)
+    R = torch.zeros((wl.n_moves, 1), dtype=torch.float64, device="cuda")
+    q.sweep(0, _dev(wl.proposals), mask=_dev(mask), R_out=R)
+    q.flush()
+    Bo = oracle.inverse(wl.A[0])[None].copy()
+    Ro, acco, _ = oracle.run(2, Bo, K, wl.proposals, mask=mask)
+    assert _rel(R.cpu().numpy(), Ro) <= RTOL_RATIO
+    assert np.max(np.abs(Bd.cpu().numpy() - Bo)) <= 1e-10
+    q.close()
