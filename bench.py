@@ -417,6 +417,7 @@ def time_phases(binding, wl, K, reps=5):
     import torch
     N, batch = wl.N, wl.batch
     q = binding.Qmcd(N, K, batch)
+    q.set_option("lookahead", 1)      # the fill below must stop at m = K-1 (the blocked sweep flushes a nearly full queue early)
     B = torch.from_numpy(wl.Ainv).cuda()
     q.set_inverse(B)
     P = torch.from_numpy(wl.proposals[:max(K, 2) + 64]).cuda()
@@ -428,6 +429,7 @@ def time_phases(binding, wl, K, reps=5):
     for rep in range(reps + 1):
         if m > 0:
             q.sweep(0, P[:m], mask=ones[:m])
+            assert int(q.pending().min()) == m, "phase timing needs the queue at m = K-1"
         e0, e1 = ev(), ev()
         n_r = 32
         e0.record()
@@ -443,13 +445,33 @@ def time_phases(binding, wl, K, reps=5):
         if rep > 0:
             ratio_ms.append(e0.elapsed_time(e1) / n_r)
             flush_ms.append(f0.elapsed_time(f1))
+    # set-up step: qmcd_invert of the batch; every one of the N elimination
+    # steps streams each matrix once (read + write): 16 N^3 bytes per walker
+    inv_ms = []
+    if getattr(wl, "A", None) is not None:
+        Ad = torch.from_numpy(wl.A).cuda()
+        Xd = torch.empty_like(Ad)
+        for rep in range(3):
+            i0, i1 = ev(), ev()
+            i0.record()
+            q.invert(Ad, Ainv=Xd)
+            i1.record()
+            torch.cuda.synchronize()
+            if rep > 0:
+                inv_ms.append(i0.elapsed_time(i1))
+        del Ad, Xd
     q.close()
     mm = max(m, 0)
     rb = batch * (8.0 * N * (2 * mm + 2) + 8.0 * mm * mm)
     ff = batch * (4.0 * N * N * mm + 2.0 * mm * mm * N)
     fb = batch * (16.0 * N * N + 24.0 * mm * N)
     r_ms, f_ms = float(np.median(ratio_ms)), float(np.median(flush_ms))
-    return {"ratio": {"m": mm, "ms_per_launch": r_ms, "bytes": rb, "gbs": rb / (r_ms * 1e-3) / 1e9},
+    inv = None
+    if inv_ms:
+        i_ms = float(np.median(inv_ms)); ib = batch * 16.0 * N ** 3
+        inv = {"ms_per_launch": i_ms, "bytes": ib, "gbs": ib / (i_ms * 1e-3) / 1e9,
+               "flops": batch * 2.0 * N ** 3, "walkers_per_s": batch / (i_ms * 1e-3)}
+    return {"invert": inv, "ratio": {"m": mm, "ms_per_launch": r_ms, "bytes": rb, "gbs": rb / (r_ms * 1e-3) / 1e9},
             "flush": {"m": mm, "ms_per_launch": f_ms, "flops": ff, "bytes": fb,
                       "tflops": (ff / (f_ms * 1e-3) / 1e12) if mm else 0.0,
                       "gbs": fb / (f_ms * 1e-3) / 1e9}}
