@@ -391,7 +391,7 @@ extern "C" int qmcd_invert(qmcd_handle h, const double* A_dev, double* Ainv_dev,
     int C = max_blocks / batch;
     if (C < 1) C = 1;
     if (C > QMCD_INV_CMAX) C = QMCD_INV_CMAX;
-    if (C > (N + 7) / 8) C = (N + 7) / 8;          // at least one row per warp
+    { const int nw = QMCD_INV_THREADS / 32; if (C > (N + nw - 1) / nw) C = (N + nw - 1) / nw; }   // at least one row per warp
     const int per_launch = (max_blocks / C < batch) ? max_blocks / C : batch;
     unsigned char* sc = (unsigned char*)scratch_dev;
     QmcdInvArgs a;

@@ -19,8 +19,9 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <cooperative_groups.h>
+#include <stdint.h>
 
-#define QMCD_INV_THREADS 256
+#define QMCD_INV_THREADS 512
 #define QMCD_INV_CMAX 256       // candidate slots per walker in the scratch area
 
 struct QmcdInvArgs {
@@ -51,6 +52,7 @@ __global__ void __launch_bounds__(QMCD_INV_THREADS, 1) qmcd_invert_kernel(const 
     double* cval = a.cand_val + (size_t)b * QMCD_INV_CMAX;
     int* cidx = a.cand_idx + (size_t)b * QMCD_INV_CMAX;
     int* piv = a.piv + (size_t)b * N;
+    const bool vec = ((N & 1) == 0) && ((reinterpret_cast<uintptr_t>(X) & 15) == 0);
 
     // copy my rows, candidates for column 0
     double best = -1.0; int besti = -1;
@@ -106,14 +108,34 @@ __global__ void __launch_bounds__(QMCD_INV_THREADS, 1) qmcd_invert_kernel(const 
             const bool from_k = (i == p);                    // slot p receives old row k (the swap)
             const double f = from_k ? rowk[k] : __ldcg(xi + k);
             double cand = 0.0;
-            for (int q = lane; q < N; q += 32) {
-                const double x = from_k ? rowk[q] : __ldcg(xi + q);
-                const double y = (q == k) ? -f * rowp[q] : x - f * rowp[q];
-                xi[q] = y;
-                if (q == kn) cand = y;
+            int src_lane;
+            if (vec) {                                       // 16-byte accesses, four rows of loads in flight per lane
+                const double2* rp2 = reinterpret_cast<const double2*>(rowp);
+                const double2* rk2 = reinterpret_cast<const double2*>(rowk);
+                double2* x2 = reinterpret_cast<double2*>(xi);
+                const int N2 = N >> 1, k2 = k >> 1, kn2 = kn >> 1;
+#pragma unroll 4
+                for (int q = lane; q < N2; q += 32) {
+                    const double2 x = from_k ? rk2[q] : __ldcg(x2 + q);
+                    const double2 rr = rp2[q];
+                    double2 y;
+                    y.x = x.x - f * rr.x; y.y = x.y - f * rr.y;
+                    if (q == k2) { if (k & 1) y.y = -f * rr.y; else y.x = -f * rr.x; }
+                    x2[q] = y;
+                    if (q == kn2) cand = (kn & 1) ? y.y : y.x;
+                }
+                src_lane = kn2 & 31;
+            } else {
+                for (int q = lane; q < N; q += 32) {
+                    const double x = from_k ? rowk[q] : __ldcg(xi + q);
+                    const double y = (q == k) ? -f * rowp[q] : x - f * rowp[q];
+                    xi[q] = y;
+                    if (q == kn) cand = y;
+                }
+                src_lane = kn & 31;
             }
             if (kn < N && i > k) {
-                cand = fabs(__shfl_sync(0xffffffffu, cand, kn & 31));
+                cand = fabs(__shfl_sync(0xffffffffu, cand, src_lane));
                 if (!(cand <= best)) { best = cand; besti = i; }
             }
         }
