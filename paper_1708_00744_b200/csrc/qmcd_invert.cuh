@@ -34,7 +34,7 @@ struct QmcdInvArgs {
     int* info;                  // [batch] 0, or k+1 of the first zero / non-finite pivot
 };
 
-__global__ void __launch_bounds__(QMCD_INV_THREADS, 1) qmcd_invert_kernel(const QmcdInvArgs a) {
+__global__ void __launch_bounds__(QMCD_INV_THREADS, 2) qmcd_invert_kernel(const QmcdInvArgs a) {
     namespace cg = cooperative_groups;
     extern __shared__ __align__(16) unsigned char inv_smem[];
     cg::grid_group grid = cg::this_grid();
