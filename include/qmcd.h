@@ -154,7 +154,7 @@ size_t qmcd_sweep_host_min_staging(int N, int batch);
  * Gauss-Jordan elimination with partial pivoting in one cooperative launch.  A_dev, Ainv_dev:
  * [batch][N][N] row-major fp64 (A: row = orbital, column = electron; may be the same buffer).
  * scratch_dev: caller-owned, 256-byte aligned, >= qmcd_invert_scratch_bytes(N, batch) bytes
- * (0 = N too large for the kernel's shared memory, N <= 11600).  info_dev: [batch] int32, 0 or
+ * (0 = N too large for the kernel's shared memory, N <= 14528).  info_dev: [batch] int32, 0 or
  * k+1 of the first zero / non-finite pivot (that walker's result is then garbage); may be NULL.
  * Does not adopt the result: call qmcd_set_inverse(Ainv_dev) afterwards.  Enqueued on the
  * handle's stream.  Errors: QMCD_EINVAL, QMCD_ESTATE (PROPOSED), QMCD_ECUDA. */

@@ -99,6 +99,8 @@ static int configure_kernel(qmcd_ctx* h, int S) {
     CK(h, cudaFuncSetAttribute(qmcd_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     CK(h, cudaFuncSetAttribute(qmcd_kernel_sweep, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     CK(h, cudaFuncSetAttribute(qmcd_kernel_sweep, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    CK(h, cudaFuncSetAttribute(qmcd_kernel_sweep_ls, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    CK(h, cudaFuncSetAttribute(qmcd_kernel_sweep_ls, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     h->smem_bytes = smem;
     h->P.S = S;
     return QMCD_OK;
@@ -154,7 +156,10 @@ static int launch(qmcd_ctx* h, QmcdArgs& a, bool with_helpers) {
         attr[1].val.cooperative = 1;
         cfg.numAttrs = 2;
     }
-    if (a.mode == QMCD_MODE_SWEEP && a.blocked && h->P.m_in_smem) CK(h, cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep, a));
+    if (a.mode == QMCD_MODE_SWEEP && a.blocked && h->P.m_in_smem) {
+        if (h->P.lockstep) CK(h, cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep_ls, a));
+        else CK(h, cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep, a));
+    }
     else CK(h, cudaLaunchKernelEx(&cfg, qmcd_kernel, a));
     return QMCD_OK;
 }
@@ -364,7 +369,7 @@ extern "C" int qmcd_sweep(qmcd_handle h, int j_begin, int n_moves,
 }
 
 // ---- batched on-device inversion (qmcd_invert.cuh)
-static size_t inv_smem_bytes(int N) { return (size_t)N * 20; }
+static size_t inv_smem_bytes(int N) { return (size_t)N * 16; }
 
 extern "C" size_t qmcd_invert_scratch_bytes(int N, int batch) {
     if (N < 1 || batch < 1 || inv_smem_bytes(N) > 227 * 1024) return 0;
@@ -381,17 +386,24 @@ extern "C" int qmcd_invert(qmcd_handle h, const double* A_dev, double* Ainv_dev,
     if (h->state != QMCD_IDLE) return QMCD_ESTATE;
     const size_t smem = inv_smem_bytes(N);
     CK(h, cudaFuncSetAttribute(qmcd_invert_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int dev = 0, sms = 0, per_sm = 0;
+    int dev = 0, sms = 0;
     CK(h, cudaGetDevice(&dev));
     CK(h, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    CK(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, qmcd_invert_kernel, QMCD_INV_THREADS, smem));
+    // 256 or 512 threads per CTA: whichever keeps more warps resident on an SM (the loop is
+    // bound by loads in flight); on a tie the smaller CTA (finer balance over the SMs)
+    int threads = 0, per_sm = 0;
+    for (int t = 256; t <= QMCD_INV_THREADS; t *= 2) {
+        int n = 0;
+        CK(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, qmcd_invert_kernel, t, smem));
+        if (n * t > per_sm * threads) { threads = t; per_sm = n; }
+    }
     const int max_blocks = sms * per_sm;
     if (max_blocks < 1) return QMCD_EINVAL;
     // C CTAs per walker (row slots interleaved), as many walkers per cooperative launch as fit
     int C = max_blocks / batch;
     if (C < 1) C = 1;
     if (C > QMCD_INV_CMAX) C = QMCD_INV_CMAX;
-    { const int nw = QMCD_INV_THREADS / 32; if (C > (N + nw - 1) / nw) C = (N + nw - 1) / nw; }   // at least one row per warp
+    { const int nw = threads / 32; if (C > (N + nw - 1) / nw) C = (N + nw - 1) / nw; }   // at least one row per warp
     const int per_launch = (max_blocks / C < batch) ? max_blocks / C : batch;
     unsigned char* sc = (unsigned char*)scratch_dev;
     QmcdInvArgs a;
@@ -408,7 +420,7 @@ extern "C" int qmcd_invert(qmcd_handle h, const double* A_dev, double* Ainv_dev,
         a.piv = piv + (size_t)b0 * N; a.cand_val = cval + (size_t)b0 * QMCD_INV_CMAX;
         a.cand_idx = cidx + (size_t)b0 * QMCD_INV_CMAX; a.info = info + b0;
         void* kargs[] = {(void*)&a};
-        CK(h, cudaLaunchCooperativeKernel((void*)qmcd_invert_kernel, dim3((unsigned)(nb * C)), dim3(QMCD_INV_THREADS),
+        CK(h, cudaLaunchCooperativeKernel((void*)qmcd_invert_kernel, dim3((unsigned)(nb * C)), dim3((unsigned)threads),
                                           kargs, smem, h->stream));
     }
     return QMCD_OK;

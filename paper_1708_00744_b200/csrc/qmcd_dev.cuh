@@ -47,6 +47,13 @@ struct QmcdDev {
     int lockstep;             // option: lock-step variant: Eq. 4 every K PROPOSALS; counters[7] = proposals in the window
 };
 
+// lock-step option as seen by the kernels (QMCD_NO_LOCKSTEP: A/B build without the variant)
+#ifdef QMCD_NO_LOCKSTEP
+#define QMCD_LOCKSTEP(P) 0
+#else
+#define QMCD_LOCKSTEP(P) ((P).lockstep)
+#endif
+
 enum QmcdMode { QMCD_MODE_RATIO = 0, QMCD_MODE_ACCEPT = 1, QMCD_MODE_FLUSH = 2, QMCD_MODE_SWEEP = 3 };
 
 struct QmcdArgs {

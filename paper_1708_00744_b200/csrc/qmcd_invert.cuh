@@ -21,7 +21,7 @@
 #include <cooperative_groups.h>
 #include <stdint.h>
 
-#define QMCD_INV_THREADS 512
+#define QMCD_INV_THREADS 512      // largest CTA; the host launches 256 or 512 threads, whichever puts more warps on an SM
 #define QMCD_INV_CMAX 256       // candidate slots per walker in the scratch area
 
 struct QmcdInvArgs {
@@ -40,10 +40,11 @@ __global__ void __launch_bounds__(QMCD_INV_THREADS, 2) qmcd_invert_kernel(const 
     cg::grid_group grid = cg::this_grid();
     const int N = a.N, C = a.C;
     const int b = blockIdx.x / C, c = blockIdx.x - b * C;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, NW = QMCD_INV_THREADS / 32;
+    const int NT = (int)blockDim.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, NW = NT >> 5;
     double* rowp = reinterpret_cast<double*>(inv_smem);     // [N] new row k (scaled pivot row)
     double* rowk = rowp + N;                                // [N] old row k
-    int* cols = reinterpret_cast<int*>(rowk + N);           // [N] final column gather
+    int* cols = reinterpret_cast<int*>(rowk) + N;           // [N] final column gather (rowk is dead by then: piv | cols)
     __shared__ double s_val[QMCD_INV_THREADS / 32];
     __shared__ int s_idx[QMCD_INV_THREADS / 32];
     __shared__ int s_p;
@@ -84,7 +85,7 @@ __global__ void __launch_bounds__(QMCD_INV_THREADS, 2) qmcd_invert_kernel(const 
         }
         __syncthreads();
         const int p = (s_p >= 0) ? s_p : k;
-        for (int q = tid; q < N; q += QMCD_INV_THREADS) {
+        for (int q = tid; q < N; q += NT) {
             rowp[q] = __ldcg(X + (size_t)p * N + q);
             rowk[q] = __ldcg(X + (size_t)k * N + q);
         }
@@ -94,7 +95,7 @@ __global__ void __launch_bounds__(QMCD_INV_THREADS, 2) qmcd_invert_kernel(const 
         if (bad && c == 0 && tid == 0 && a.info[b] == 0) a.info[b] = k + 1;
         const double d = bad ? 1.0 : 1.0 / pv;
         __syncthreads();
-        for (int q = tid; q < N; q += QMCD_INV_THREADS) rowp[q] = (q == k) ? d : rowp[q] * d;
+        for (int q = tid; q < N; q += NT) rowp[q] = (q == k) ? d : rowp[q] * d;
         grid.sync();                                         // every CTA holds rows p and k: slots may change
         // ---- rewrite my slots; collect candidates for column k+1 on the way
         best = -1.0; besti = -1;
@@ -144,7 +145,7 @@ __global__ void __launch_bounds__(QMCD_INV_THREADS, 2) qmcd_invert_kernel(const 
     grid.sync();
     // ---- undo the row swaps as column swaps, last first, composed into one gather per row
     int* piv_s = reinterpret_cast<int*>(rowk);
-    for (int q = tid; q < N; q += QMCD_INV_THREADS) piv_s[q] = __ldcg(piv + q);
+    for (int q = tid; q < N; q += NT) piv_s[q] = __ldcg(piv + q);
     __syncthreads();
     if (tid == 0) {
         for (int q = 0; q < N; ++q) cols[q] = q;
@@ -156,9 +157,9 @@ __global__ void __launch_bounds__(QMCD_INV_THREADS, 2) qmcd_invert_kernel(const 
     __syncthreads();
     for (int i = c; i < N; i += C) {
         double* xi = X + (size_t)i * N;
-        for (int q = tid; q < N; q += QMCD_INV_THREADS) rowp[q] = __ldcg(xi + q);
+        for (int q = tid; q < N; q += NT) rowp[q] = __ldcg(xi + q);
         __syncthreads();
-        for (int q = tid; q < N; q += QMCD_INV_THREADS) xi[q] = rowp[cols[q]];
+        for (int q = tid; q < N; q += NT) xi[q] = rowp[cols[q]];
         __syncthreads();
     }
 }

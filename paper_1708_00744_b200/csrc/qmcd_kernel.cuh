@@ -121,7 +121,7 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
         if (j < 0) return;
         const double R = __ldcg(P.sR + b);
         // lock-step: this proposal takes a slot of the window whatever the decision
-        int pw = P.lockstep ? (int)__ldcg(P.counters + (size_t)b * 8 + 7) + 1 : 0;
+        int pw = QMCD_LOCKSTEP(P) ? (int)__ldcg(P.counters + (size_t)b * 8 + 7) + 1 : 0;
         // every CTA has read the staged proposal before the leader clears it
         if (S > 1) cl.sync();
         bool acc;
@@ -137,7 +137,7 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
             P.sj[b] = -1;
         }
         if (!acc) {
-            if (P.lockstep) {
+            if (QMCD_LOCKSTEP(P)) {
                 if (pw >= P.K) {                       // the window is full: Eq. 4 for whatever was accepted in it
                     if (m > 0) qmcd_flush_phase<false>(P, s, cl, w, m);   // M is in global memory between launches
                     pw = 0;
@@ -154,7 +154,7 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
         for (int i = 0; i < m; ++i) inq |= (s.Js[i] == j);
         __syncthreads();
         m = qmcd_do_accept<MS>(P, s, cl, w, j, m, R, inq, pbuf);
-        if (P.lockstep) {
+        if (QMCD_LOCKSTEP(P)) {
             if (inq) pw = 1;                           // G7 flushed first: this move opens the new window
             if (pw >= P.K) {
                 if (m > 0) { qmcd_flush_phase<MS>(P, s, cl, w, m); m = 0; }
@@ -162,7 +162,7 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
             }
         }
         qmcd_writeback_M<MS>(P, s, w, m);
-        if (r == 0 && tid == 0) { P.m[b] = m; if (P.lockstep) P.counters[(size_t)b * 8 + 7] = pw; }
+        if (r == 0 && tid == 0) { P.m[b] = m; if (QMCD_LOCKSTEP(P)) P.counters[(size_t)b * 8 + 7] = pw; }
         return;
     }
 
@@ -175,15 +175,11 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
     // ---- QMCD_MODE_SWEEP: the whole move loop, no host round trip, one cluster
     // barrier per move (inside the look-ahead); every CTA decides for itself.
     qmcd_load_state<MS>(P, s, w, m);
-    if (MS && A.blocked) {
-        m = qmcd_sweep_blocked(A, s, cl, w, m);
-        qmcd_writeback_M<MS>(P, s, w, m);
-        if (r == 0 && tid == 0) { P.sj[b] = -1; P.m[b] = m; }
-        return;
-    }
+    // (the blocked look-ahead has its own entries, qmcd_kernel_sweep / qmcd_kernel_sweep_ls: the host
+    // never launches this one with A.blocked set; the per-move loop below is correct for any input)
     const int len = w.khi - w.klo;
     const bool prof = (r == 0 && tid == 0);
-    int pw = P.lockstep ? (int)__ldcg(P.counters + (size_t)b * 8 + 7) : 0;   // proposals in the window (lock-step)
+    int pw = QMCD_LOCKSTEP(P) ? (int)__ldcg(P.counters + (size_t)b * 8 + 7) : 0;   // proposals in the window (lock-step)
     long long cy_la = 0, cy_acc = 0, c0 = prof ? clock64() : 0, c_start = c0;
     for (int t = 0; t < A.n_moves; ++t) {
         const int j = (A.j_begin + t) % P.N;
@@ -213,7 +209,7 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
             if (A.acc_out) A.acc_out[tb] = acc ? 1 : 0;
         }
         if (acc) m = qmcd_do_accept<MS>(P, s, cl, w, j, m, R, inq, pbuf);
-        if (P.lockstep) {
+        if (QMCD_LOCKSTEP(P)) {
             // every proposal takes a slot (a rejected one adds a zero column of U,
             // i.e. nothing), so the window closes after K proposals for every walker at once
             pw = (acc && inq) ? 1 : pw + 1;
@@ -224,7 +220,7 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
         }
         if (prof) { const long long c1 = clock64(); cy_acc += c1 - c0; c0 = c1; }   // accept + flush (per-move path)
     }
-    if (P.lockstep && r == 0 && tid == 0) P.counters[(size_t)b * 8 + 7] = pw;
+    if (QMCD_LOCKSTEP(P) && r == 0 && tid == 0) P.counters[(size_t)b * 8 + 7] = pw;
     qmcd_writeback_M<MS>(P, s, w, m);
     if (prof) {
         long long* pc = P.counters + (size_t)b * 8;
@@ -235,7 +231,7 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
 
 // Common prologue / epilogue of both entry points.  BLOCKED = true: the blocked sweep only (its
 // own register allocation: the per-move look-ahead of the generic entry is not compiled in).
-template <bool BLOCKED>
+template <int BLOCKED>      // 0 generic, 1 blocked sweep, 2 blocked sweep in lock-step
 __device__ __forceinline__ void qmcd_kernel_body(const QmcdArgs& A) {
     extern __shared__ __align__(1024) unsigned char qmcd_smem_raw[];
     const QmcdDev& P = A.P;
@@ -252,7 +248,7 @@ __device__ __forceinline__ void qmcd_kernel_body(const QmcdArgs& A) {
     if (BLOCKED) {
         int m = __ldcg(P.m + b);
         qmcd_load_state<true>(P, s, w, m);
-        m = qmcd_sweep_blocked(A, s, cl, w, m);
+        m = qmcd_sweep_blocked<BLOCKED == 2>(A, s, cl, w, m);
         qmcd_writeback_M<true>(P, s, w, m);
         if (r == 0 && threadIdx.x == 0) { P.sj[b] = -1; P.m[b] = m; }
     } else {
@@ -266,5 +262,6 @@ __device__ __forceinline__ void qmcd_kernel_body(const QmcdArgs& A) {
     }
 }
 
-__global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel(const QmcdArgs A) { qmcd_kernel_body<false>(A); }
-__global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel_sweep(const QmcdArgs A) { qmcd_kernel_body<true>(A); }
+__global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel(const QmcdArgs A) { qmcd_kernel_body<0>(A); }
+__global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel_sweep(const QmcdArgs A) { qmcd_kernel_body<1>(A); }
+__global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel_sweep_ls(const QmcdArgs A) { qmcd_kernel_body<2>(A); }
