@@ -165,7 +165,8 @@ int qmcd_invert(qmcd_handle h, const double* A_dev, double* Ainv_dev,
 /* Tuning / introspection.  set: "cluster" (CTAs per cluster, 1..16; resets
  * "clusters_per_walker" to 1), "clusters_per_walker" (1..16, 1..4 when K > 64: cluster 0 of a walker
  * runs the look-ahead, all of them share the rows of a flush; they must all fit
- * on the device at once, else QMCD_EINVAL), "flush_path"
+ * on the device at once, else QMCD_EINVAL; such launches are cooperative, and when the driver
+ * refuses one at launch time the same step runs with the leader clusters alone), "flush_path"
  * (0 auto, 1 CUDA-core, 2 DMMA), "lookahead" (qmcd_sweep: 0 auto = blocked
  * look-ahead when the shape allows, 1 = per move, the arithmetic of the per-call
  * API), "lockstep" (0/1, IDLE only: the lock-step variant of PAPER.md:97-99 --

@@ -156,11 +156,23 @@ static int launch(qmcd_ctx* h, QmcdArgs& a, bool with_helpers) {
         attr[1].val.cooperative = 1;
         cfg.numAttrs = 2;
     }
-    if (a.mode == QMCD_MODE_SWEEP && a.blocked && h->P.m_in_smem) {
-        if (h->P.lockstep) CK(h, cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep_ls, a));
-        else CK(h, cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep, a));
+    auto fire = [&]() -> cudaError_t {
+        if (a.mode == QMCD_MODE_SWEEP && a.blocked && h->P.m_in_smem)
+            return h->P.lockstep ? cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep_ls, a) : cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep, a);
+        return cudaLaunchKernelEx(&cfg, qmcd_kernel, a);
+    };
+    cudaError_t e = fire();
+    if (e != cudaSuccess && G_act > 1) {
+        // helper clusters are an optimisation: when the cooperative launch is refused (device shared
+        // with other work, or a profiler that cannot replay cooperative cluster launches) run the
+        // same step with the leader clusters alone
+        (void)cudaGetLastError();
+        a.P.G_act = 1;
+        cfg.gridDim = dim3((unsigned)(h->batch * h->P.S), 1, 1);
+        cfg.numAttrs = 1;
+        e = fire();
     }
-    else CK(h, cudaLaunchKernelEx(&cfg, qmcd_kernel, a));
+    if (e != cudaSuccess) return cuda_fail(h, e, "cudaLaunchKernelEx");
     return QMCD_OK;
 }
 
