@@ -750,3 +750,23 @@ def test_invert_permutation_singular_and_pipeline(qmcd):
     assert _rel(R.cpu().numpy(), Ro) <= RTOL_RATIO
     assert np.max(np.abs(Bd.cpu().numpy() - Bo)) <= 1e-10
     q.close()
+
+
+def test_invert_c4_full_size_residual_and_lapack(qmcd):
+    """qmcd_invert at BASELINE configs[4]'s size (8 walkers, N = 4096, 512 threads x 2 CTAs/SM,
+    37 CTAs per walker): the north_star residual max|A.Ainv - I| <= 1e-8 for every walker (fp64
+    product on the device, a library call used as a checker only) and agreement with the LAPACK
+    inverse the input generator made."""
+    import torch
+    wl = inputs.make_workload(8, 4096, n_moves=1, seed=44)
+    q = qmcd.Qmcd(4096, 1, 8)
+    Ad = _dev(wl.A)
+    X, info = q.invert(Ad)
+    torch.cuda.synchronize()
+    assert int(info.abs().max()) == 0
+    eye = torch.eye(4096, dtype=torch.float64, device="cuda")
+    for w in range(8):
+        assert float((Ad[w] @ X[w] - eye).abs().max()) <= TOL_RESID
+        assert float((X[w] @ Ad[w] - eye).abs().max()) <= TOL_RESID
+    assert float((X - _dev(wl.Ainv)).abs().max()) <= 1e-9
+    q.close()
