@@ -770,3 +770,27 @@ def test_invert_c4_full_size_residual_and_lapack(qmcd):
         assert float((X[w] @ Ad[w] - eye).abs().max()) <= TOL_RESID
     assert float((X - _dev(wl.Ainv)).abs().max()) <= 1e-9
     q.close()
+
+
+@pytest.mark.parametrize("mode", ["bern0.5", "metropolis"])
+def test_c1_full_size_lockstep_default_launch_vs_oracle_path3(qmcd, mode):
+    """Lock-step at BASELINE configs[1]'s full size in the library's default launch configuration
+    (helper clusters, blocked look-ahead, kernel entry qmcd_kernel_sweep_ls) against the oracle's
+    literal path 3, every walker, every ratio."""
+    wl = inputs.make_config("c1")
+    K = 32
+    mask = wl.bernoulli_mask(0.5) if mode == "bern0.5" else None
+    u = wl.uniforms if mode == "metropolis" else None
+    Ao, Bo = wl.A.copy(), wl.Ainv.copy()
+    Ro, acco, flo, _ = oracle.run_lockstep(Ao, Bo, K, wl.proposals, mask=mask, uniforms=u)
+    g = gpu_sweep(qmcd, wl, K, mask=mask, uniforms=u, lockstep=1)
+    assert g["status"] == 0 and g["blocked"]
+    if u is not None:
+        near_tie = np.abs(u - np.minimum(1.0, Ro * Ro)) < 1e-9            # reading G20
+        assert np.array_equal(g["acc"][~near_tie], acco[~near_tie])
+    else:
+        assert np.array_equal(g["acc"], acco)
+    assert _rel(g["R"], Ro) <= RTOL_RATIO
+    assert np.max(np.abs(g["B"] - Bo)) <= 1e-9
+    assert np.all(flo == wl.n_moves // K) and np.all(g["counters"][:, 1] <= wl.n_moves // K)
+    check_residuals(wl, acco, g["B"])
