@@ -10,7 +10,8 @@ Paths (citations: /root/reference/PAPER.md):
   * path 0 -- explicit LU determinant ratio / inverse
   * path 1 -- rank-1 Sherman-Morrison, Eqs. 1-2
   * path 2 -- delayed rank-K, Eqs. 3-4
-Pins: tests/test_oracle_pins.py.  Parity unpinned: nothing.
+Pins: tests/test_oracle_pins.py (every function, incl. the residual on known non-zero
+cases).  Parity unpinned: nothing.
 """
 from __future__ import annotations
 

@@ -33,7 +33,9 @@
  *           (PAPER.md:78-93).
  * The method is exact, so path 0 is the definition of truth and
  * paths 1-2 must agree with it to rounding.  Pins: tests/test_oracle_pins.py.
- * Parity unpinned: nothing (every function below has a pin there; path 3: P11).
+ * Parity unpinned: nothing (every function below has a pin there; path 3: P11;
+ * orc_residual: test_residual_known_nonzero_values_order_and_sign -- known non-zero
+ * residuals, A.B versus B.A, negative entries, NaN).
  *
  * No blocking, fusion or reordering beyond what the formulas state; the only
  * parallelism is an OpenMP "parallel for" over independent walkers in the

@@ -48,6 +48,38 @@ def test_known_determinants():
     assert s == 1 and abs(la - math.log(np.prod(np.diag(T)))) < 1e-13
 
 
+# ------------------------------------------------------------------ the residual itself
+def test_residual_known_nonzero_values_order_and_sign():
+    """max|A.B - I| (BASELINE.json north_star) pinned on pairs whose residual is known in closed
+    form -- a residual that returns 0, drops the fabs, or forms B.A instead of A.B fails here."""
+    n, eps = 6, 2.0 ** -9                                # (1 + eps) - 1 is exact
+    I = np.eye(n)
+    # A = I, B = I + eps e_i e_j^T  ->  A.B - I = eps e_i e_j^T: exactly eps (off the diagonal and on it)
+    for (i, j) in [(1, 4), (4, 1), (2, 2)]:
+        E = np.zeros((n, n)); E[i, j] = eps
+        assert oracle.residual(I, I + E) == eps
+        assert oracle.residual(I, I - E) == eps          # a negative entry: needs the fabs
+    assert oracle.residual(I, I) == 0.0
+    assert oracle.residual(2.0 * I, I) == 1.0            # 2I.I - I = I
+    assert oracle.residual(I, np.zeros((n, n))) == 1.0   # -I
+    # order: a pair with max|A.B - I| != max|B.A - I|, hand-computable
+    A = np.array([[1.0, 4.0], [0.0, 1.0]])
+    B = np.array([[1.0, 0.0], [0.0, 3.0]])
+    # A.B - I = [[0, 12], [0, 2]] -> 12 ;  B.A - I = [[0, 4], [0, 2]] -> 4
+    assert oracle.residual(A, B) == 12.0
+    assert oracle.residual(B, A) == 4.0
+    # and against numpy on a random nonsymmetric pair where the two orders differ
+    rng = np.random.default_rng(77)
+    A = rng.standard_normal((9, 9)); B = rng.standard_normal((9, 9))
+    ab = float(np.max(np.abs(A @ B - np.eye(9)))); ba = float(np.max(np.abs(B @ A - np.eye(9))))
+    assert abs(ab - ba) > 1e-3
+    assert oracle.residual(A, B) == pytest.approx(ab, rel=1e-13)
+    assert oracle.residual(B, A) == pytest.approx(ba, rel=1e-13)
+    # a non-finite product is reported, not hidden
+    Bn = np.eye(3); Bn[1, 1] = np.nan
+    assert math.isnan(oracle.residual(np.eye(3), Bn))
+
+
 # ------------------------------------------------------------------ P3: A = I and diagonal A
 def test_P3_identity_and_diagonal_closed_forms():
     """PAPER.md:59-66 with A = I: R = v[j]; B_new = I - (v - e_j) e_j^T / v[j]."""
