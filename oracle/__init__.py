@@ -10,6 +10,8 @@ Paths (citations: /root/reference/PAPER.md):
   * path 0 -- explicit LU determinant ratio / inverse
   * path 1 -- rank-1 Sherman-Morrison, Eqs. 1-2
   * path 2 -- delayed rank-K, Eqs. 3-4
+  * path 3 -- lock-step variant; path 4 -- path 2 with the slot-replacement
+    accept for an electron accepted twice inside one window (reading G7)
 Pins: tests/test_oracle_pins.py (every function, incl. the residual on known non-zero
 cases).  Parity unpinned: nothing.
 """
@@ -93,6 +95,12 @@ def _load():
                                    _dp, _dp, _dp, _up, _dp, ctypes.c_int, ctypes.c_int,
                                    _dp, _up, ctypes.POINTER(ctypes.c_long), _ip]
     L.orc_run_lockstep.restype = ctypes.c_int
+    L.orc_delayed_set_replace.argtypes = [ctypes.c_void_p, ctypes.c_int]
+    L.orc_delayed_set_replace.restype = None
+    L.orc_run_jseq.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, _ip, ctypes.c_int,
+                               _dp, _dp, _up, _dp, ctypes.c_int, ctypes.c_int,
+                               _dp, _up, ctypes.POINTER(ctypes.c_long), _ip]
+    L.orc_run_jseq.restype = ctypes.c_int
     L.orc_residual.argtypes = [ctypes.c_int, _dp, _dp]
     L.orc_residual.restype = ctypes.c_double
     L.orc_max_threads.argtypes = []
@@ -186,7 +194,9 @@ class Delayed:
     """One walker's delayed rank-K state.  ``B`` is borrowed and
     updated in place at every flush."""
 
-    def __init__(self, B, K):
+    def __init__(self, B, K, replace=False):
+        """replace=True: path 4 -- an electron accepted again inside one window replaces the column of
+        its queue slot instead of flushing first (reading G7, second alternative)."""
         if not (isinstance(B, np.ndarray) and B.dtype == np.float64 and B.flags.c_contiguous):
             raise ValueError("B must be a C-contiguous float64 ndarray (updated in place)")
         self.B = B
@@ -196,6 +206,8 @@ class Delayed:
         self._h = self._L.orc_delayed_create(self.n, self.K, _p(B))
         if not self._h:
             raise OracleError("delayed_create: bad arguments (need 1 <= K <= N)")
+        if replace:
+            self._L.orc_delayed_set_replace(self._h, 1)
 
     def __del__(self):
         h, self._h = getattr(self, "_h", None), None
@@ -309,6 +321,40 @@ def run_lockstep(A, B, K, proposals, j_begin=0, mask=None, uniforms=None, final_
                                   mp, up, mode, int(bool(final_flush)), _p(R), acc.ctypes.data_as(_up),
                                   fl, ctypes.byref(thr))
     _chk(rc, "run_lockstep")
+    return R, acc, np.array(list(fl), dtype=np.int64), thr.value
+
+
+def run_jseq(B, K, proposals, jseq, replace, mask=None, uniforms=None, final_flush=True):
+    """Delayed rank-K run with an ARBITRARY electron sequence jseq [n_moves] (the same for every
+    walker).  replace=False: path 2 (a repeated electron flushes first); replace=True: path 4
+    (slot replacement).  Returns (R, acc, flushes [batch], threads_used); B updated in place."""
+    if not (isinstance(B, np.ndarray) and B.dtype == np.float64 and B.flags.c_contiguous and B.ndim == 3):
+        raise ValueError("B must be a C-contiguous float64 [batch][N][N] ndarray")
+    batch, n, _ = B.shape
+    proposals = _f64(proposals)
+    n_moves = proposals.shape[0]
+    if proposals.shape != (n_moves, batch, n):
+        raise ValueError("proposals must be [n_moves][batch][N]")
+    jseq = np.ascontiguousarray(jseq, dtype=np.int32)
+    if jseq.shape != (n_moves,):
+        raise ValueError("jseq must be [n_moves]")
+    if (mask is None) == (uniforms is None):
+        raise ValueError("exactly one of mask / uniforms")
+    R = np.zeros((n_moves, batch), dtype=np.float64)
+    acc = np.zeros((n_moves, batch), dtype=np.uint8)
+    fl = (ctypes.c_long * batch)()
+    thr = ctypes.c_int()
+    if mask is not None:
+        mask = np.ascontiguousarray(mask, dtype=np.uint8)
+        assert mask.shape == (n_moves, batch)
+        mp, up, mode = mask.ctypes.data_as(_up), None, 0
+    else:
+        uniforms = _f64(uniforms, (n_moves, batch))
+        mp, up, mode = None, _p(uniforms), 1
+    rc = _load().orc_run_jseq(batch, n, int(K), n_moves, jseq.ctypes.data_as(_ip), int(bool(replace)),
+                              _p(B), _p(proposals), mp, up, mode, int(bool(final_flush)), _p(R),
+                              acc.ctypes.data_as(_up), fl, ctypes.byref(thr))
+    _chk(rc, "run_jseq")
     return R, acc, np.array(list(fl), dtype=np.int64), thr.value
 
 

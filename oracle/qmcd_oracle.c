@@ -25,7 +25,8 @@
  *   S      = I_m + V'A^-1 U of Eq. 3 = W C^T  (derived below)
  *
  * Three independent paths (plus path 3, the lock-step variant of PAPER.md:97-99,
- * which is path 2 with every proposal occupying a queue slot):
+ * which is path 2 with every proposal occupying a queue slot, and path 4, path 2
+ * with the slot-replacement accept for a repeated electron -- pin P12):
  *   path 0  the plain definition: explicit LU determinants / inverse
  *           (PAPER.md:55,57 -- "p ~ det(A_new)/det(A)").
  *   path 1  classic rank-1 Sherman-Morrison, Eqs. 1-2.
@@ -259,6 +260,7 @@ typedef struct orc_delayed {
     double sd;      /*     B0[j,:].v                                    */
     double sR;
     long n_flush;
+    int replace;    /* slot-replacement accept for a repeated electron (path 4) */
 } orc_delayed;
 
 void orc_delayed_destroy(orc_delayed *h)
@@ -384,6 +386,26 @@ int orc_delayed_accept(orc_delayed *h)
     if (h->sj < 0) return ORC_EINVAL;
     int j = h->sj, flushed = 0;
     if (h->sR == 0.0 || !isfinite(h->sR)) return ORC_ESINGULAR;
+    if (h->replace)
+        for (int a = 0; a < h->m; ++a)
+            if (h->J[a] == j) {
+                /* Path 4 (reading G7, second alternative; the paper is silent,
+                 * PAPER.md:84): electron j_a moved again before the queue was applied.  The
+                 * current matrix is A0 with column j_a = the NEWEST accepted column, so the
+                 * queue entry keeps its slot and its row W[a,:] = B0[j_a,:] and only its column
+                 * changes: C[a,:] <- v.  S = W C^T is then rebuilt from its definition (plain
+                 * loops, no incremental trick); nothing is flushed and m is unchanged. */
+                const int m = h->m;
+                memcpy(h->C + (size_t)a * n, h->sv, sizeof(double) * (size_t)n);
+                for (int x = 0; x < m; ++x)
+                    for (int i = 0; i < m; ++i) {
+                        double t = 0.0;
+                        for (int k = 0; k < n; ++k) t += h->W[(size_t)x * n + k] * h->C[(size_t)i * n + k];
+                        h->S[(size_t)x * K + i] = t;
+                    }
+                h->sj = -1;
+                return 0;
+            }
     for (int i = 0; i < h->m; ++i)
         if (h->J[i] == j) {                 /* repeated electron: flush first */
             double *v = (double *)malloc(sizeof(double) * (size_t)n);
@@ -567,6 +589,62 @@ int orc_run_lockstep(int batch, int n, int K, int n_moves, int j_begin,
             orc_delayed_destroy(h);
         }
         free(col);
+        if (rc != ORC_OK) {
+#pragma omp critical
+            { if (err == ORC_OK) err = rc; }
+        }
+    }
+    return err;
+}
+
+/* Path 4 switch: with `on` != 0, accepting an electron that is already queued replaces the
+ * column of its queue slot instead of flushing first (see orc_delayed_accept). */
+void orc_delayed_set_replace(orc_delayed *h, int on) { h->replace = on ? 1 : 0; }
+
+/* ------------------------------------------------------------------ */
+/* Batch driver with an ARBITRARY electron sequence jseq[t] (the same  */
+/* for every walker) -- needed to exercise a repeated electron inside  */
+/* one window.  replace = 0: path 2 as it stands (flush first, G7);    */
+/* replace = 1: path 4 (slot replacement).  Other arguments as in      */
+/* orc_run; flushes_out[b] = number of Eq.-4 applications of walker b. */
+/* ------------------------------------------------------------------ */
+int orc_run_jseq(int batch, int n, int K, int n_moves, const int *jseq, int replace,
+                 double *B, const double *proposals, const unsigned char *mask,
+                 const double *uniforms, int mode, int final_flush,
+                 double *R_out, unsigned char *acc_out, long *flushes_out, int *threads_used)
+{
+    if (batch < 1 || n < 1 || n_moves < 0 || !B || (n_moves > 0 && !jseq)) return ORC_EINVAL;
+    if (mode == 0 && !mask) return ORC_EINVAL;
+    if (mode == 1 && !uniforms) return ORC_EINVAL;
+    int err = ORC_OK;
+    int nthreads = 1;
+#ifdef _OPENMP
+    nthreads = omp_get_max_threads();
+    if (nthreads > batch) nthreads = batch;
+#endif
+    if (threads_used) *threads_used = nthreads;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads)
+    for (int b = 0; b < batch; ++b) {
+        int rc = ORC_OK;
+        orc_delayed *h = orc_delayed_create(n, K, B + (size_t)b * n * n);
+        if (!h) rc = ORC_EINVAL;
+        else orc_delayed_set_replace(h, replace);
+        for (int t = 0; t < n_moves && rc == ORC_OK; ++t) {
+            const double *v = proposals + ((size_t)t * batch + b) * n;
+            double R;
+            rc = orc_delayed_ratio(h, jseq[t], v, &R);
+            if (rc != ORC_OK) break;
+            int acc;
+            if (mode == 0) acc = mask[(size_t)t * batch + b] != 0;
+            else { double pa = R * R; if (pa > 1.0) pa = 1.0; acc = uniforms[(size_t)t * batch + b] < pa; }
+            if (R_out) R_out[(size_t)t * batch + b] = R;
+            if (acc_out) acc_out[(size_t)t * batch + b] = (unsigned char)acc;
+            if (acc) { int r2 = orc_delayed_accept(h); if (r2 < 0) rc = r2; }
+            else orc_delayed_reject(h);
+        }
+        if (rc == ORC_OK && final_flush) rc = orc_delayed_flush(h);
+        if (h && flushes_out) flushes_out[b] = orc_delayed_flush_count(h);
+        if (h) orc_delayed_destroy(h);
         if (rc != ORC_OK) {
 #pragma omp critical
             { if (err == ORC_OK) err = rc; }

@@ -384,6 +384,71 @@ def test_P10_same_electron_twice_in_one_window():
     assert np.abs(B - np.linalg.inv(A)).max() < 1e-11
 
 
+# ------------------------------------------------------------------ P12: slot replacement (path 4, G7)
+def test_P12_slot_replacement_vs_bruteforce_and_flush_first():
+    """The same electron accepted again before the queue is applied (PAPER.md:84 is silent; DESIGN.md
+    G7, second alternative): the slot's column is replaced, nothing is flushed.  Every ratio against
+    the plain definition (library determinants), the inverse against the library inverse, and the
+    whole run against flush-first (path 2) -- the same ratios and inverse with fewer flushes."""
+    rng = np.random.default_rng(77)
+    n, K = 10, 6
+    A = np.eye(n) + 0.5 * rng.standard_normal((n, n)) / math.sqrt(n)
+    B = np.linalg.inv(A)
+    D = oracle.Delayed(B, K, replace=True)
+    pend = []
+    for j in (1, 4, 1, 4, 4, 2):
+        v = A[:, j] + 0.3 * rng.standard_normal(n)
+        An = A.copy(); An[:, j] = v
+        truth = np.linalg.det(An) / np.linalg.det(A)
+        assert D.ratio(j, v) == pytest.approx(truth, rel=1e-11)
+        assert D.accept() is False                   # never flushes: 3 distinct electrons < K
+        pend.append(D.pending)
+        A = An
+    assert pend == [1, 2, 2, 2, 2, 3]                # a repeat keeps its slot
+    assert list(D.J()) == [1, 4, 2]
+    assert D.flush_count == 0
+    # Eq. 3 still holds with the replaced columns: det S = det(A_cur) / det(A0)
+    A0 = np.linalg.inv(B)                            # B is still the stale inverse
+    assert np.linalg.det(D.S()) == pytest.approx(np.linalg.det(A) / np.linalg.det(A0), rel=1e-11)
+    D.flush()
+    assert np.abs(B - np.linalg.inv(A)).max() < 1e-11
+
+
+@pytest.mark.parametrize("K,p", [(64, 0.3), (8, 0.6), (3, 1.0), (1, 1.0)])
+def test_P12_run_jseq_replace_equals_flush_first_and_rank1(K, p):
+    """K = N = 64 at 30 % acceptance revisits queued electrons in every window (the case the verdict
+    names); path 4 must give path 2's ratios, decisions and inverse, with no more flushes."""
+    wl = inputs.make_workload(batch=2, N=64, n_moves=300, seed=5)
+    rng = np.random.default_rng(9)
+    jseq = rng.integers(0, 12, size=wl.n_moves).astype(np.int32)       # few electrons: many repeats
+    jseq[::7] = rng.integers(0, 64, size=len(jseq[::7]))
+    # proposals must perturb the CURRENT column j of the walked matrix only loosely: use the generator's
+    # columns of the initial matrix at jseq (reading G14)
+    props = np.stack([np.stack([wl.A[w][:, jseq[t]] for w in range(2)]) for t in range(wl.n_moves)])
+    props = props + 0.3 / 8.0 * np.random.default_rng(3).standard_normal(props.shape)
+    mask = (wl.uniforms < p).astype(np.uint8)
+    Bf, Br = wl.Ainv.copy(), wl.Ainv.copy()
+    Rf, af, flf, _ = oracle.run_jseq(Bf, K, props, jseq, False, mask=mask)
+    Rr, ar, flr, _ = oracle.run_jseq(Br, K, props, jseq, True, mask=mask)
+    assert np.array_equal(af, ar) and np.array_equal(af, mask)
+    assert np.abs(Rr / Rf - 1).max() < 1e-10
+    assert np.abs(Br - Bf).max() < 1e-10
+    assert (flr <= flf).all() and (K == 1 or (flr < flf).all())
+    # and against rank-1 Sherman-Morrison, move by move (path 1 has no queue at all)
+    for w in range(2):
+        B1 = wl.Ainv[w].copy()
+        for t in range(wl.n_moves):
+            assert oracle.sm_ratio(B1, int(jseq[t]), props[t, w]) == pytest.approx(Rr[t, w], rel=1e-10)
+            if mask[t, w]:
+                oracle.sm_accept(B1, int(jseq[t]), props[t, w])
+        assert np.abs(B1 - Br[w]).max() < 1e-10
+        A_cur = wl.A[w].copy()
+        for t in range(wl.n_moves):
+            if mask[t, w]:
+                A_cur[:, jseq[t]] = props[t, w]
+        assert np.max(np.abs(A_cur @ Br[w] - np.eye(64))) < 1e-10
+
+
 # ------------------------------------------------------------------ Metropolis mode (G11)
 def test_metropolis_rule_and_path_agreement():
     wl = inputs.make_workload(batch=2, N=40, n_moves=80, seed=21)
