@@ -42,6 +42,7 @@ extern "C" {
 #define QMCD_ESTATE    (-2)   /* call not legal in the handle's current state      */
 #define QMCD_ECUDA     (-3)   /* CUDA runtime/driver error (see qmcd_strerror)     */
 #define QMCD_ESINGULAR (-4)   /* device status: accept of a move with R==0/non-finite */
+#define QMCD_ENOMEM    (-5)   /* host allocation failed                             */
 
 typedef struct qmcd_ctx* qmcd_handle;   /* opaque */
 
@@ -117,6 +118,14 @@ int qmcd_status(qmcd_handle h, int* host_out, int* info_out);
  * chain (F1 small part + F2), queue append, flush (F3), whole sweep, proposals in
  * the current window (option "lockstep", else 0)}. */
 int qmcd_counters(qmcd_handle h, long long* counters_dev);
+
+/* Measurement aid (not part of the method).  stats_dev: [512][4] int64, one row per CTA of the
+ * last qmcd_sweep / qmcd_flush grids since set_inverse (leader clusters first, then the pool):
+ * {flush tiles done, SM cycles inside tiles (leader CTAs: inside their flush jobs), cycles looking
+ * for a tile (leader CTAs: waiting for tiles taken by others), cycles in the launch}.
+ * flush_rank_sum_dev: [batch] int64, the sum of the ranks m of the walker's flushes (with
+ * qmcd_counters[.][1] = their number it gives the mean flush rank).  Either may be NULL.  Enqueued. */
+int qmcd_worker_stats(qmcd_handle h, long long* stats_dev, long long* flush_rank_sum_dev);
 
 /* Device-resident run of n_moves proposals with no host round trip (the same
  * ratio -> accept -> flush-when-full sequence, one persistent launch; results

@@ -10,7 +10,7 @@ import os
 
 from . import buildlib
 
-OK, EINVAL, ESTATE, ECUDA, ESINGULAR = 0, -1, -2, -3, -4
+OK, EINVAL, ESTATE, ECUDA, ESINGULAR, ENOMEM = 0, -1, -2, -3, -4, -5
 
 # name -> (restype, argtypes); mirrors include/qmcd.h one to one
 _vp, _ci, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
@@ -28,6 +28,7 @@ SYMBOLS = {
     "qmcd_pending": (_ci, [_vp, _vp]),
     "qmcd_status": (_ci, [_vp, ctypes.POINTER(_ci), ctypes.POINTER(_ci)]),
     "qmcd_counters": (_ci, [_vp, _vp]),
+    "qmcd_worker_stats": (_ci, [_vp, _vp, _vp]),
     "qmcd_sweep": (_ci, [_vp, _ci, _ci, _vp, _vp, _vp, _vp, _vp]),
     "qmcd_sweep_host": (_ci, [_vp, _ci, _ci, _vp, _vp, _vp, _vp, _vp, _vp, _sz]),
     "qmcd_sweep_host_min_staging": (_sz, [_ci, _ci]),
@@ -180,6 +181,14 @@ class Qmcd:
         out = torch.empty((self.batch, 8), dtype=torch.int64, device="cuda")
         _chk(self._L.qmcd_counters(self._h, _ptr(out, torch.int64)), "qmcd_counters")
         return out
+
+    def worker_stats(self):
+        """-> (stats [512][4] int64 per CTA of the grid, flush_rank_sum [batch] int64); see qmcd.h."""
+        import torch
+        st = torch.empty((512, 4), dtype=torch.int64, device="cuda")
+        fr = torch.empty(self.batch, dtype=torch.int64, device="cuda")
+        _chk(self._L.qmcd_worker_stats(self._h, _ptr(st, torch.int64), _ptr(fr, torch.int64)), "qmcd_worker_stats")
+        return st, fr
 
     def status(self):
         st, info = _ci(), (_ci * 2)()

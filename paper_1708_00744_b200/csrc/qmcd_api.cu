@@ -23,7 +23,10 @@ struct qmcd_ctx {
     size_t smem_bytes;
     int max_cluster;          // largest cluster size the device can co-schedule
     int lookahead;            // qmcd_sweep: 0 auto (blocked when possible), 1 per move
-    unsigned launch_seq;      // tags the leader/helper words of each launch
+    int pool_opt;             // option "pool": -1 auto (every SM the leaders leave free), 0 off, > 0 that many CTAs
+    int coop;                 // option "cooperative": pooled launches ask the driver for co-residency
+    size_t ctl_off, ctl_bytes;    // job words inside the workspace (zeroed before every pooled launch)
+    unsigned char* ws;
     char last_cuda_error[256];
 };
 
@@ -38,15 +41,14 @@ static int cuda_fail(qmcd_ctx* h, cudaError_t e, const char* what) {
 
 static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-#define QMCD_GMAX 4        // clusters per walker (Y copies in the workspace)
-struct WsLayout { size_t C, W, Y, ybytes, M, J, m, sj, sR, sp, sc, sr, counters, status, go, done, total; };
+struct WsLayout { size_t C, W, Y, M, J, m, sj, sR, sp, sc, sr, counters, fstat, wstat, status, ticket, jdesc, fin, ctrl, ctl_end, total; };
 
 static WsLayout ws_layout(int N, int K, int batch) {
     WsLayout L; size_t o = 0;
     size_t kn = (size_t)batch * K * N * 8;
     L.C = o; o += al256(kn);
     L.W = o; o += al256(kn);
-    L.Y = o; L.ybytes = al256(kn); o += QMCD_GMAX * L.ybytes;     // one Y = M W per cluster of a walker
+    L.Y = o; o += al256(kn);                                      // Y = M W of Eq. 4 (K > 64 and the CUDA-core flush)
     L.M = o; o += al256((size_t)batch * K * K * 8);
     L.J = o; o += al256((size_t)batch * K * 4);
     L.m = o; o += al256((size_t)batch * 4);
@@ -56,29 +58,21 @@ static WsLayout ws_layout(int N, int K, int batch) {
     L.sc = o; o += al256((size_t)batch * K * 8);
     L.sr = o; o += al256((size_t)batch * K * 8);
     L.counters = o; o += al256((size_t)batch * 8 * 8);
+    L.fstat = o; o += al256((size_t)batch * 2 * 8);
+    L.wstat = o; o += al256((size_t)QMCD_WSTAT_CTAS * 4 * 8);
     L.status = o; o += 256;
-    L.go = o; o += al256((size_t)batch * 8);
-    L.done = o; o += al256((size_t)batch * 16 * 8);
+    L.ticket = o; o += al256((size_t)batch * 8);                  // job words: one block, zeroed per launch
+    L.jdesc = o; o += al256((size_t)batch * 8);
+    L.fin = o; o += al256((size_t)batch * 4);
+    L.ctrl = o; o += 256;
+    L.ctl_end = o;
     L.total = o;
     return L;
 }
 
 extern "C" size_t qmcd_workspace_bytes(int N, int K, int batch) {
-    if (N < 1 || K < 1 || K > N || batch < 1) return 0;
+    if (N < 1 || K < 1 || K > N || K > 4095 || batch < 1) return 0;
     return ws_layout(N, K, batch).total;
-}
-
-static int pow2_floor(int x) { int p = 1; while (p * 2 <= x) p *= 2; return p; }
-
-// Pick CTAs per walker: fill the 148 SMs with batch*S CTAs, keep slices >= 64
-// columns, stay within what the device can co-schedule.
-static int default_cluster(int N, int batch, int sms, int max_cluster) {
-    int s = pow2_floor(sms / batch > 0 ? sms / batch : 1);
-    int cap_n = pow2_floor(N / 64 > 0 ? N / 64 : 1);
-    if (s > cap_n) s = cap_n;
-    if (s > max_cluster) s = max_cluster;
-    if (s < 1) s = 1;
-    return s;
 }
 
 static int configure_kernel(qmcd_ctx* h, int S) {
@@ -103,6 +97,7 @@ static int configure_kernel(qmcd_ctx* h, int S) {
     CK(h, cudaFuncSetAttribute(qmcd_kernel_sweep_ls, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     h->smem_bytes = smem;
     h->P.S = S;
+    if (h->K > 64) h->P.tile_rows = 64;          // T for 128 rows does not fit beside the chunk ring
     return QMCD_OK;
 }
 
@@ -120,25 +115,23 @@ static int max_active_clusters(qmcd_ctx* h, int S, int nclusters) {
     return n;
 }
 
-// Clusters per walker: as many as fit, but no more workers (S*G CTAs) than 64-row tiles of B,
-// and at most QMCD_GMAX when the flush keeps one Y = M W per cluster (K > 64).
-static int pick_G(int N, int K, int S, int limit) {
-    const int gmax = (K <= 64) ? 16 : QMCD_GMAX;
-    if (limit > gmax) limit = gmax;
-    int by_tiles = (N / 64) / S;
-    if (N % 64 != 0 || by_tiles < 1) by_tiles = 1;
-    if (limit > by_tiles) limit = by_tiles;
-    return limit < 1 ? 1 : limit;
+// Pool CTAs for a launch that may flush: every cluster the device can hold beyond the `batch`
+// leader clusters (0 when the leaders alone do not fit at once: a leader waits for its tiles, so
+// pool and leaders must be co-resident; the leaders then flush alone, each taking its own tiles).
+static int pool_ctas(qmcd_ctx* h) {
+    if (h->pool_opt == 0 || !h->P.mma_smem_ok || h->N % 64 != 0 || h->P.flush_path == 1) return 0;
+    const int fit = max_active_clusters(h, h->P.S, h->batch + 1);
+    int extra = fit - h->batch;
+    if (extra < 1) return 0;
+    if (h->pool_opt > 0 && extra * h->P.S > h->pool_opt) extra = h->pool_opt / h->P.S;
+    return extra * h->P.S;
 }
 
-// with_helpers: the walker's helper clusters take part (launches that may flush many rows)
-static int launch(qmcd_ctx* h, QmcdArgs& a, bool with_helpers) {
-    const int G_act = with_helpers ? h->P.G : 1;
-    a.P.G_act = G_act;
-    a.P.launch_id = ++h->launch_seq;
+// with_pool: launches that may flush many rows (qmcd_sweep, qmcd_flush) bring the pool along
+static int launch(qmcd_ctx* h, QmcdArgs& a, bool with_pool) {
+    int pool = with_pool ? pool_ctas(h) : 0;
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
-    cfg.gridDim = dim3((unsigned)(h->batch * G_act * h->P.S), 1, 1);
     cfg.blockDim = dim3(QMCD_THREADS, 1, 1);
     cfg.dynamicSmemBytes = h->smem_bytes;
     cfg.stream = h->stream;
@@ -147,33 +140,45 @@ static int launch(qmcd_ctx* h, QmcdArgs& a, bool with_helpers) {
     attr[0].val.clusterDim.x = (unsigned)h->P.S;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
+    // leaders wait for tiles taken by pool CTAs: ask the driver to guarantee co-residency of the
+    // whole grid (the launch fails instead of dead-locking when the device is shared)
+    attr[1].id = cudaLaunchAttributeCooperative;
+    attr[1].val.cooperative = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    if (G_act > 1) {
-        // helper clusters spin on their leader: ask the driver to guarantee co-residency of the
-        // whole grid (the launch fails instead of dead-locking when the device is shared)
-        attr[1].id = cudaLaunchAttributeCooperative;
-        attr[1].val.cooperative = 1;
-        cfg.numAttrs = 2;
-    }
     auto fire = [&]() -> cudaError_t {
+        a.P.pool = pool;
+        cfg.gridDim = dim3((unsigned)(h->batch * h->P.S + pool), 1, 1);
+        cfg.numAttrs = (pool > 0 && h->coop) ? 2 : 1;
+        cudaError_t e = cudaMemsetAsync(h->ws + h->ctl_off, 0, h->ctl_bytes, h->stream);   // job words of this launch
+        if (e != cudaSuccess) return e;
         if (a.mode == QMCD_MODE_SWEEP && a.blocked && h->P.m_in_smem)
             return h->P.lockstep ? cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep_ls, a) : cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep, a);
         return cudaLaunchKernelEx(&cfg, qmcd_kernel, a);
     };
     cudaError_t e = fire();
-    if (e != cudaSuccess && G_act > 1) {
-        // helper clusters are an optimisation: when the cooperative launch is refused (device shared
-        // with other work, or a profiler that cannot replay cooperative cluster launches) run the
-        // same step with the leader clusters alone
+    if (e != cudaSuccess && pool > 0) {
+        // the pool is an optimisation: when the cooperative launch is refused (device shared with
+        // other work) run the same step with the leader clusters alone
         (void)cudaGetLastError();
-        a.P.G_act = 1;
-        cfg.gridDim = dim3((unsigned)(h->batch * h->P.S), 1, 1);
-        cfg.numAttrs = 1;
+        pool = 0;
         e = fire();
     }
     if (e != cudaSuccess) return cuda_fail(h, e, "cudaLaunchKernelEx");
     return QMCD_OK;
+}
+
+// CTAs per leader cluster.  The look-ahead of a walker is a latency chain on its leader cluster
+// (strips: ~N (2m + 32) 8 / S bytes per CTA and block of 16 proposals; then ~1100 cycles per move
+// that do not shrink with S), while flush tiles go to any free CTA.  With many walkers the pool
+// hides one walker's look-ahead behind the others' flushes, so small clusters (more pool CTAs,
+// no DSMEM exchange) win; with few walkers the chain is exposed and a larger S shortens it.
+static int default_S(int N, int batch, int cap) {
+    int s = 1;
+    if (batch <= 4) s = 8; else if (batch <= 16) s = 2;
+    if ((long long)N * batch <= 16384) s *= 2;     // small problems: the flush is short, the chain dominates
+    while (s > 1 && (N / s < 64 || N % (8 * s) != 0)) s /= 2;
+    if (s > cap) s = cap;
+    return s < 1 ? 1 : s;
 }
 
 extern "C" int qmcd_create(qmcd_handle* out, int N, int K, int batch,
@@ -188,23 +193,27 @@ extern "C" int qmcd_create(qmcd_handle* out, int N, int K, int batch,
     CK(nullptr, cudaGetDeviceProperties(&prop, dev));
     if (prop.major < 10) { snprintf(g_last_error, sizeof(g_last_error), "device sm_%d%d is not Blackwell (sm_100a build)", prop.major, prop.minor); return QMCD_ECUDA; }
     qmcd_ctx* h = new (std::nothrow) qmcd_ctx();
-    if (!h) return QMCD_EINVAL;
+    if (!h) return QMCD_ENOMEM;
     memset(h, 0, sizeof(*h));
     h->N = N; h->K = K; h->batch = batch;
     h->stream = (cudaStream_t)cuda_stream;
     h->state = QMCD_IDLE;
     unsigned char* ws = (unsigned char*)workspace_dev;
     WsLayout L = ws_layout(N, K, batch);
+    h->ws = ws; h->ctl_off = L.ticket; h->ctl_bytes = L.ctl_end - L.ticket;
+    h->pool_opt = -1; h->coop = 1;
     QmcdDev& P = h->P;
     P.N = N; P.K = K; P.batch = batch; P.S = 1; P.B = nullptr;
     P.C = (double*)(ws + L.C); P.W = (double*)(ws + L.W); P.Y = (double*)(ws + L.Y);
     P.M = (double*)(ws + L.M); P.J = (int*)(ws + L.J); P.m = (int*)(ws + L.m);
     P.sj = (int*)(ws + L.sj); P.sR = (double*)(ws + L.sR);
     P.sp = (double*)(ws + L.sp); P.sc = (double*)(ws + L.sc); P.sr = (double*)(ws + L.sr);
-    P.counters = (long long*)(ws + L.counters); P.status = (int*)(ws + L.status);
-    P.go = (unsigned long long*)(ws + L.go); P.done = (unsigned long long*)(ws + L.done);
-    P.chain_regs = 1; P.G = 1; P.G_act = 1; P.launch_id = 0; P.y_stride = L.ybytes / 8;
+    P.counters = (long long*)(ws + L.counters); P.fstat = (long long*)(ws + L.fstat); P.wstat = (long long*)(ws + L.wstat); P.status = (int*)(ws + L.status);
+    P.ticket = (unsigned long long*)(ws + L.ticket); P.jdesc = (unsigned long long*)(ws + L.jdesc);
+    P.fin = (unsigned*)(ws + L.fin); P.ctrl = (unsigned*)(ws + L.ctrl);
+    P.chain_regs = 1; P.pool = 0;
     P.flush_path = 0;
+    P.tile_rows = (K <= 64 && N >= 2048) ? 128 : 64;
     int rc = QMCD_OK;
     do {
         cudaError_t e = cudaMemsetAsync(ws, 0, L.total, h->stream);
@@ -219,26 +228,14 @@ extern "C" int qmcd_create(qmcd_handle* out, int N, int K, int batch,
         }
         if (rc != QMCD_OK) break;
         h->max_cluster = 16;
-        // Choose (S, G): S CTAs per cluster, G clusters per walker, maximising the SMs a walker
-        // gets (S*G) among the shapes the device can hold at once (a helper cluster spins on
-        // its leader, so all batch*G clusters must be co-resident); ties go to the larger S.
-        const int s_cap = default_cluster(N, batch, 16 * batch, h->max_cluster);   // N / 64 and 16 cap it
-        int bestS = 1, bestG = 1;
-        double best_score = 0.0;
-        for (int S = s_cap; S >= 1; S /= 2) {
+        // S = CTAs per leader cluster: the default of default_S, halved until `batch` clusters of it
+        // are co-resident (so that a pool can be attached) or S = 1
+        int S = default_S(N, batch, h->max_cluster);
+        for (;; S /= 2) {
             rc = configure_kernel(h, S);
-            if (rc != QMCD_OK) break;
-            const int n = max_active_clusters(h, S, batch);
-            if (n < batch && S > 1) continue;
-            const int G = (n >= batch) ? pick_G(N, K, S, n / batch) : 1;
-            // SMs per walker, with a bonus for clusters of >= 4: the look-ahead products run on the
-            // leader cluster only and cost ~N/S per CTA (measured: c4 with S=2,G=9 is slower than S=4,G=4)
-            const double score = (double)(S * G) * (S >= 4 ? 1.25 : 1.0);
-            if (score > best_score) { best_score = score; bestS = S; bestG = G; }
+            if (rc != QMCD_OK || S == 1) break;
+            if (max_active_clusters(h, S, batch) >= batch) break;
         }
-        if (rc != QMCD_OK) break;
-        rc = configure_kernel(h, bestS);
-        h->P.G = bestG;
     } while (0);
     if (rc != QMCD_OK) {
         if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
@@ -267,6 +264,8 @@ extern "C" int qmcd_set_inverse(qmcd_handle h, double* Ainv_dev) {
     CK(h, cudaMemsetAsync(h->P.m, 0, (size_t)h->batch * 4, h->stream));
     CK(h, cudaMemsetAsync(h->P.sj, 0xff, (size_t)h->batch * 4, h->stream));
     CK(h, cudaMemsetAsync(h->P.counters, 0, (size_t)h->batch * 64, h->stream));
+    CK(h, cudaMemsetAsync(h->P.fstat, 0, (size_t)h->batch * 16, h->stream));
+    CK(h, cudaMemsetAsync(h->P.wstat, 0, (size_t)QMCD_WSTAT_CTAS * 32, h->stream));
     CK(h, cudaMemsetAsync(h->P.status, 0, 16, h->stream));
     h->has_inverse = true;
     return QMCD_OK;
@@ -352,6 +351,13 @@ extern "C" int qmcd_pending(qmcd_handle h, int* m_dev) {
 extern "C" int qmcd_counters(qmcd_handle h, long long* counters_dev) {
     if (!h || !counters_dev) return QMCD_EINVAL;
     CK(h, cudaMemcpyAsync(counters_dev, h->P.counters, (size_t)h->batch * 64, cudaMemcpyDeviceToDevice, h->stream));
+    return QMCD_OK;
+}
+
+extern "C" int qmcd_worker_stats(qmcd_handle h, long long* stats_dev, long long* flush_rank_sum_dev) {
+    if (!h || (!stats_dev && !flush_rank_sum_dev)) return QMCD_EINVAL;
+    if (stats_dev) CK(h, cudaMemcpyAsync(stats_dev, h->P.wstat, (size_t)QMCD_WSTAT_CTAS * 32, cudaMemcpyDeviceToDevice, h->stream));
+    if (flush_rank_sum_dev) CK(h, cudaMemcpy2DAsync(flush_rank_sum_dev, 8, h->P.fstat, 16, 8, (size_t)h->batch, cudaMemcpyDeviceToDevice, h->stream));
     return QMCD_OK;
 }
 
@@ -490,16 +496,33 @@ extern "C" int qmcd_sweep_host(qmcd_handle h, int j_begin, int n_moves,
 extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
     if (!h || !key) return QMCD_EINVAL;
     if (h->state != QMCD_IDLE) return QMCD_ESTATE;
-    if (!strcmp(key, "cluster")) {
-        if (value < 1 || value > 16 || value > h->N) return QMCD_EINVAL;
+    if (!strcmp(key, "cluster")) {                 // powers of two only: the blocked look-ahead deals 16 strip rows over the CTAs
+        if (value < 1 || value > 16 || value > h->N || (value & (value - 1)) != 0) return QMCD_EINVAL;
         CK(h, cudaStreamSynchronize(h->stream));
-        h->P.G = 1;
-        return configure_kernel(h, value);
+        const int old = h->P.S;
+        int rc = configure_kernel(h, value);
+        if (rc == QMCD_OK && max_active_clusters(h, value, 1) < 1) rc = QMCD_EINVAL;
+        if (rc != QMCD_OK) configure_kernel(h, old);
+        return rc;
     }
-    if (!strcmp(key, "clusters_per_walker")) {     // helper clusters spin on the leader: all must be co-resident
-        if (value < 1 || value > ((h->K <= 64) ? 16 : QMCD_GMAX)) return QMCD_EINVAL;
-        if (value > 1 && max_active_clusters(h, h->P.S, h->batch) < h->batch * value) return QMCD_EINVAL;
-        h->P.G = value;
+    if (!strcmp(key, "pool")) {                    // -1 auto, 0 off, n > 0: at most n pool CTAs
+        if (value < -1) return QMCD_EINVAL;
+        h->pool_opt = value;
+        return QMCD_OK;
+    }
+    if (!strcmp(key, "clusters_per_walker")) {     // round-1 name: 1 = leaders only (pool off), > 1 = pool on
+        if (value < 1) return QMCD_EINVAL;
+        h->pool_opt = (value == 1) ? 0 : -1;
+        return QMCD_OK;
+    }
+    if (!strcmp(key, "cooperative")) {             // 0: pooled launches without the co-residency guarantee (profilers)
+        if (value < 0 || value > 1) return QMCD_EINVAL;
+        h->coop = value;
+        return QMCD_OK;
+    }
+    if (!strcmp(key, "tile_rows")) {
+        if ((value != 64 && value != 128) || (value == 128 && h->K > 64)) return QMCD_EINVAL;
+        h->P.tile_rows = value;
         return QMCD_OK;
     }
     if (!strcmp(key, "flush_path")) {
@@ -529,7 +552,10 @@ extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
 extern "C" int qmcd_get_option(qmcd_handle h, const char* key) {
     if (!h || !key) return QMCD_EINVAL;
     if (!strcmp(key, "cluster")) return h->P.S;
-    if (!strcmp(key, "clusters_per_walker")) return h->P.G;
+    if (!strcmp(key, "clusters_per_walker")) return pool_ctas(h) > 0 ? 2 : 1;
+    if (!strcmp(key, "pool")) return pool_ctas(h);
+    if (!strcmp(key, "cooperative")) return h->coop;
+    if (!strcmp(key, "tile_rows")) return h->P.tile_rows;
     if (!strcmp(key, "flush_path")) return h->P.flush_path;
     if (!strcmp(key, "lookahead")) return h->lookahead;
     if (!strcmp(key, "lockstep")) return h->P.lockstep;
@@ -548,8 +574,9 @@ extern "C" const char* qmcd_strerror(int code) {
         case QMCD_ESTATE: return "call not legal in the current state";
         case QMCD_ECUDA: return g_last_error[0] ? g_last_error : "CUDA error";
         case QMCD_ESINGULAR: return "accepted a move with R == 0 or non-finite R (singular)";
+        case QMCD_ENOMEM: return "out of host memory";
         default: return "unknown error";
     }
 }
 
-extern "C" const char* qmcd_version(void) { return "qmcd 0.1 (sm_100a)"; }
+extern "C" const char* qmcd_version(void) { return "qmcd 0.2 (sm_100a)"; }

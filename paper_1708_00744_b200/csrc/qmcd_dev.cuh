@@ -1,8 +1,9 @@
 // qmcd_dev.cuh -- device-side state, shared-memory carving and small helpers.
-// One thread-block CLUSTER of S CTAs owns one walker (walkers are
-// independent, so there is no cross-cluster dependency anywhere).  CTA r of the
-// cluster owns COLUMN slice [N r/S, N (r+1)/S) of every length-N vector in the
-// look-ahead (Eq. 3) and ROW slice [N r/S, N (r+1)/S) of B in the flush (Eq. 4).
+// One thread-block CLUSTER of S CTAs LEADS one walker (walkers are
+// independent): CTA r of it owns COLUMN slice [N r/S, N (r+1)/S) of every length-N
+// vector in the look-ahead (Eq. 3).  The flush (Eq. 4) is cut into row tiles of B that
+// are taken, one at a time, by the leader's own CTAs and by the POOL: the CTAs of the
+// grid that lead no walker and serve the flush jobs of all of them (qmcd_kernel.cuh).
 #pragma once
 #include <cuda_runtime.h>
 #include <cooperative_groups.h>
@@ -11,6 +12,7 @@
 namespace cg = cooperative_groups;
 
 #define QMCD_THREADS 256
+#define QMCD_WSTAT_CTAS 512   // CTAs with a slot in QmcdDev::wstat
 #define QMCD_WARPS (QMCD_THREADS / 32)
 
 // Status codes mirrored from include/qmcd.h (kept numerically identical).
@@ -19,16 +21,17 @@ namespace cg = cooperative_groups;
 
 struct QmcdDev {
     int N, K, batch, S;       // S = CTAs per cluster
-    int G;                    // clusters per walker: cluster 0 leads (look-ahead + flush), the rest help flushing
-    int G_act;                // clusters per walker taking part in THIS launch (1 or G), set per launch
-    unsigned launch_id;       // host counter, tags the go / done words of this launch
-    size_t y_stride;          // doubles between the Y copies of two clusters of one walker
-    unsigned long long* go;   // [batch]      leader -> helpers: (launch id << 32) | (flush no. << 12) | m
-    unsigned long long* done; // [batch][16]   helper g -> leader: (launch id << 32) | flush no.
+    int pool;                 // pool CTAs (flush workers serving every walker) in THIS launch, set per launch
+    int tile_rows;            // rows of B per flush tile (64 or 128), host choice
+    // ---- flush jobs (leader cluster of walker b -> every worker: its own CTAs and the pool)
+    unsigned long long* ticket;   // [batch]  (job number << 32) | next tile; tiles are taken by CAS
+    unsigned long long* jdesc;    // [batch]  m | phase << 16 | ntiles << 32 of the posted job
+    unsigned* fin;                // [batch]  tiles completed since the launch began
+    unsigned* ctrl;               // [4]      [0] = leader clusters that have finished this launch
     double* B;                // [batch][N][N]  inverse, borrowed, updated in place
     double* C;                // [batch][K][N]  queued new columns v_i (one per row)
     double* W;                // [batch][K][N]  rows j_i of the stale inverse B0
-    double* Y;                // [batch][K][N]  scratch: Y = M W of Eq. 4
+    double* Y;                // [batch][K][N]  scratch: Y = M W of Eq. 4 (K > 64, CUDA-core path)
     double* M;                // [batch][K][K]  (I + V'A^-1 U)^-1 = (W C^T)^-1, ld = K
     int* J;                   // [batch][K]     queued electron indices
     int* m;                   // [batch]        queue length
@@ -38,6 +41,8 @@ struct QmcdDev {
     double* sc;               // [batch][K]     staged c = M q
     double* sr;               // [batch][K]     staged r = M^T p
     long long* counters;      // [batch][8]     accepted, flushes, cycles: look-ahead, chain, queue append, flush, total; [7] = proposals since the last flush (lock-step)
+    long long* fstat;         // [batch][2]     sum of flush ranks, (spare)
+    long long* wstat;         // [QMCD_WSTAT_CTAS][4]  per CTA of the grid: flush tiles done, cycles inside tiles, cycles looking for a tile, cycles in the launch
     int* status;              // [4]            sticky: code, walker, move counter
     int flush_path;           // 0 auto, 1 CUDA-core, 2 DMMA
     int mma_smem_ok;          // host: the DMMA flush's shared memory fits
@@ -157,13 +162,17 @@ __device__ __forceinline__ void qmcd_set_status(const QmcdDev& P, int code, int 
     }
 }
 
-// ---- leader <-> helper clusters of one walker: words in global memory, release / acquire at gpu scope
-#define QMCD_GO_EXIT 0xFFFFFu
+// ---- leader <-> flush workers: words in global memory, release / acquire at gpu scope
 __device__ __forceinline__ void qmcd_st_release(unsigned long long* p, unsigned long long v) {
     asm volatile("st.release.gpu.global.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
 }
 __device__ __forceinline__ unsigned long long qmcd_ld_acquire(const unsigned long long* p) {
     unsigned long long v;
     asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned qmcd_ld_acquire32(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }

@@ -1,9 +1,9 @@
 // qmcd_flush_mma.cuh -- FP64 tensor-core (DMMA) flush of Eq. 4, per tile of
-// 128 / 64 rows of B (tiles dealt round-robin to the walker's CTAs):
+// 128 / 64 rows of B (tiles are taken one at a time by whichever CTA is free: qmcd_kernel.cuh):
 //     T = B0 C^T - E_J   (row tile x m, reduction over N)          "NT stage"
 //     K <= 64:  T <- T M (warp-local)                              "TM stage"
 //               B <- B0 - T W                                      "NN stage"
-//     K >  64:  Y = M W first (m x N, by column slice, one cluster barrier), B <- B0 - T Y
+//     K >  64:  Y = M W first (m x N, a job of 64-column tiles of its own), then B <- B0 - T Y
 // sm_100a has no tcgen05 f64 kind; its FP64 tensor instruction is DMMA.8x8x4
 // (mma.sync.m8n8k4.f64), measured at 37 TFLOP/s against 34 for DFMA.  Operand
 // fragments are loaded as 16-byte vectors by permuting the contraction index
@@ -42,13 +42,10 @@ template <int N_> __device__ __forceinline__ void qmcd_cp_async_wait() {
     asm volatile("cp.async.wait_group %0;" :: "n"(N_) : "memory");
 }
 
-__device__ inline bool qmcd_flush_use_mma(const QmcdDev& P, int m, int G_act) {
+__device__ inline bool qmcd_flush_use_mma(const QmcdDev& P) {
     if (P.flush_path == 1) return false;
-    (void)G_act;
-    const bool ok = (P.N % 64 == 0) && ((P.N / P.S) % 64 == 0 || P.K <= 64) && P.mma_smem_ok;
-    if (!ok) return false;
-    (void)m;
-    return true;     // rank 1 (the K = 1 Sherman-Morrison path) too: measured 2-4x faster than the CUDA-core flush
+    // rank 1 (the K = 1 Sherman-Morrison path) too: measured 2-4x faster than the CUDA-core flush
+    return (P.N % 64 == 0) && P.mma_smem_ok;
 }
 
 // Stage `nrows` (<= 64, multiple of 8 after zero padding) rows x 64 columns of a
@@ -84,10 +81,11 @@ __device__ __forceinline__ void qmcd_stage_half(double* __restrict__ dst, const 
 }
 
 __device__ __forceinline__ double2 qmcd_lds128(const double* p) { return *reinterpret_cast<const double2*>(p); }
-// coherent (never .nc) 16-byte global load / store of B: the same kernel rewrites B
+// coherent 16-byte global load / store of B: the same kernel rewrites B, and a tile is taken by a
+// different CTA from one flush to the next, so the loads go to L2 (.cg), never through L1
 __device__ __forceinline__ double2 qmcd_ldg128(const double* p) {
     double2 v;
-    asm volatile("ld.global.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p) : "memory");
+    asm volatile("ld.global.cg.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p) : "memory");
     return v;
 }
 __device__ __forceinline__ void qmcd_stg128(double* p, double x, double y) {
@@ -408,69 +406,86 @@ __device__ void qmcd_mma_tm(double* __restrict__ Ts, int ldT, int mp8, const dou
     __syncwarp();
 }
 
-// Tiles of R rows of B are dealt round-robin to the walker's workers (every CTA of
-// every participating cluster; helper clusters first, the leader cluster last).
-__device__ __forceinline__ int qmcd_worker_id(const QmcdDev& P, const QmcdWalker& w) {
-    return (w.g == 0) ? (P.G_act - 1) * P.S + w.r : (w.g - 1) * P.S + w.r;
+// ---------------------------------------------------------------------------
+// One tile of one flush job of walker b (the unit of work a CTA takes from the
+// walker's ticket word, qmcd_kernel.cuh).  Job phases:
+//   0 (K <= 64): row tile, entirely local:  T = -(B C^T - E_J);  T <- T M;  B += T W
+//   1 (K >  64): 64-column tile of Y = M W
+//   2 (K >  64): row tile with the finished Y:  T = -(B C^T - E_J);  B += T Y
+// `mf_key` caches which job's M sits in this CTA's Mf area (phase 0).
+// ---------------------------------------------------------------------------
+#define QMCD_JOB_LOCAL 0
+#define QMCD_JOB_Y 1
+#define QMCD_JOB_ROWS_Y 2
+#define QMCD_Y_TILE_COLS 64
+
+__host__ __device__ inline int qmcd_job_ntiles(int N, int tile_rows, int phase) {
+    return (phase == QMCD_JOB_Y) ? N / QMCD_Y_TILE_COLS : (N + tile_rows - 1) / tile_rows;
 }
 
 template <int A_T, int NS>
-__device__ void qmcd_flush_mma_impl(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
-                                    const QmcdWalker& w, int m) {
+__device__ void qmcd_flush_tile_impl(const QmcdDev& P, unsigned char* dyn, int b, int phase, int m, int tile,
+                                     unsigned long long job_key, unsigned long long& mf_key) {
     constexpr int R = 64 * A_T;
     const int N = P.N, K = P.K, tid = threadIdx.x;
     const int ldT = qmcd_mma_ldT(K);
     const int mp8 = (m + 7) & ~7;
-    double* Ts = reinterpret_cast<double*>(s.dyn);
+    double* Ts = reinterpret_cast<double*>(dyn);
     double* cb = Ts + (size_t)qmcd_mma_rows(K) * ldT;
-    const int NW = P.G_act * P.S, wf = qmcd_worker_id(P, w);
-    const int ntiles = (N + R - 1) / R;
-    if (K <= 64) {
-        // ---- local path: T = -(B C^T - E_J); T <- T M; B += T W.  No Y, no cluster barrier.
+    double* Bw = P.B + (size_t)b * N * N;
+    const double* Cw = P.C + (size_t)b * K * N;
+    const double* Ww = P.W + (size_t)b * K * N;
+    double* Yw = P.Y + (size_t)b * K * N;
+    const double* Mw = P.M + (size_t)b * K * K;
+    const int* Jw = P.J + (size_t)b * K;
+    if (phase == QMCD_JOB_LOCAL) {
         double* Mf = cb + (size_t)NS * QMCD_MMA_CHUNK_DOUBLES;
-        for (int idx = tid; idx < 64 * 64; idx += QMCD_THREADS) {
-            const int a = idx >> 6, b = idx & 63;
-            Mf[a * QMCD_MMA_LDX + b] = (a < m && b < m) ? __ldcg(w.M + (size_t)a * K + b) : 0.0;
-        }
-        for (int tile = wf; tile < ntiles; tile += NW) {
-            const int row0 = tile * R, nvalid = min(R, N - row0);
-            if (mp8 <= 32) qmcd_mma_nt<A_T, 4, NS>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
-            else qmcd_mma_nt<A_T, 8, NS>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
-            qmcd_mma_tm<A_T>(Ts, ldT, mp8, Mf);      // (the NT stage ended with a barrier: Mf and Ts are visible)
-            qmcd_mma_nn<A_T, true, NS>(Ts, ldT, mp8, w.W, m, N, w.B, row0, nvalid, 0, N, cb);
+        if (mf_key != job_key) {                       // M of this job is not staged yet in this CTA
             __syncthreads();
+            for (int idx = tid; idx < 64 * 64; idx += QMCD_THREADS) {
+                const int a = idx >> 6, bb = idx & 63;
+                Mf[a * QMCD_MMA_LDX + bb] = (a < m && bb < m) ? __ldcg(Mw + (size_t)a * K + bb) : 0.0;
+            }
+            mf_key = job_key;
         }
+        const int row0 = tile * R, nvalid = min(R, N - row0);
+        if (mp8 <= 32) qmcd_mma_nt<A_T, 4, NS>(Bw, N, row0, nvalid, Cw, Jw, m, Ts, ldT, cb);
+        else qmcd_mma_nt<A_T, 8, NS>(Bw, N, row0, nvalid, Cw, Jw, m, Ts, ldT, cb);
+        qmcd_mma_tm<A_T>(Ts, ldT, mp8, Mf);      // (the NT stage ended with a barrier: Mf and Ts are visible)
+        qmcd_mma_nn<A_T, true, NS>(Ts, ldT, mp8, Ww, m, N, Bw, row0, nvalid, 0, N, cb);
+        __syncthreads();
         return;
     }
-    // ---- Y = M W on my column slice, M taken R rows at a time as the A operand
-    for (int r0 = 0; r0 < m; r0 += R) {
-        for (int idx = tid; idx < R * mp8; idx += QMCD_THREADS) {
-            const int r = idx / mp8, a = idx - r * mp8;
-            Ts[(size_t)r * ldT + a] = (r0 + r < m && a < m) ? __ldcg(w.M + (size_t)(r0 + r) * K + a) : 0.0;
+    mf_key = 0;                                        // the other phases overwrite the Mf area's neighbours / Ts
+    if (phase == QMCD_JOB_Y) {
+        // Y[:, c0 .. c0+64) = M W[:, c0 .. c0+64), M taken R rows at a time as the A operand
+        const int c0 = tile * QMCD_Y_TILE_COLS;
+        for (int r0 = 0; r0 < m; r0 += R) {
+            __syncthreads();
+            for (int idx = tid; idx < R * mp8; idx += QMCD_THREADS) {
+                const int r = idx / mp8, a = idx - r * mp8;
+                Ts[(size_t)r * ldT + a] = (r0 + r < m && a < m) ? __ldcg(Mw + (size_t)(r0 + r) * K + a) : 0.0;
+            }
+            __syncthreads();
+            qmcd_mma_nn<A_T, false, NS>(Ts, ldT, mp8, Ww, m, N, Yw, r0, min(R, m - r0), c0, c0 + QMCD_Y_TILE_COLS, cb);
         }
         __syncthreads();
-        qmcd_mma_nn<A_T, false, NS>(Ts, ldT, mp8, w.W, m, N, w.Y, r0, min(R, m - r0), w.klo, w.khi, cb);
-        __syncthreads();
+        return;
     }
-    if (P.S > 1) cl.sync(); else __syncthreads();
-    // ---- my tiles:  T = -(B C^T - E_J);  B += T Y
-    for (int tile = wf; tile < ntiles; tile += NW) {
-        const int row0 = tile * R, nvalid = min(R, N - row0);
-        if (mp8 <= 32) qmcd_mma_nt<A_T, 4, NS>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
-        else qmcd_mma_nt<A_T, 8, NS>(w.B, N, row0, nvalid, w.C, w.J, m, Ts, ldT, cb);
-        qmcd_mma_nn<A_T, true, NS>(Ts, ldT, mp8, w.Y, m, N, w.B, row0, nvalid, 0, N, cb);
-        __syncthreads();
-    }
+    const int row0 = tile * R, nvalid = min(R, N - row0);
+    if (mp8 <= 32) qmcd_mma_nt<A_T, 4, NS>(Bw, N, row0, nvalid, Cw, Jw, m, Ts, ldT, cb);
+    else qmcd_mma_nt<A_T, 8, NS>(Bw, N, row0, nvalid, Cw, Jw, m, Ts, ldT, cb);
+    qmcd_mma_nn<A_T, true, NS>(Ts, ldT, mp8, Yw, m, N, Bw, row0, nvalid, 0, N, cb);
+    __syncthreads();
 }
 
-// 128-row tiles when there are enough of them for every worker, else 64-row tiles
-__device__ inline void qmcd_flush_mma(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
-                                      const QmcdWalker& w, int m) {
-    const int NW = P.G_act * P.S;
+// tile_rows = 128 needs K <= 64 (T for 128 rows beside the chunk ring); the host guarantees it
+__device__ inline void qmcd_flush_tile(const QmcdDev& P, unsigned char* dyn, int b, int phase, int m, int tile,
+                                       unsigned long long job_key, unsigned long long& mf_key) {
     if (qmcd_mma_stages(P.K) == 3) {
-        if (qmcd_mma_rows(P.K) == 128 && P.N / 128 >= NW) qmcd_flush_mma_impl<2, 3>(P, s, cl, w, m);
-        else qmcd_flush_mma_impl<1, 3>(P, s, cl, w, m);
+        if (P.tile_rows == 128) qmcd_flush_tile_impl<2, 3>(P, dyn, b, phase, m, tile, job_key, mf_key);
+        else qmcd_flush_tile_impl<1, 3>(P, dyn, b, phase, m, tile, job_key, mf_key);
     } else {
-        qmcd_flush_mma_impl<1, 2>(P, s, cl, w, m);
+        qmcd_flush_tile_impl<1, 2>(P, dyn, b, phase, m, tile, job_key, mf_key);
     }
 }

@@ -1,73 +1,169 @@
-// qmcd_kernel.cuh -- the two __global__ entries over one body: clusters of S CTAs, G clusters
-// per walker.  qmcd_kernel runs one phase (per-call API) or the per-move sweep, qmcd_kernel_sweep
-// the blocked sweep (persistent: the whole move loop); helper clusters serve the flushes.
+// qmcd_kernel.cuh -- the __global__ entries over one body.  The grid is `batch` LEADER clusters of
+// S CTAs (cluster b leads walker b: look-ahead, accept, and the posting of its flush jobs) followed,
+// in qmcd_sweep / qmcd_flush launches, by the POOL: CTAs that lead no walker and take flush tiles of
+// whichever walker has some (work stealing through one CAS per tile).  While one walker's leader
+// runs its look-ahead chain, the pool and the other leaders keep the FP64 tensor pipe busy with the
+// flushes of the others; every SM of the device is in the grid.
 #pragma once
 #include "qmcd_phases.cuh"
 #include "qmcd_flush_mma.cuh"
 
-// Eq. 4 on this CTA's row slice (either path); ends with every CTA of the CLUSTER done.
-__device__ void qmcd_flush_rows(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
-                                const QmcdWalker& w, int m) {
-    if (qmcd_flush_use_mma(P, m, P.G_act)) qmcd_flush_mma(P, s, cl, w, m);
-    else qmcd_flush_simt(P, s, cl, w, m);
+// ---- job words (QmcdDev::ticket / jdesc / fin), all at gpu scope
+// jdesc = job number << 32 | ntiles << 16 | phase << 12 | m   (m <= 4095: checked by qmcd_create)
+__device__ __forceinline__ unsigned long long qmcd_jdesc_pack(unsigned seq, int m, int phase, int ntiles) {
+    return ((unsigned long long)seq << 32) | ((unsigned long long)(unsigned)ntiles << 16) |
+           ((unsigned long long)(unsigned)phase << 12) | (unsigned long long)(unsigned)m;
+}
+// does the (ticket, descriptor) pair read by one thread name a job with a tile left?
+__device__ __forceinline__ bool qmcd_job_has_tile(unsigned long long t, unsigned long long d) {
+    return (t >> 32) != 0 && (t >> 32) == (d >> 32) && (unsigned)t < (unsigned)((d >> 16) & 0xFFFFu);
+}
+// Try to take one tile of walker b's posted job.  One thread.  Returns the tile (>= 0) and the
+// job's (seq, m, phase), or -1 when the walker has no tile to give right now.  The descriptor is
+// written before the ticket is released and carries the job number, so a pair that matches and
+// survives the CAS belongs to one job.
+__device__ __forceinline__ int qmcd_take_tile(const QmcdDev& P, int b, unsigned& seq, int& m, int& phase) {
+    for (int tries = 0; tries < 4; ++tries) {
+        const unsigned long long t = qmcd_ld_acquire(P.ticket + b);
+        const unsigned long long d = __ldcg(P.jdesc + b);
+        if (!qmcd_job_has_tile(t, d)) return -1;
+        if (atomicCAS(P.ticket + b, t, t + 1) == t) {
+            seq = (unsigned)(t >> 32); m = (int)(d & 0xFFFu); phase = (int)((d >> 12) & 0xFu);
+            return (int)(unsigned)t;
+        }
+    }
+    return -1;
+}
+__device__ __forceinline__ void qmcd_tile_done(const QmcdDev& P, int b) {
+    __syncthreads();                       // every thread's stores of the tile are issued
+    if (threadIdx.x == 0) { __threadfence(); atomicAdd(P.fin + b, 1u); }
 }
 
-// Flush wrapper for the LEADER cluster: all its CTAs call it with the same m > 0.
-// M goes back to global memory first (the flush reads it from there).  With
-// G_act > 1 the walker's helper clusters are released through the `go` word
-// (they own the other row slices) and awaited through their `done` words.
-// Barriers: (entry) queue slots / M written by other CTAs become visible;
-// (exit) nobody restages slot 0 or reads B rows before every CTA is done.
-// s.iflag[8] counts the flushes of this launch (same value in every CTA).
+// One job of walker b posted by its leader cluster: every CTA of the cluster takes tiles until none
+// is left, then the leader thread waits until all `ntiles` are FINISHED (by whoever took them).
+// s.iflag[8] = jobs posted so far in this launch, s.iflag[10] = tiles they had (same in every CTA).
+__device__ void qmcd_run_job(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
+                             const QmcdWalker& w, int m, int phase, unsigned long long& mf_key) {
+    const int ntiles = qmcd_job_ntiles(P.N, P.tile_rows, phase);
+    const int k = s.iflag[8] + 1;
+    const unsigned expect = (unsigned)(s.iflag[10] + ntiles);
+    if (w.r == 0 && threadIdx.x == 0) {
+        __threadfence();                   // queue rows, M, J (and Y) written by this cluster, seen through its barriers
+        P.jdesc[w.b] = qmcd_jdesc_pack((unsigned)k, m, phase, ntiles);
+        qmcd_st_release(P.ticket + w.b, (unsigned long long)(unsigned)k << 32);
+    }
+    if (P.S > 1) cl.sync(); else __syncthreads();            // the job is posted before any CTA of the cluster looks for it
+    const bool prof = threadIdx.x == 0 && blockIdx.x < QMCD_WSTAT_CTAS;
+    long long c0 = prof ? clock64() : 0, ntile = 0;
+    for (;;) {
+        if (threadIdx.x == 0) {
+            unsigned seq; int mm, ph;
+            s.iflag[9] = qmcd_take_tile(P, w.b, seq, mm, ph);
+        }
+        __syncthreads();
+        const int tile = s.iflag[9];
+        __syncthreads();
+        if (tile < 0) break;
+        qmcd_flush_tile(P, s.dyn, w.b, phase, m, tile, ((unsigned long long)(w.b + 1) << 32) | (unsigned)k, mf_key);
+        qmcd_tile_done(P, w.b);
+        ++ntile;
+    }
+    long long c1 = prof ? clock64() : 0;
+    if (w.r == 0 && threadIdx.x == 0)
+        while (qmcd_ld_acquire32(P.fin + w.b) != expect) __nanosleep(40);
+    __syncthreads();
+    if (prof) {                                              // leader CTAs: [2] = cycles waiting for tiles others took
+        long long* ws = P.wstat + (size_t)blockIdx.x * 4;
+        ws[0] += ntile; ws[1] += c1 - c0; ws[2] += clock64() - c1;
+    }
+    if (threadIdx.x == 0) { s.iflag[8] = k; s.iflag[10] = (int)expect; }
+    if (P.S > 1) cl.sync(); else __syncthreads();
+}
+
+// Flush wrapper for the leader cluster: all its CTAs call it with the same m > 0.
+// M goes back to global memory first (the flush reads it from there).
+// Barriers: (entry) queue slots / M written by other CTAs are complete before the job is posted;
+// (exit) nobody restages slot 0 or reads B rows before every tile is finished.
 template <bool MS>
 __device__ void qmcd_flush_phase(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
                                  const QmcdWalker& w, int m, bool writeback = true) {
     if (writeback) qmcd_writeback_M<MS>(P, s, w, m);
+    __threadfence();
     if (P.S > 1) cl.sync(); else __syncthreads();
-    const int k = s.iflag[8] + 1;
-    if (P.G_act > 1 && w.r == 0 && threadIdx.x == 0) {
-        __threadfence();
-        qmcd_st_release(P.go + w.b, ((unsigned long long)P.launch_id << 32) | ((unsigned long long)k << 12) | (unsigned)m);
+    if (qmcd_flush_use_mma(P)) {
+        unsigned long long mf_key = 0;     // the look-ahead arrays alias the flush's shared memory
+        if (P.K <= 64) qmcd_run_job(P, s, cl, w, m, QMCD_JOB_LOCAL, mf_key);
+        else {
+            qmcd_run_job(P, s, cl, w, m, QMCD_JOB_Y, mf_key);
+            qmcd_run_job(P, s, cl, w, m, QMCD_JOB_ROWS_Y, mf_key);
+        }
+    } else {
+        qmcd_flush_simt(P, s, cl, w, m);   // CUDA-core path: the leader cluster alone, rows split over its CTAs
+        if (P.S > 1) cl.sync(); else __syncthreads();
     }
-    qmcd_flush_rows(P, s, cl, w, m);
-    __syncthreads();
-    if (threadIdx.x == 0) s.iflag[8] = k;
     if (w.r == 0 && threadIdx.x == 0) {
         P.m[w.b] = 0;
         P.counters[(size_t)w.b * 8 + 1] += 1;
         P.counters[(size_t)w.b * 8 + 7] = 0;          // a new window starts (lock-step proposal count)
-        const unsigned long long want = ((unsigned long long)P.launch_id << 32) | (unsigned)k;
-        for (int g = 1; g < P.G_act; ++g)
-            while (qmcd_ld_acquire(P.done + (size_t)w.b * 16 + g) != want) __nanosleep(20);
+        P.fstat[(size_t)w.b * 2] += m;
     }
-    if (P.S > 1) cl.sync(); else __syncthreads();
 }
 
-// Helper cluster (w.g > 0): flush my row slices whenever the leader says so, until it says exit.
-__device__ void qmcd_helper_loop(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
-                                 const QmcdWalker& w) {
-    for (int k = 1;; ++k) {
-        if (threadIdx.x == 0) {
-            unsigned long long v;
+// Pool CTA: take tiles of any walker's posted job until every leader cluster has finished the launch.
+// Warp 0 scans the ticket words (lane i looks at walker start + i), starting after the walker served last.
+__device__ void qmcd_pool_loop(const QmcdDev& P, const QmcdSmem& s) {
+    unsigned long long mf_key = 0;
+    int start = (int)((blockIdx.x * 7u) % (unsigned)P.batch);
+    const bool prof = threadIdx.x == 0 && blockIdx.x < QMCD_WSTAT_CTAS;
+    long long cy_busy = 0, cy_seek = 0, ntile = 0, c_begin = prof ? clock64() : 0, c0 = c_begin;
+    for (;;) {
+        if (threadIdx.x < 32) {
+            const int lane = threadIdx.x;
+            int got = -1, gb = 0, gm = 0, gph = 0; unsigned gseq = 0;
+            int idle = 0;
             for (;;) {
-                v = qmcd_ld_acquire(P.go + w.b);
-                if ((unsigned)(v >> 32) == P.launch_id) {
-                    const unsigned f = (unsigned)(v >> 12) & 0xFFFFFu;
-                    if (f == QMCD_GO_EXIT || f == (unsigned)k) break;
+                for (int b0 = 0; b0 < P.batch && got < 0; b0 += 32) {
+                    const int i = b0 + lane;
+                    int bb = start + i; if (bb >= P.batch) bb -= P.batch;
+                    bool has = false;
+                    if (i < P.batch) {
+                        const unsigned long long t = qmcd_ld_acquire(P.ticket + bb);
+                        const unsigned long long d = __ldcg(P.jdesc + bb);
+                        has = qmcd_job_has_tile(t, d);
+                    }
+                    unsigned mask = __ballot_sync(0xffffffffu, has);
+                    while (mask != 0 && got < 0) {
+                        const int l = __ffs(mask) - 1;
+                        mask &= mask - 1;
+                        int cand = start + b0 + l; if (cand >= P.batch) cand -= P.batch;
+                        if (lane == 0) { got = qmcd_take_tile(P, cand, gseq, gm, gph); gb = cand; }
+                        got = __shfl_sync(0xffffffffu, got, 0);
+                    }
                 }
-                __nanosleep(20);
+                if (got >= 0) break;
+                unsigned fin_leaders = 0;
+                if (lane == 0) fin_leaders = qmcd_ld_acquire32(P.ctrl);
+                fin_leaders = __shfl_sync(0xffffffffu, fin_leaders, 0);
+                if (fin_leaders >= (unsigned)P.batch) { got = -2; break; }
+                __nanosleep(idle < 8 ? 100 : 400);
+                ++idle;
             }
-            s.iflag[9] = (((unsigned)(v >> 12) & 0xFFFFFu) == QMCD_GO_EXIT) ? -1 : (int)(v & 0xFFFu);
+            if (lane == 0) { s.iflag[9] = got; s.iflag[11] = gb; s.iflag[12] = gm; s.iflag[13] = gph; s.iflag[14] = (int)gseq; }
         }
         __syncthreads();
-        const int m = s.iflag[9];
-        if (m < 0) return;
-        qmcd_flush_rows(P, s, cl, w, m);
-        if (P.S > 1) cl.sync(); else __syncthreads();      // the whole cluster is done with its rows
-        if (w.r == 0 && threadIdx.x == 0) {
-            __threadfence();
-            qmcd_st_release(P.done + (size_t)w.b * 16 + w.g, ((unsigned long long)P.launch_id << 32) | (unsigned)k);
-        }
+        const int tile = s.iflag[9], b = s.iflag[11], m = s.iflag[12], phase = s.iflag[13];
+        const unsigned seq = (unsigned)s.iflag[14];
+        __syncthreads();
+        if (prof) { const long long c1 = clock64(); cy_seek += c1 - c0; c0 = c1; }
+        if (tile < 0) break;
+        qmcd_flush_tile(P, s.dyn, b, phase, m, tile, ((unsigned long long)(b + 1) << 32) | seq, mf_key);
+        qmcd_tile_done(P, b);
+        if (prof) { const long long c1 = clock64(); cy_busy += c1 - c0; c0 = c1; ++ntile; }
+        start = b;                          // stay with this walker while it has tiles (its M is staged here)
+    }
+    if (prof) {
+        long long* ws = P.wstat + (size_t)blockIdx.x * 4;
+        ws[0] += ntile; ws[1] += cy_busy; ws[2] += cy_seek; ws[3] += clock64() - c_begin;
     }
 }
 
@@ -122,8 +218,8 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
         const double R = __ldcg(P.sR + b);
         // lock-step: this proposal takes a slot of the window whatever the decision
         int pw = QMCD_LOCKSTEP(P) ? (int)__ldcg(P.counters + (size_t)b * 8 + 7) + 1 : 0;
-        // every CTA has read the staged proposal before the leader clears it
-        if (S > 1) cl.sync();
+        // every thread has read the staged proposal before the leader clears it
+        if (S > 1) cl.sync(); else __syncthreads();
         bool acc;
         if (A.reject_all) acc = false;
         else if (A.uniforms) { double pa = fmin(1.0, R * R); acc = A.uniforms[b] < pa; }
@@ -229,7 +325,7 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
     if (r == 0 && tid == 0) { P.sj[b] = -1; P.m[b] = m; }
 }
 
-// Common prologue / epilogue of both entry points.  BLOCKED = true: the blocked sweep only (its
+// Common prologue / epilogue of the entry points.  BLOCKED != 0: the blocked sweep only (its
 // own register allocation: the per-move look-ahead of the generic entry is not compiled in).
 template <int BLOCKED>      // 0 generic, 1 blocked sweep, 2 blocked sweep in lock-step
 __device__ __forceinline__ void qmcd_kernel_body(const QmcdArgs& A) {
@@ -238,13 +334,14 @@ __device__ __forceinline__ void qmcd_kernel_body(const QmcdArgs& A) {
     cg::cluster_group cl = cg::this_cluster();
     const int S = P.S;
     const int r = (S > 1) ? (int)cl.block_rank() : 0;
-    const int cidx = blockIdx.x / S;                 // cluster index
-    const int b = cidx / P.G_act, g = cidx - b * P.G_act;
+    const int b = blockIdx.x / S;                    // cluster index: < batch leads walker b, else pool
     const QmcdSmem s = qmcd_carve(qmcd_smem_raw, P.N, P.K, S, P.m_in_smem != 0);
-    const QmcdWalker w = qmcd_walker(P, b, r, g, P.G_act);
-    if (threadIdx.x == 0) s.iflag[8] = 0;
+    if (threadIdx.x == 0) { s.iflag[8] = 0; s.iflag[10] = 0; }
     __syncthreads();
-    if (g > 0) { qmcd_helper_loop(P, s, cl, w); return; }
+    if (b >= P.batch) { qmcd_pool_loop(P, s); return; }
+    const QmcdWalker w = qmcd_walker(P, b, r);
+    const long long c_launch = clock64();
+    if (S > 1) cl.sync();                            // every CTA of the cluster runs before any remote shared-memory access
     if (BLOCKED) {
         int m = __ldcg(P.m + b);
         qmcd_load_state<true>(P, s, w, m);
@@ -255,10 +352,10 @@ __device__ __forceinline__ void qmcd_kernel_body(const QmcdArgs& A) {
         if (P.m_in_smem) qmcd_run<true>(A, s, cl, w);
         else qmcd_run<false>(A, s, cl, w);
     }
-    if (P.G_act > 1) {                               // release the helpers (every return path lands here)
+    if (threadIdx.x == 0 && blockIdx.x < QMCD_WSTAT_CTAS) P.wstat[(size_t)blockIdx.x * 4 + 3] += clock64() - c_launch;
+    if (P.pool > 0) {                                // tell the pool this walker is done (every return path lands here)
         if (S > 1) cl.sync(); else __syncthreads();
-        if (r == 0 && threadIdx.x == 0)
-            qmcd_st_release(P.go + b, ((unsigned long long)P.launch_id << 32) | ((unsigned long long)QMCD_GO_EXIT << 12));
+        if (r == 0 && threadIdx.x == 0) { __threadfence(); atomicAdd(P.ctrl, 1u); }
     }
 }
 

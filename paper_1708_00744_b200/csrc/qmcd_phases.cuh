@@ -4,27 +4,25 @@
 #pragma once
 #include "qmcd_dev.cuh"
 
-struct QmcdWalker {          // per-CTA view of the walker this cluster works for
+struct QmcdWalker {          // per-CTA view of the walker this (leader) cluster works for
     int b;                   // walker index
     int r;                   // CTA rank in the cluster
-    int g;                   // cluster index within the walker (0 = leader)
-    int klo, khi;            // column slice of the look-ahead and of Y = M W (per cluster)
-    int rlo, rhi;            // row slice of B in the flush (over all G_act * S CTAs of the walker)
+    int klo, khi;            // column slice of the look-ahead and of the CUDA-core flush's Y = M W
+    int rlo, rhi;            // row slice of B in the CUDA-core flush (over the S CTAs of the cluster)
     double *B, *C, *W, *Y, *M;
     int* J;
 };
 
-__device__ inline QmcdWalker qmcd_walker(const QmcdDev& P, int b, int r, int g, int G_act) {
+__device__ inline QmcdWalker qmcd_walker(const QmcdDev& P, int b, int r) {
     QmcdWalker w;
-    w.b = b; w.r = r; w.g = g;
+    w.b = b; w.r = r;
     w.klo = qmcd_slice_lo(P.N, P.S, r);
     w.khi = qmcd_slice_lo(P.N, P.S, r + 1);
-    w.rlo = qmcd_slice_lo(P.N, P.S * G_act, g * P.S + r);
-    w.rhi = qmcd_slice_lo(P.N, P.S * G_act, g * P.S + r + 1);
+    w.rlo = w.klo; w.rhi = w.khi;
     w.B = P.B + (size_t)b * P.N * P.N;
     w.C = P.C + (size_t)b * P.K * P.N;
     w.W = P.W + (size_t)b * P.K * P.N;
-    w.Y = P.Y + (size_t)b * P.K * P.N + (size_t)g * P.y_stride;   // every cluster forms its own Y = M W
+    w.Y = P.Y + (size_t)b * P.K * P.N;
     w.M = P.M + (size_t)b * P.K * P.K;
     w.J = P.J + (size_t)b * P.K;
     return w;

@@ -45,9 +45,10 @@ def test_workspace_bytes_validation(lib):
     assert lib.qmcd_workspace_bytes(8, 0, 1) == 0
     assert lib.qmcd_workspace_bytes(8, 9, 1) == 0          # K > N (reading G16)
     assert lib.qmcd_workspace_bytes(8, 8, 0) == 0
-    # K x N buffers per walker dominate: C, W and one Y per cluster of a walker (up to 4)
+    assert lib.qmcd_workspace_bytes(8192, 4096, 1) == 0    # K <= 4095: the job descriptor holds m in 12 bits
+    # K x N buffers per walker dominate: C, W and Y = M W (one per walker)
     big = lib.qmcd_workspace_bytes(4096, 256, 8)
-    assert 6 * 8 * 256 * 4096 * 8 <= big < 6 * 8 * 256 * 4096 * 8 + (8 << 20)
+    assert 3 * 8 * 256 * 4096 * 8 <= big < 3 * 8 * 256 * 4096 * 8 + (8 << 20)
 
 
 def test_strerror_and_version(lib):

@@ -24,7 +24,7 @@ def _rel(a, b):
 
 
 def gpu_sweep(qmcd, wl, K, mask=None, uniforms=None, final_flush=True, cluster=None, j_begin=0,
-              flush_path=None, lookahead=None, lockstep=None, G=None, split=None):
+              flush_path=None, lookahead=None, lockstep=None, G=None, split=None, tile_rows=None, pool=None):
     import torch
     q = qmcd.Qmcd(wl.N, K, wl.batch)
     if lockstep is not None:
@@ -36,7 +36,11 @@ def gpu_sweep(qmcd, wl, K, mask=None, uniforms=None, final_flush=True, cluster=N
     if lookahead is not None:
         q.set_option("lookahead", lookahead)
     if G is not None:
-        q.set_option("clusters_per_walker", G)
+        q.set_option("clusters_per_walker", G)       # round-1 name: 1 = leader clusters only, > 1 = with the pool
+    if pool is not None:
+        q.set_option("pool", pool)
+    if tile_rows is not None:
+        q.set_option("tile_rows", tile_rows)
     blocked = bool(q.get_option("blocked_ok")) and q.get_option("lookahead") == 0
     B = _dev(wl.Ainv)
     q.set_inverse(B)
@@ -55,7 +59,7 @@ def gpu_sweep(qmcd, wl, K, mask=None, uniforms=None, final_flush=True, cluster=N
     cnt = q.counters().cpu().numpy()
     pend = q.pending().cpu().numpy()
     out = dict(R=R.cpu().numpy(), acc=acc.cpu().numpy(), B=B.cpu().numpy(), status=st, info=info,
-               counters=cnt, pending=pend, S=q.get_option("cluster"), blocked=blocked)
+               counters=cnt, pending=pend, S=q.get_option("cluster"), blocked=blocked, pool=q.get_option("pool"))
     q.close()
     return out
 
@@ -175,8 +179,8 @@ def test_dmma_flush_matches_oracle(qmcd, N, K, batch, cluster, p):
 @pytest.mark.parametrize("N,K,batch,cluster,G", [(512, 32, 3, 4, 2), (512, 16, 2, 2, 4), (256, 8, 4, 1, 4),
                                                  (1024, 64, 2, 4, 4), (384, 24, 2, 2, 3)])
 def test_helper_clusters_share_the_flush(qmcd, N, K, batch, cluster, G):
-    """clusters_per_walker > 1: cluster 0 of a walker runs the look-ahead, all G clusters split
-    the rows of every flush (leader/helper handshake through global memory)."""
+    """With the pool (round-1 option name clusters_per_walker > 1): the leader cluster of a walker runs
+    the look-ahead and posts its flush jobs; its own CTAs and the pool CTAs take the row tiles."""
     wl = inputs.make_workload(batch, N, n_moves=N + 2 * K + 5, seed=31)
     mask = wl.bernoulli_mask(0.9)
     Bo = wl.Ainv.copy(); Ro, acco, _ = oracle.run(2, Bo, K, wl.proposals, mask=mask)
@@ -184,7 +188,7 @@ def test_helper_clusters_share_the_flush(qmcd, N, K, batch, cluster, G):
     q = qmcd.Qmcd(N, K, batch)
     q.set_option("cluster", cluster)
     q.set_option("clusters_per_walker", G)
-    assert q.get_option("clusters_per_walker") == G
+    assert q.get_option("pool") > 0
     B = _dev(wl.Ainv); q.set_inverse(B)
     R = torch.zeros((wl.n_moves, batch), dtype=torch.float64, device="cuda")
     acc = torch.zeros((wl.n_moves, batch), dtype=torch.uint8, device="cuda")
@@ -606,6 +610,51 @@ def test_randomized_shapes_seeds_modes_and_launch_splits(qmcd):
         assert np.array_equal(acc.cpu().numpy(), acco), ctx
         assert _rel(R.cpu().numpy(), Ro) <= RTOL_RATIO, ctx
         assert np.max(np.abs(B.cpu().numpy() - Bo)) <= 1e-10, ctx
+
+
+@pytest.mark.parametrize("N,K,batch,cluster,tile_rows,pool,p", [
+    (256, 16, 5, 1, 64, -1, 0.9),       # S = 1 leaders, everything else is pool
+    (256, 16, 5, 1, 128, -1, 0.9),      # 128-row tiles: two tiles per job
+    (512, 64, 3, 2, 128, -1, 0.99),     # full-rank local jobs
+    (512, 64, 3, 2, 64, 3, 0.99),       # a pool of one cluster (2 CTAs... rounded down to whole clusters)
+    (512, 96, 2, 4, 64, -1, 0.9),       # K > 64: the Y = M W job, then the row job with Y
+    (256, 200, 2, 1, 64, -1, 0.9),      # four m-blocks, several M row blocks, two-phase jobs
+    (320, 24, 40, 1, 64, -1, 0.5),      # 40 walkers drifting apart at 50 % acceptance, 5 tiles per job
+    (192, 1, 3, 1, 64, -1, 0.9),        # rank-1 jobs (K = 1 Sherman-Morrison) through the pool
+    (1024, 64, 2, 8, 128, -1, 0.99),    # clusters of 8: 15 fit, 13 of them pool
+    (128, 32, 140, 1, 64, -1, 0.8),     # 140 leaders + 8 pool CTAs
+])
+def test_pool_flush_jobs_match_oracle(qmcd, N, K, batch, cluster, tile_rows, pool, p):
+    """Flush jobs taken tile by tile by the leader's own CTAs and by the pool (qmcd_kernel.cuh): every
+    ratio, the accept sequence and the inverse against the oracle's delayed path, with launches cut in
+    the middle of a window and an explicit qmcd_flush in between; and the same run without the pool."""
+    wl = inputs.make_workload(batch, N, n_moves=min(2 * N, 700) + K + 3, seed=61)
+    mask = wl.bernoulli_mask(p)
+    Bo = wl.Ainv.copy(); Ro, acco, _ = oracle.run(2, Bo, K, wl.proposals, mask=mask)
+    g = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, tile_rows=tile_rows, pool=pool,
+                  split=[wl.n_moves // 3, wl.n_moves // 3 + 5])
+    assert g["status"] == 0 and g["S"] == cluster
+    assert g["pool"] > 0 and g["pool"] % cluster == 0
+    assert np.array_equal(g["acc"], acco)
+    assert _rel(g["R"], Ro) <= RTOL_RATIO
+    assert np.max(np.abs(g["B"] - Bo)) <= 1e-10
+    check_residuals(wl, mask, g["B"])
+    g0 = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, tile_rows=tile_rows, pool=0)
+    assert g0["pool"] == 0 and np.array_equal(g0["acc"], acco)
+    assert np.max(np.abs(g0["B"] - Bo)) <= 1e-10 and _rel(g0["R"], Ro) <= RTOL_RATIO
+
+
+def test_cluster_option_rejects_non_powers_of_two(qmcd):
+    """the blocked look-ahead deals its 16 strip rows over the CTAs of a cluster, which
+    needs a power of two; 3, 5, 6, 7 used to be accepted and raced."""
+    q = qmcd.Qmcd(768, 16, 2)
+    for bad in (3, 5, 6, 7, 12, 0, 17):
+        with pytest.raises(qmcd.QmcdError):
+            q.set_option("cluster", bad)
+    for ok in (1, 2, 4, 8):
+        q.set_option("cluster", ok)
+        assert q.get_option("cluster") == ok
+    q.close()
 
 
 # ------------------------------------------------------------------ lock-step variant (SURVEY 8(f1))
