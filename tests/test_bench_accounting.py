@@ -52,7 +52,11 @@ def test_mode_inputs_and_config_names():
     m, u = bench.mode_inputs(wl, "bern0.5")
     assert u is None and m.shape == (8, 2) and set(np.unique(m)) <= {0, 1}
     m, u = bench.mode_inputs(wl, "metropolis")
-    assert m is None and u is wl.uniforms
+    assert m is None and np.array_equal(u, wl.uniforms)
+    m, u = bench.mode_inputs(wl, "bern0.99", 5)            # the bounded sample of the oracle / K = 1 legs
+    assert m.shape == (5, 2) and np.array_equal(m, wl.bernoulli_mask(0.99)[:5])
+    assert bench.sample_moves(4096, 64) == 128 and bench.sample_moves(4096, 256) == 512 and bench.sample_moves(100, 64) == 100
+    assert bench.DEFAULT_CONFIG in ("c3", "c4")          # the headline is a large configuration
     assert set(inputs.CONFIGS) == {"c0", "c1", "c2", "c3", "c4"}
 
 
