@@ -1,5 +1,6 @@
 // qmcd_api.cu -- host side of the C-ABI declared in include/qmcd.h: argument and
 // state checks, workspace carving, launch policy.  No CPU fallback anywhere.
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdio.h>
@@ -25,6 +26,9 @@ struct qmcd_ctx {
     int lookahead;            // qmcd_sweep: 0 auto (blocked when possible), 1 per move
     int pool_opt;             // option "pool": -1 auto (every SM the leaders leave free), 0 off, > 0 that many CTAs
     int coop;                 // option "cooperative": pooled launches ask the driver for co-residency
+    QmcdTmaps tmaps;          // 4-D tensor maps of B, C, W, M for the TMA-fed flush (B re-encoded by set_inverse)
+    int tma_opt;              // option "tma": 1 = use the TMA-fed flush when the shape allows
+    bool tmaps_ok;            // C, W, M encoded
     size_t ctl_off, ctl_bytes;    // job words inside the workspace (zeroed before every pooled launch)
     unsigned char* ws;
     char last_cuda_error[256];
@@ -40,6 +44,7 @@ static int cuda_fail(qmcd_ctx* h, cudaError_t e, const char* what) {
 #define CK(h, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(h, e_, #call); } while (0)
 
 static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
+static int qmcd_ldMg_host(int K) { return K <= 64 ? 64 : K; }
 
 struct WsLayout { size_t C, W, Y, M, J, m, sj, sR, sp, sc, sr, counters, fstat, wstat, status, ticket, jdesc, fin, ctrl, ctl_end, total; };
 
@@ -49,7 +54,7 @@ static WsLayout ws_layout(int N, int K, int batch) {
     L.C = o; o += al256(kn);
     L.W = o; o += al256(kn);
     L.Y = o; o += al256(kn);                                      // Y = M W of Eq. 4 (K > 64 and the CUDA-core flush)
-    L.M = o; o += al256((size_t)batch * K * K * 8);
+    L.M = o; o += al256((size_t)batch * qmcd_ldMg_host(K) * qmcd_ldMg_host(K) * 8);
     L.J = o; o += al256((size_t)batch * K * 4);
     L.m = o; o += al256((size_t)batch * 4);
     L.sj = o; o += al256((size_t)batch * 4);
@@ -75,6 +80,48 @@ extern "C" size_t qmcd_workspace_bytes(int N, int K, int batch) {
     return ws_layout(N, K, batch).total;
 }
 
+// ---- TMA tensor maps (driver entry point fetched through the runtime: no link against libcuda)
+typedef CUresult (*qmcd_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static qmcd_encode_fn get_encode_fn() {
+    static qmcd_encode_fn fn = nullptr;
+    if (!fn) {
+        cudaDriverEntryPointQueryResult q;
+        void* p = nullptr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+        fn = (qmcd_encode_fn)p;
+    }
+    return fn;
+}
+// A row-major fp64 array [batch][rows][N] seen as {inner, rows, N / inner, batch}: inner = 8 without swizzle
+// (an 8 x 8 block of doubles lands as 512 contiguous bytes) or 16 with SWIZZLE_128B; box {inner, box_rows, groups, 1}.
+static bool encode_view(CUtensorMap* tm, double* base, int rows, int N, size_t batch_stride_elems, int batch,
+                        int inner, int box_rows, int groups, bool swizzle) {
+    qmcd_encode_fn enc = get_encode_fn();
+    if (!enc) return false;
+    cuuint64_t gd[4] = {(cuuint64_t)inner, (cuuint64_t)rows, (cuuint64_t)(N / inner), (cuuint64_t)batch};
+    cuuint64_t gs[3] = {(cuuint64_t)N * 8, (cuuint64_t)inner * 8, (cuuint64_t)batch_stride_elems * 8};
+    cuuint32_t bd[4] = {(cuuint32_t)inner, (cuuint32_t)box_rows, (cuuint32_t)groups, 1}, es[4] = {1, 1, 1, 1};
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, gd, gs, bd, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               swizzle ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+static bool tma_shape_ok(int N, int K) { return K <= 64 && N % 64 == 0 && N >= 128; }
+static void encode_queue_tmaps(qmcd_ctx* h) {
+    h->tmaps_ok = false;
+    if (!tma_shape_ok(h->N, h->K)) return;
+    const int N = h->N, K = h->K, rows = 8 * qmcd_tma_NB(K);
+    h->tmaps_ok = encode_view(&h->tmaps.C, h->P.C, K, N, (size_t)K * N, h->batch, 8, rows, 4, false) &&
+                  encode_view(&h->tmaps.W, h->P.W, K, N, (size_t)K * N, h->batch, 16, rows, 2, true) &&
+                  encode_view(&h->tmaps.M, h->P.M, 64, 64, (size_t)64 * 64, h->batch, 16, 64, 4, true);
+}
+static void refresh_use_tma(qmcd_ctx* h) {
+    h->P.use_tma = (h->tma_opt && h->tmaps_ok && h->P.B != nullptr && h->P.mma_smem_ok && h->P.flush_path != 1 &&
+                    h->smem_bytes >= qmcd_flush_tma_smem_bytes()) ? 1 : 0;
+    if (h->P.use_tma) h->P.tile_rows = QMCD_TMA_ROWS;
+}
+
 static int configure_kernel(qmcd_ctx* h, int S) {
     const size_t cap = 227 * 1024;
     // blocked look-ahead: 16-byte vector access to every slice, <= 40 output tiles
@@ -87,7 +134,8 @@ static int configure_kernel(qmcd_ctx* h, int S) {
     const size_t mma = QMCD_SMEM_HEADER + qmcd_flush_mma_smem_bytes(h->N, h->K);
     if (base > cap) { snprintf(g_last_error, sizeof(g_last_error), "shared memory need %zu > 227 KB", base); return QMCD_EINVAL; }
     h->P.mma_smem_ok = (mma <= cap) ? 1 : 0;
-    const size_t smem = (h->P.mma_smem_ok && mma > base) ? mma : base;
+    size_t smem = (h->P.mma_smem_ok && mma > base) ? mma : base;
+    if (tma_shape_ok(h->N, h->K) && qmcd_flush_tma_smem_bytes() > smem && qmcd_flush_tma_smem_bytes() <= cap) smem = qmcd_flush_tma_smem_bytes();
     // the attribute is per function, not per handle: always allow the device maximum
     CK(h, cudaFuncSetAttribute(qmcd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     CK(h, cudaFuncSetAttribute(qmcd_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
@@ -98,6 +146,7 @@ static int configure_kernel(qmcd_ctx* h, int S) {
     h->smem_bytes = smem;
     h->P.S = S;
     if (h->K > 64) h->P.tile_rows = 64;          // T for 128 rows does not fit beside the chunk ring
+    refresh_use_tma(h);
     return QMCD_OK;
 }
 
@@ -152,8 +201,8 @@ static int launch(qmcd_ctx* h, QmcdArgs& a, bool with_pool) {
         cudaError_t e = cudaMemsetAsync(h->ws + h->ctl_off, 0, h->ctl_bytes, h->stream);   // job words of this launch
         if (e != cudaSuccess) return e;
         if (a.mode == QMCD_MODE_SWEEP && a.blocked && h->P.m_in_smem)
-            return h->P.lockstep ? cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep_ls, a) : cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep, a);
-        return cudaLaunchKernelEx(&cfg, qmcd_kernel, a);
+            return h->P.lockstep ? cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep_ls, a, h->tmaps) : cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep, a, h->tmaps);
+        return cudaLaunchKernelEx(&cfg, qmcd_kernel, a, h->tmaps);
     };
     cudaError_t e = fire();
     if (e != cudaSuccess && pool > 0) {
@@ -212,7 +261,9 @@ extern "C" int qmcd_create(qmcd_handle* out, int N, int K, int batch,
     P.ticket = (unsigned long long*)(ws + L.ticket); P.jdesc = (unsigned long long*)(ws + L.jdesc);
     P.fin = (unsigned*)(ws + L.fin); P.ctrl = (unsigned*)(ws + L.ctrl);
     P.chain_regs = 1; P.pool = 0;
-    P.flush_path = 0;
+    P.flush_path = 0; P.use_tma = 0; P.ldMg = qmcd_ldMg_host(K);
+    h->tma_opt = 1;
+    encode_queue_tmaps(h);
     P.tile_rows = (K <= 64 && N >= 2048) ? 128 : 64;
     int rc = QMCD_OK;
     do {
@@ -261,6 +312,9 @@ extern "C" int qmcd_set_inverse(qmcd_handle h, double* Ainv_dev) {
     if (!h || !Ainv_dev || ((uintptr_t)Ainv_dev & 15)) return QMCD_EINVAL;
     if (h->state != QMCD_IDLE) return QMCD_ESTATE;
     h->P.B = Ainv_dev;
+    if (h->tmaps_ok && !encode_view(&h->tmaps.B, Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, QMCD_TMA_ROWS, 4, false))
+        h->tmaps_ok = false;
+    refresh_use_tma(h);
     CK(h, cudaMemsetAsync(h->P.m, 0, (size_t)h->batch * 4, h->stream));
     CK(h, cudaMemsetAsync(h->P.sj, 0xff, (size_t)h->batch * 4, h->stream));
     CK(h, cudaMemsetAsync(h->P.counters, 0, (size_t)h->batch * 64, h->stream));
@@ -520,14 +574,23 @@ extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
         h->coop = value;
         return QMCD_OK;
     }
-    if (!strcmp(key, "tile_rows")) {
+    if (!strcmp(key, "tile_rows")) {               // cp.async flush only (the TMA-fed flush works on 128-row tiles)
         if ((value != 64 && value != 128) || (value == 128 && h->K > 64)) return QMCD_EINVAL;
+        if (h->P.use_tma && value != QMCD_TMA_ROWS) return QMCD_EINVAL;
         h->P.tile_rows = value;
+        return QMCD_OK;
+    }
+    if (!strcmp(key, "tma")) {                     // 0: K <= 64 flush tiles through the cp.async kernels instead
+        if (value < 0 || value > 1) return QMCD_EINVAL;
+        h->tma_opt = value;
+        refresh_use_tma(h);
+        if (!h->P.use_tma && h->K <= 64) h->P.tile_rows = (h->N >= 2048) ? 128 : 64;
         return QMCD_OK;
     }
     if (!strcmp(key, "flush_path")) {
         if (value < 0 || value > 2) return QMCD_EINVAL;
         h->P.flush_path = value;
+        refresh_use_tma(h);
         return QMCD_OK;
     }
     if (!strcmp(key, "lookahead")) {
@@ -556,6 +619,7 @@ extern "C" int qmcd_get_option(qmcd_handle h, const char* key) {
     if (!strcmp(key, "pool")) return pool_ctas(h);
     if (!strcmp(key, "cooperative")) return h->coop;
     if (!strcmp(key, "tile_rows")) return h->P.tile_rows;
+    if (!strcmp(key, "tma")) return h->P.use_tma;
     if (!strcmp(key, "flush_path")) return h->P.flush_path;
     if (!strcmp(key, "lookahead")) return h->lookahead;
     if (!strcmp(key, "lockstep")) return h->P.lockstep;

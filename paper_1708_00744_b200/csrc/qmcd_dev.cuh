@@ -23,6 +23,8 @@ struct QmcdDev {
     int N, K, batch, S;       // S = CTAs per cluster
     int pool;                 // pool CTAs (flush workers serving every walker) in THIS launch, set per launch
     int tile_rows;            // rows of B per flush tile (64 or 128), host choice
+    int use_tma;              // host: K <= 64 flush tiles through qmcd_flush_tma.cuh (TMA-fed, 128-row tiles)
+    int ldMg;                 // row stride of M in GLOBAL memory: 64 when K <= 64 (a 64 x 64 tile, TMA box), else K
     // ---- flush jobs (leader cluster of walker b -> every worker: its own CTAs and the pool)
     unsigned long long* ticket;   // [batch]  (job number << 32) | next tile; tiles are taken by CAS
     unsigned long long* jdesc;    // [batch]  m | phase << 16 | ntiles << 32 of the posted job
@@ -32,7 +34,7 @@ struct QmcdDev {
     double* C;                // [batch][K][N]  queued new columns v_i (one per row)
     double* W;                // [batch][K][N]  rows j_i of the stale inverse B0
     double* Y;                // [batch][K][N]  scratch: Y = M W of Eq. 4 (K > 64, CUDA-core path)
-    double* M;                // [batch][K][K]  (I + V'A^-1 U)^-1 = (W C^T)^-1, ld = K
+    double* M;                // [batch][ldMg][ldMg]  (I + V'A^-1 U)^-1 = (W C^T)^-1, m x m valid, row stride ldMg
     int* J;                   // [batch][K]     queued electron indices
     int* m;                   // [batch]        queue length
     int* sj;                  // [batch]        staged electron, -1 = none
@@ -84,8 +86,10 @@ struct QmcdArgs {
 // header, then the look-ahead arrays.  The flush (either path) ALIASES everything
 // after the header (s.dyn): nothing there is live across a flush (M is written
 // back to global memory first, and the queue is empty afterwards).
+struct QmcdTmaps;
 struct QmcdSmem {
-    double* red;     // [40]  header: block-reduction scratch
+    const QmcdTmaps* tm;   // the kernel's tensor maps (a __grid_constant__ parameter)
+    double* red;     // [40]  header: block-reduction scratch (red == start of the CTA's dynamic shared memory)
     int* iflag;      // [16]  header
     unsigned char* dyn;  // start of the aliased region
     double* rs;      // [Ns]  slice of B0[j,:]
@@ -105,7 +109,7 @@ __host__ __device__ inline size_t qmcd_align16(size_t x) { return (x + 15) & ~(s
 __host__ __device__ inline int qmcd_PL(int K) { return 2 * K + 2; }
 __host__ __device__ inline int qmcd_ldM(int K) { return K | 1; }
 
-#define QMCD_SMEM_HEADER (40 * 8 + 16 * 4)      // red[40], iflag[16]; multiple of 16
+#define QMCD_SMEM_HEADER 1024                   // red[40], iflag[16] (384 B); the TMA ring's mbarriers at +512 (qmcd_flush_tma.cuh)
 
 // Bytes after the header: fixed arrays (pf qf cf rf Ts Js [Ms]) followed by a
 // union of the per-move look-ahead arrays (rs vs part) and the blocked
@@ -129,8 +133,10 @@ __device__ inline QmcdSmem qmcd_carve(unsigned char* base, int N, int K, int S, 
     QmcdSmem s;
     size_t ns = (size_t)(N + S - 1) / S + 1;
     unsigned char* p = base;
+    s.tm = nullptr;
     s.red = (double*)p; p += 40 * 8;
-    s.iflag = (int*)p; p += 16 * 4;
+    s.iflag = (int*)p;
+    p = base + QMCD_SMEM_HEADER;
     s.dyn = p;
     s.pf = (double*)p; p += qmcd_align16((size_t)K * 8);
     s.qf = (double*)p; p += qmcd_align16((size_t)K * 8);

@@ -436,7 +436,7 @@ __device__ void qmcd_flush_tile_impl(const QmcdDev& P, unsigned char* dyn, int b
     const double* Cw = P.C + (size_t)b * K * N;
     const double* Ww = P.W + (size_t)b * K * N;
     double* Yw = P.Y + (size_t)b * K * N;
-    const double* Mw = P.M + (size_t)b * K * K;
+    const double* Mw = P.M + (size_t)b * P.ldMg * P.ldMg;
     const int* Jw = P.J + (size_t)b * K;
     if (phase == QMCD_JOB_LOCAL) {
         double* Mf = cb + (size_t)NS * QMCD_MMA_CHUNK_DOUBLES;
@@ -444,7 +444,7 @@ __device__ void qmcd_flush_tile_impl(const QmcdDev& P, unsigned char* dyn, int b
             __syncthreads();
             for (int idx = tid; idx < 64 * 64; idx += QMCD_THREADS) {
                 const int a = idx >> 6, bb = idx & 63;
-                Mf[a * QMCD_MMA_LDX + bb] = (a < m && bb < m) ? __ldcg(Mw + (size_t)a * K + bb) : 0.0;
+                Mf[a * QMCD_MMA_LDX + bb] = (a < m && bb < m) ? __ldcg(Mw + (size_t)a * P.ldMg + bb) : 0.0;
             }
             mf_key = job_key;
         }
@@ -464,7 +464,7 @@ __device__ void qmcd_flush_tile_impl(const QmcdDev& P, unsigned char* dyn, int b
             __syncthreads();
             for (int idx = tid; idx < R * mp8; idx += QMCD_THREADS) {
                 const int r = idx / mp8, a = idx - r * mp8;
-                Ts[(size_t)r * ldT + a] = (r0 + r < m && a < m) ? __ldcg(Mw + (size_t)(r0 + r) * K + a) : 0.0;
+                Ts[(size_t)r * ldT + a] = (r0 + r < m && a < m) ? __ldcg(Mw + (size_t)(r0 + r) * P.ldMg + a) : 0.0;
             }
             __syncthreads();
             qmcd_mma_nn<A_T, false, NS>(Ts, ldT, mp8, Ww, m, N, Yw, r0, min(R, m - r0), c0, c0 + QMCD_Y_TILE_COLS, cb);

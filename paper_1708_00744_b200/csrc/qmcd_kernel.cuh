@@ -7,6 +7,7 @@
 #pragma once
 #include "qmcd_phases.cuh"
 #include "qmcd_flush_mma.cuh"
+#include "qmcd_flush_tma.cuh"
 
 // ---- job words (QmcdDev::ticket / jdesc / fin), all at gpu scope
 // jdesc = job number << 32 | ntiles << 16 | phase << 12 | m   (m <= 4095: checked by qmcd_create)
@@ -29,6 +30,7 @@ __device__ __forceinline__ int qmcd_take_tile(const QmcdDev& P, int b, unsigned&
         if (!qmcd_job_has_tile(t, d)) return -1;
         if (atomicCAS(P.ticket + b, t, t + 1) == t) {
             seq = (unsigned)(t >> 32); m = (int)(d & 0xFFFu); phase = (int)((d >> 12) & 0xFu);
+            qmcd_fence_proxy_async();      // what the acquire made visible is read next through TMA (async proxy)
             return (int)(unsigned)t;
         }
     }
@@ -37,6 +39,27 @@ __device__ __forceinline__ int qmcd_take_tile(const QmcdDev& P, int b, unsigned&
 __device__ __forceinline__ void qmcd_tile_done(const QmcdDev& P, int b) {
     __syncthreads();                       // every thread's stores of the tile are issued
     if (threadIdx.x == 0) { __threadfence(); atomicAdd(P.fin + b, 1u); }
+}
+
+// One tile of a job, by all threads of this CTA: the TMA-fed kernel for the local K <= 64 phase
+// (s.iflag[15] = iterations this CTA has pushed through the TMA ring), else the cp.async kernels.
+__device__ void qmcd_do_tile(const QmcdDev& P, const QmcdSmem& s, int b, int phase, int m, int tile,
+                             unsigned long long job_key, unsigned long long& mf_key) {
+    if (P.use_tma && phase == QMCD_JOB_LOCAL) {
+        unsigned char* base = reinterpret_cast<unsigned char*>(s.red);
+        unsigned itc = (unsigned)s.iflag[15];
+        switch (qmcd_tma_NB(P.K)) {
+            case 1: qmcd_flush_tile_tma<1>(P, *s.tm, base, b, m, tile, itc); break;
+            case 2: qmcd_flush_tile_tma<2>(P, *s.tm, base, b, m, tile, itc); break;
+            case 4: qmcd_flush_tile_tma<4>(P, *s.tm, base, b, m, tile, itc); break;
+            default: qmcd_flush_tile_tma<8>(P, *s.tm, base, b, m, tile, itc); break;
+        }
+        __syncthreads();                  // every warp has left the ring (and read iflag[15])
+        if (threadIdx.x == 0) s.iflag[15] = (int)itc;
+        mf_key = 0;
+        return;
+    }
+    qmcd_flush_tile(P, s.dyn, b, phase, m, tile, job_key, mf_key);
 }
 
 // One job of walker b posted by its leader cluster: every CTA of the cluster takes tiles until none
@@ -64,7 +87,7 @@ __device__ void qmcd_run_job(const QmcdDev& P, const QmcdSmem& s, cg::cluster_gr
         const int tile = s.iflag[9];
         __syncthreads();
         if (tile < 0) break;
-        qmcd_flush_tile(P, s.dyn, w.b, phase, m, tile, ((unsigned long long)(w.b + 1) << 32) | (unsigned)k, mf_key);
+        qmcd_do_tile(P, s, w.b, phase, m, tile, ((unsigned long long)(w.b + 1) << 32) | (unsigned)k, mf_key);
         qmcd_tile_done(P, w.b);
         ++ntile;
     }
@@ -88,7 +111,9 @@ template <bool MS>
 __device__ void qmcd_flush_phase(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
                                  const QmcdWalker& w, int m, bool writeback = true) {
     if (writeback) qmcd_writeback_M<MS>(P, s, w, m);
+    if (P.use_tma && qmcd_flush_use_mma(P)) qmcd_zero_pad_M(P, w, m);
     __threadfence();
+    qmcd_fence_proxy_async();              // queue rows / M written above are read through TMA by the flush
     if (P.S > 1) cl.sync(); else __syncthreads();
     if (qmcd_flush_use_mma(P)) {
         unsigned long long mf_key = 0;     // the look-ahead arrays alias the flush's shared memory
@@ -156,7 +181,7 @@ __device__ void qmcd_pool_loop(const QmcdDev& P, const QmcdSmem& s) {
         __syncthreads();
         if (prof) { const long long c1 = clock64(); cy_seek += c1 - c0; c0 = c1; }
         if (tile < 0) break;
-        qmcd_flush_tile(P, s.dyn, b, phase, m, tile, ((unsigned long long)(b + 1) << 32) | seq, mf_key);
+        qmcd_do_tile(P, s, b, phase, m, tile, ((unsigned long long)(b + 1) << 32) | seq, mf_key);
         qmcd_tile_done(P, b);
         if (prof) { const long long c1 = clock64(); cy_busy += c1 - c0; c0 = c1; ++ntile; }
         start = b;                          // stay with this walker while it has tiles (its M is staged here)
@@ -328,15 +353,19 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
 // Common prologue / epilogue of the entry points.  BLOCKED != 0: the blocked sweep only (its
 // own register allocation: the per-move look-ahead of the generic entry is not compiled in).
 template <int BLOCKED>      // 0 generic, 1 blocked sweep, 2 blocked sweep in lock-step
-__device__ __forceinline__ void qmcd_kernel_body(const QmcdArgs& A) {
+__device__ __forceinline__ void qmcd_kernel_body(const QmcdArgs& A, const QmcdTmaps& TM) {
     extern __shared__ __align__(1024) unsigned char qmcd_smem_raw[];
     const QmcdDev& P = A.P;
     cg::cluster_group cl = cg::this_cluster();
     const int S = P.S;
     const int r = (S > 1) ? (int)cl.block_rank() : 0;
     const int b = blockIdx.x / S;                    // cluster index: < batch leads walker b, else pool
-    const QmcdSmem s = qmcd_carve(qmcd_smem_raw, P.N, P.K, S, P.m_in_smem != 0);
-    if (threadIdx.x == 0) { s.iflag[8] = 0; s.iflag[10] = 0; }
+    QmcdSmem s = qmcd_carve(qmcd_smem_raw, P.N, P.K, S, P.m_in_smem != 0);
+    s.tm = &TM;
+    if (threadIdx.x == 0) {
+        s.iflag[8] = 0; s.iflag[10] = 0; s.iflag[15] = 0;
+        if (P.use_tma) qmcd_tma_init_barriers(qmcd_smem_raw);
+    }
     __syncthreads();
     if (b >= P.batch) { qmcd_pool_loop(P, s); return; }
     const QmcdWalker w = qmcd_walker(P, b, r);
@@ -359,6 +388,6 @@ __device__ __forceinline__ void qmcd_kernel_body(const QmcdArgs& A) {
     }
 }
 
-__global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel(const QmcdArgs A) { qmcd_kernel_body<0>(A); }
-__global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel_sweep(const QmcdArgs A) { qmcd_kernel_body<1>(A); }
-__global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel_sweep_ls(const QmcdArgs A) { qmcd_kernel_body<2>(A); }
+__global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel(const QmcdArgs A, const __grid_constant__ QmcdTmaps TM) { qmcd_kernel_body<0>(A, TM); }
+__global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel_sweep(const QmcdArgs A, const __grid_constant__ QmcdTmaps TM) { qmcd_kernel_body<1>(A, TM); }
+__global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel_sweep_ls(const QmcdArgs A, const __grid_constant__ QmcdTmaps TM) { qmcd_kernel_body<2>(A, TM); }

@@ -23,17 +23,17 @@ __device__ inline QmcdWalker qmcd_walker(const QmcdDev& P, int b, int r) {
     w.C = P.C + (size_t)b * P.K * P.N;
     w.W = P.W + (size_t)b * P.K * P.N;
     w.Y = P.Y + (size_t)b * P.K * P.N;
-    w.M = P.M + (size_t)b * P.K * P.K;
+    w.M = P.M + (size_t)b * P.ldMg * P.ldMg;
     w.J = P.J + (size_t)b * P.K;
     return w;
 }
 
 // M lives either in every CTA's shared memory (MS = true: s.Ms, row stride K|1,
 // identical copies kept in step by identical arithmetic) or, when K is too large
-// for that, in global memory (w.M, row stride K, written by the leader CTA only).
+// for that, in global memory (w.M, row stride P.ldMg, written by the leader CTA only).
 template <bool MS> struct QmcdM {
     static __device__ __forceinline__ const double* base(const QmcdSmem& s, const QmcdWalker& w) { return MS ? s.Ms : w.M; }
-    static __device__ __forceinline__ int ld(int K) { return MS ? qmcd_ldM(K) : K; }
+    static __device__ __forceinline__ int ld(const QmcdDev& P) { return MS ? qmcd_ldM(P.K) : P.ldMg; }
     static __device__ __forceinline__ double get(const double* p) { return MS ? *p : __ldcg(p); }
 };
 
@@ -129,7 +129,7 @@ __device__ double qmcd_lookahead(const QmcdDev& P, const QmcdSmem& s, cg::cluste
     // ---- c = M q and r = M^T p: 8 threads per index x, strided partial sums
     {
         const double* Mb = QmcdM<MS>::base(s, w);
-        const int ldM = QmcdM<MS>::ld(K);
+        const int ldM = QmcdM<MS>::ld(P);
         const int h = tid & 7;
         for (int x0 = 0; x0 < m; x0 += QMCD_THREADS / 8) {
             const int x = x0 + (tid >> 3);
@@ -171,11 +171,10 @@ template <bool MS>
 __device__ void qmcd_accept_update(const QmcdDev& P, const QmcdSmem& s, const QmcdWalker& w,
                                    int j, int m, double R) {
     const int tid = threadIdx.x;
-    const int K = P.K;
     const double sigma = 1.0 / R;
     if (MS || w.r == 0) {
         double* Mb = MS ? s.Ms : w.M;
-        const int ldM = QmcdM<MS>::ld(K);
+        const int ldM = QmcdM<MS>::ld(P);
         for (int idx = tid; idx < m * m; idx += QMCD_THREADS) {
             int a = idx / m, bb = idx - a * m;
             double* p = Mb + (size_t)a * ldM + bb;
@@ -205,7 +204,18 @@ __device__ void qmcd_writeback_M(const QmcdDev& P, const QmcdSmem& s, const Qmcd
     const int K = P.K, ldM = qmcd_ldM(K);
     for (int idx = threadIdx.x; idx < m * m; idx += QMCD_THREADS) {
         int a = idx / m, bb = idx - a * m;
-        w.M[(size_t)a * K + bb] = s.Ms[(size_t)a * ldM + bb];
+        w.M[(size_t)a * P.ldMg + bb] = s.Ms[(size_t)a * ldM + bb];
+    }
+}
+
+// Leader CTA, before a TMA-fed flush (P.use_tma): the 64 x 64 tile of M in global memory must be zero
+// outside its valid m x m block (the flush multiplies by the whole zero-padded tile; entries of an
+// earlier, longer window may still sit there).
+__device__ void qmcd_zero_pad_M(const QmcdDev& P, const QmcdWalker& w, int m) {
+    if (w.r != 0) return;
+    for (int idx = threadIdx.x; idx < 64 * 64; idx += QMCD_THREADS) {
+        const int a = idx >> 6, bb = idx & 63;
+        if (a >= m || bb >= m) w.M[(size_t)a * 64 + bb] = 0.0;
     }
 }
 
@@ -217,7 +227,7 @@ __device__ void qmcd_load_state(const QmcdDev& P, const QmcdSmem& s, const QmcdW
     if (MS)
         for (int idx = threadIdx.x; idx < m * m; idx += QMCD_THREADS) {
             int a = idx / m, bb = idx - a * m;
-            s.Ms[(size_t)a * ldM + bb] = __ldcg(w.M + (size_t)a * K + bb);
+            s.Ms[(size_t)a * ldM + bb] = __ldcg(w.M + (size_t)a * P.ldMg + bb);
         }
     __syncthreads();
 }
@@ -234,7 +244,7 @@ __device__ void qmcd_flush_simt(const QmcdDev& P, const QmcdSmem& s, cg::cluster
     // step 1: Y[a][k] = sum_b M[a][b] W[b][k], k in my column slice
     for (int k = w.klo + tid; k < w.khi; k += QMCD_THREADS) {
         for (int a = 0; a < m; ++a) {
-            const double* Ma = w.M + (size_t)a * K;
+            const double* Ma = w.M + (size_t)a * P.ldMg;
             double acc = 0;
             for (int bb = 0; bb < m; ++bb) acc += qmcd_ldcg(Ma + bb) * qmcd_ldcg(w.W + (size_t)bb * N + k);
             w.Y[(size_t)a * N + k] = acc;

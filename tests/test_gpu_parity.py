@@ -24,7 +24,7 @@ def _rel(a, b):
 
 
 def gpu_sweep(qmcd, wl, K, mask=None, uniforms=None, final_flush=True, cluster=None, j_begin=0,
-              flush_path=None, lookahead=None, lockstep=None, G=None, split=None, tile_rows=None, pool=None):
+              flush_path=None, lookahead=None, lockstep=None, G=None, split=None, tile_rows=None, pool=None, tma=None):
     import torch
     q = qmcd.Qmcd(wl.N, K, wl.batch)
     if lockstep is not None:
@@ -39,6 +39,8 @@ def gpu_sweep(qmcd, wl, K, mask=None, uniforms=None, final_flush=True, cluster=N
         q.set_option("clusters_per_walker", G)       # round-1 name: 1 = leader clusters only, > 1 = with the pool
     if pool is not None:
         q.set_option("pool", pool)
+    if tma is not None:
+        q.set_option("tma", tma)                     # 0: the cp.async flush kernels also for K <= 64
     if tile_rows is not None:
         q.set_option("tile_rows", tile_rows)
     blocked = bool(q.get_option("blocked_ok")) and q.get_option("lookahead") == 0
@@ -59,7 +61,8 @@ def gpu_sweep(qmcd, wl, K, mask=None, uniforms=None, final_flush=True, cluster=N
     cnt = q.counters().cpu().numpy()
     pend = q.pending().cpu().numpy()
     out = dict(R=R.cpu().numpy(), acc=acc.cpu().numpy(), B=B.cpu().numpy(), status=st, info=info,
-               counters=cnt, pending=pend, S=q.get_option("cluster"), blocked=blocked, pool=q.get_option("pool"))
+               counters=cnt, pending=pend, S=q.get_option("cluster"), blocked=blocked, pool=q.get_option("pool"),
+               tma=q.get_option("tma"))
     q.close()
     return out
 
@@ -612,36 +615,78 @@ def test_randomized_shapes_seeds_modes_and_launch_splits(qmcd):
         assert np.max(np.abs(B.cpu().numpy() - Bo)) <= 1e-10, ctx
 
 
-@pytest.mark.parametrize("N,K,batch,cluster,tile_rows,pool,p", [
-    (256, 16, 5, 1, 64, -1, 0.9),       # S = 1 leaders, everything else is pool
-    (256, 16, 5, 1, 128, -1, 0.9),      # 128-row tiles: two tiles per job
-    (512, 64, 3, 2, 128, -1, 0.99),     # full-rank local jobs
-    (512, 64, 3, 2, 64, 3, 0.99),       # a pool of one cluster (2 CTAs... rounded down to whole clusters)
-    (512, 96, 2, 4, 64, -1, 0.9),       # K > 64: the Y = M W job, then the row job with Y
-    (256, 200, 2, 1, 64, -1, 0.9),      # four m-blocks, several M row blocks, two-phase jobs
-    (320, 24, 40, 1, 64, -1, 0.5),      # 40 walkers drifting apart at 50 % acceptance, 5 tiles per job
-    (192, 1, 3, 1, 64, -1, 0.9),        # rank-1 jobs (K = 1 Sherman-Morrison) through the pool
-    (1024, 64, 2, 8, 128, -1, 0.99),    # clusters of 8: 15 fit, 13 of them pool
-    (128, 32, 140, 1, 64, -1, 0.8),     # 140 leaders + 8 pool CTAs
+@pytest.mark.parametrize("N,K,batch,cluster,path,pool,p", [
+    (256, 16, 5, 1, "tma", -1, 0.9),        # S = 1 leaders, everything else is pool; TMA-fed tiles, NB = 2
+    (256, 16, 5, 1, "cp64", -1, 0.9),       # the cp.async kernels on 64-row tiles
+    (256, 16, 5, 1, "cp128", -1, 0.9),      # ... on 128-row tiles: two tiles per job
+    (512, 64, 3, 2, "tma", -1, 0.99),       # full-rank local jobs, NB = 8
+    (512, 64, 3, 2, "cp128", -1, 0.99),
+    (512, 64, 3, 2, "cp64", 3, 0.99),       # a pool of one cluster (3 CTAs asked, rounded down to whole clusters)
+    (512, 96, 2, 4, "cp64", -1, 0.9),       # K > 64: the Y = M W job, then the row job with Y
+    (256, 200, 2, 1, "cp64", -1, 0.9),      # four m-blocks, several M row blocks, two-phase jobs
+    (320, 24, 40, 1, "tma", -1, 0.5),       # 40 walkers drifting apart at 50 % acceptance; 320 rows = 2.5 tiles (TMA clips)
+    (320, 24, 40, 1, "cp64", -1, 0.5),
+    (192, 1, 3, 1, "tma", -1, 0.9),         # rank-1 jobs (K = 1 Sherman-Morrison) through the pool, NB = 1
+    (192, 5, 3, 1, "tma", -1, 1.0),         # K not a multiple of 8: queue rows past K are zero-filled by TMA
+    (1024, 64, 2, 8, "tma", -1, 0.99),      # clusters of 8: 15 fit, 13 of them pool
+    (1024, 40, 2, 2, "tma", -1, 0.3),       # NB = 8 with ranks 33 ... 40 and low-rank final flushes
+    (128, 32, 140, 1, "tma", -1, 0.8),      # 140 leaders + 8 pool CTAs, one tile per job
+    (128, 32, 140, 1, "cp64", -1, 0.8),
 ])
-def test_pool_flush_jobs_match_oracle(qmcd, N, K, batch, cluster, tile_rows, pool, p):
-    """Flush jobs taken tile by tile by the leader's own CTAs and by the pool (qmcd_kernel.cuh): every
-    ratio, the accept sequence and the inverse against the oracle's delayed path, with launches cut in
-    the middle of a window and an explicit qmcd_flush in between; and the same run without the pool."""
+def test_pool_flush_jobs_match_oracle(qmcd, N, K, batch, cluster, path, pool, p):
+    """Flush jobs taken tile by tile by the leader's own CTAs and by the pool (qmcd_kernel.cuh), through the
+    TMA-fed tile kernel (qmcd_flush_tma.cuh) or the cp.async kernels: every ratio, the accept sequence and
+    the inverse against the oracle's delayed path, with launches cut in the middle of a window; and the
+    same run without the pool."""
     wl = inputs.make_workload(batch, N, n_moves=min(2 * N, 700) + K + 3, seed=61)
     mask = wl.bernoulli_mask(p)
     Bo = wl.Ainv.copy(); Ro, acco, _ = oracle.run(2, Bo, K, wl.proposals, mask=mask)
-    g = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, tile_rows=tile_rows, pool=pool,
-                  split=[wl.n_moves // 3, wl.n_moves // 3 + 5])
+    kw = dict(tma=1) if path == "tma" else dict(tma=0, tile_rows=int(path[2:]))
+    g = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, pool=pool,
+                  split=[wl.n_moves // 3, wl.n_moves // 3 + 5], **kw)
     assert g["status"] == 0 and g["S"] == cluster
+    assert g["tma"] == (1 if path == "tma" else 0)
     assert g["pool"] > 0 and g["pool"] % cluster == 0
     assert np.array_equal(g["acc"], acco)
     assert _rel(g["R"], Ro) <= RTOL_RATIO
     assert np.max(np.abs(g["B"] - Bo)) <= 1e-10
     check_residuals(wl, mask, g["B"])
-    g0 = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, tile_rows=tile_rows, pool=0)
+    g0 = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, pool=0, **kw)
     assert g0["pool"] == 0 and np.array_equal(g0["acc"], acco)
     assert np.max(np.abs(g0["B"] - Bo)) <= 1e-10 and _rel(g0["R"], Ro) <= RTOL_RATIO
+
+
+def test_tma_flush_per_call_api_partial_ranks_and_stale_M(qmcd):
+    """The TMA-fed flush behind the per-call API: a long window (rank 48) followed by short ones (ranks 3, 9)
+    flushed explicitly -- M's 64 x 64 tile in global memory still holds the long window's entries outside the
+    short windows' m x m blocks and must be zero-padded before the flush multiplies by the whole tile."""
+    import torch
+    N, K, batch = 256, 48, 3
+    wl = inputs.make_workload(batch, N, n_moves=48 + 3 + 9, seed=77)
+    q = qmcd.Qmcd(N, K, batch)
+    assert q.get_option("tma") == 0                    # no inverse adopted yet: no tensor map of B
+    B = _dev(wl.Ainv); q.set_inverse(B)
+    assert q.get_option("tma") == 1
+    P = _dev(wl.proposals)
+    R = torch.zeros(batch, dtype=torch.float64, device="cuda")
+    Bo = wl.Ainv.copy()
+    D = [oracle.Delayed(Bo[w], K) for w in range(batch)]
+    t = 0
+    for win in (48, 3, 9):
+        for _ in range(win):
+            q.ratio(t % N, P[t], R)
+            Rg = R.cpu().numpy()
+            for w in range(batch):
+                assert abs(D[w].ratio(t % N, wl.proposals[t, w]) / Rg[w] - 1) <= RTOL_RATIO
+                D[w].accept()
+            q.accept()
+            t += 1
+        q.flush()
+        for w in range(batch):
+            D[w].flush()
+        assert np.max(np.abs(B.cpu().numpy() - Bo)) <= 1e-10, win
+    assert q.status()[0] == 0
+    q.close()
 
 
 def test_cluster_option_rejects_non_powers_of_two(qmcd):
