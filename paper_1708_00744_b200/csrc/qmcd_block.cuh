@@ -393,14 +393,29 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
         QMCD_TICK(cy_chain);
         // ---- append the block's accepted moves to the queue: C[slot] = v, W[slot] = B0[j,:]
         {
-            const int vpr = len >> 1;
-            for (int idx = tid; idx < na * vpr; idx += QMCD_THREADS) {
-                const int e = idx / vpr, k = (idx - e * vpr) * 2;
-                const int al = __fns(accmask, 0, e + 1);
-                const double2 vv = qmcd_ldcg128(A.v + ((size_t)(t + al) * P.batch + w.b) * N + w.klo + k);
-                const double2 bb = qmcd_ldcg128(w.B + (size_t)((j0 + al) % N) * N + w.klo + k);
-                qmcd_stg128(w.C + (size_t)(m0 + e) * N + w.klo + k, vv.x, vv.y);
-                qmcd_stg128(w.W + (size_t)(m0 + e) * N + w.klo + k, bb.x, bb.y);
+            // four 16-byte vectors of each source row in flight per thread (the copy is a latency chain otherwise)
+            const int vpr = len >> 1, total = na * vpr;
+            for (int i0 = tid; i0 < total; i0 += 4 * QMCD_THREADS) {
+                double2 vv[4], bb[4];
+                size_t off[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int idx = i0 + u * QMCD_THREADS;
+                    if (idx < total) {
+                        const int e = idx / vpr, k = (idx - e * vpr) * 2;
+                        const int al = __fns(accmask, 0, e + 1);
+                        vv[u] = qmcd_ldcg128(A.v + ((size_t)(t + al) * P.batch + w.b) * N + w.klo + k);
+                        bb[u] = qmcd_ldcg128(w.B + (size_t)((j0 + al) % N) * N + w.klo + k);
+                        off[u] = (size_t)(m0 + e) * N + w.klo + k;
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    if (i0 + u * QMCD_THREADS < total) {
+                        qmcd_stg128(w.C + off[u], vv[u].x, vv[u].y);
+                        qmcd_stg128(w.W + off[u], bb[u].x, bb[u].y);
+                    }
+                }
             }
             __syncthreads();                       // Rb of the last move
             if (w.r == 0 && tid < L) {

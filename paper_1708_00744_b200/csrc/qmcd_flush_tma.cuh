@@ -1,35 +1,38 @@
 // qmcd_flush_tma.cuh -- the rank-m flush of Eq. 4 for K <= 64, one tile of 128 rows
 // of B per call, with every operand brought into shared memory by TMA (cp.async.bulk.tensor + mbarrier)
-// and the eight warps doing nothing but LDS.128 + DMMA.8x8x4:
+// and the eight warps doing nothing but LDS + DMMA.8x8x4 in straight-line code:
 //
 //     iterations 0 .. nk-1      (nk = N/32)   T  = B0[tile, 32 k-columns] . C[:, same]^T   accumulated in registers
 //     iteration  nk                            T  = -T + E_J ;  T <- T M                   (M = S^-1, 64 x 64, zero outside m x m)
 //     iterations nk+1 .. 2nk                   B[tile, 32 columns] += T . W[:, same]       written back from registers
 //
-// One ring of 3 stages of 48 KB carries all of it; stage contents per kind of iteration:
+// T NEVER LEAVES THE REGISTERS: with the permuted contraction index of qmcd_flush_mma.cuh (k-slot c of k-step s
+// is k = 8q + 2c + s) the accumulator fragment of n-tile q -- lane (g, c) holds T[g][8q + 2c], T[g][8q + 2c + 1] --
+// IS the A fragment of k-group q of the next product.  A warp owns 16 rows of the tile through all three parts.
+//
+// One ring of 4 stages of 48 KB carries everything else; stage contents per kind of iteration:
 //     NT : B0 tile as [4 k-groups][128 rows][8]      + C as [4 k-groups][8 NB rows][8]          (4-D tensor maps, no swizzle:
 //          an 8 x 8 fp64 fragment block is 512 contiguous bytes, so the 16-byte fragment loads are conflict-free)
-//     M  : M as [4 column groups][64 rows][16]       (SWIZZLE_128B: 16-byte chunk ^= row % 8 -- with the permuted
-//          contraction index k = 8q + 2c + s of qmcd_flush_mma.cuh the fragment loads are conflict-free)
-//     NN : B0 tile as [4 column groups][128 rows][8] + W as [2 column groups][8 NB rows][16]   (W swizzled like M)
-// A warp owns 16 rows of the tile through all three parts, so nothing but the ring's mbarriers synchronises
-// the CTA.  Thread 0 issues the loads two iterations ahead (half way through an iteration it waits for the
-// stage freed one iteration ago -- by then every warp has left it).  Rows past N and queue rows past K are
-// zero-filled by TMA; ranks m < K use the leading mp8 = round8(m) columns / rows only.
+//     M  : M as [4 column groups][64 rows][16]       (SWIZZLE_128B: 16-byte chunk ^= row % 8; read with 8-byte loads,
+//          n-slot g of tile t = column 8t + g, conflict-free under the same k permutation)
+//     NN : B0 tile as [4 column groups][128 rows][8] + W as [2 column groups][8 NB rows][16]   (W swizzled like M, read
+//          with 16-byte loads: n-slot g of tile t of group G is column 16G + 2g + t)
+// Lane 0 of warp (j mod 8) issues, at the top of iteration j, the loads of iteration j + 3 into the stage every warp
+// left in iteration j - 1.  Rows past N and queue rows past K are zero-filled by TMA.  Any rank m <= K runs the
+// full 8 NB columns: M is zero outside m x m, so the stale (finite) queue rows past m contribute exact zeros.
 #pragma once
 #include <cuda.h>
 #include "qmcd_flush_mma.cuh"
 
 struct QmcdTmaps { CUtensorMap B, C, W, M; };      // 4-D views, see qmcd_api.cu (encode_tmaps)
 
-#define QMCD_TMA_NS 3
+#define QMCD_TMA_NS 4
 #define QMCD_TMA_STAGE_BYTES 49152
-#define QMCD_TMA_BAR_OFF 512                 // full[3], empty[3] mbarriers inside the shared-memory header
+#define QMCD_TMA_BAR_OFF 512                 // full[NS], empty[NS] mbarriers inside the shared-memory header
 #define QMCD_TMA_STAGE_OFF 1024              // stages are 1024-byte aligned (swizzle atoms)
-#define QMCD_TMA_LDT 72                      // row stride of T in doubles (== 8 mod 16: conflict-free fragment loads)
 #define QMCD_TMA_ROWS 128
 __host__ __device__ inline size_t qmcd_flush_tma_smem_bytes() {
-    return (size_t)QMCD_TMA_STAGE_OFF + QMCD_TMA_NS * QMCD_TMA_STAGE_BYTES + (size_t)QMCD_TMA_ROWS * QMCD_TMA_LDT * 8;
+    return (size_t)QMCD_TMA_STAGE_OFF + QMCD_TMA_NS * QMCD_TMA_STAGE_BYTES;
 }
 __host__ __device__ inline int qmcd_tma_NB(int K) { return K <= 8 ? 1 : K <= 16 ? 2 : K <= 32 ? 4 : 8; }
 
@@ -68,23 +71,20 @@ __device__ __forceinline__ void qmcd_tma_init_barriers(unsigned char* smem) {
 // fixes stage and mbarrier parity), updated on return.  All 256 threads; ends without a CTA barrier.
 template <int NB>
 __device__ __noinline__ void qmcd_flush_tile_tma(const QmcdDev& P, const QmcdTmaps& TM, unsigned char* smem, int b, int m, int tile,
-                                    unsigned& itc) {
-    constexpr int NG = (NB + 1) / 2;              // 16-column groups of T
+                                                 unsigned& itc) {
     constexpr unsigned TX_ROWS = 32768u + 2048u * NB;
+    constexpr int NS = QMCD_TMA_NS;
     const int N = P.N, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, g = lane >> 2, c = lane & 3;
-    const int mp8 = (m + 7) & ~7, nqm = mp8 >> 3, nG = (mp8 + 15) >> 4;
     const int nk = N / 32, total = 2 * nk + 1;
     const int row0 = tile * QMCD_TMA_ROWS;
     const unsigned bar0 = qmcd_su32(smem + QMCD_TMA_BAR_OFF);
     unsigned char* st0 = smem + QMCD_TMA_STAGE_OFF;
-    double* Ts = reinterpret_cast<double*>(st0 + QMCD_TMA_NS * QMCD_TMA_STAGE_BYTES);
     const unsigned it0 = itc;
     double* Bw = P.B + (size_t)b * N * N;
-    const int* Jw = P.J + (size_t)b * P.K;
 
-    auto issue = [&](int j) {                     // thread 0: the loads of iteration j of this tile
-        const unsigned gi = it0 + (unsigned)j, s = gi % QMCD_TMA_NS, u = gi / QMCD_TMA_NS;
-        if (u > 0) qmcd_mbar_wait(bar0 + 8 * QMCD_TMA_NS + 8 * s, (u - 1) & 1);      // every warp has left the stage
+    auto issue = [&](int j) {                     // one thread: the loads of iteration j of this tile
+        const unsigned gi = it0 + (unsigned)j, s = gi % NS, u = gi / NS;
+        if (u > 0) qmcd_mbar_wait(bar0 + 8 * NS + 8 * s, (u - 1) & 1);               // every warp has left the stage
         const unsigned dst = qmcd_su32(st0 + s * QMCD_TMA_STAGE_BYTES), fb = bar0 + 8 * s;
         if (j < nk) {
             qmcd_mbar_expect_tx(fb, TX_ROWS);
@@ -100,158 +100,168 @@ __device__ __noinline__ void qmcd_flush_tile_tma(const QmcdDev& P, const QmcdTma
             qmcd_tma_load4(dst + 32768, &TM.W, 0, 0, 2 * jj, b, fb);
         }
     };
-    if (tid == 0) { issue(0); issue(1); }
+    if (tid == 0) {
+#pragma unroll
+        for (int j = 0; j < NS - 1; ++j) issue(j);            // total >= 2 * 4 + 1 > NS - 1
+    }
 
-    double acc[2][NB][2];
+    // T for this warp's 16 rows: T[a][q][e] = T[row 16 wid + 8 a + g][column 8 q + 2 c + e]
+    double T[2][NB][2];
 #pragma unroll
     for (int a = 0; a < 2; ++a)
 #pragma unroll
-        for (int bt = 0; bt < NB; ++bt) { acc[a][bt][0] = 0.0; acc[a][bt][1] = 0.0; }
-    const double* Trow = Ts + (size_t)(wid * 16 + g) * QMCD_TMA_LDT + 2 * c;     // + a * 8 * LDT + 8 q
+        for (int q = 0; q < NB; ++q) { T[a][q][0] = 0.0; T[a][q][1] = 0.0; }
 
-    for (int j = 0; j < total; ++j) {
-        const unsigned gi = it0 + (unsigned)j, s = gi % QMCD_TMA_NS, u = gi / QMCD_TMA_NS;
+    // ---------------- NT: T = B0[tile,:] C^T, 4 k-groups of 8 columns per iteration
+    for (int j = 0; j < nk; ++j) {
+        const unsigned gi = it0 + (unsigned)j, s = gi % NS, u = gi / NS;
         const unsigned char* stg = st0 + s * QMCD_TMA_STAGE_BYTES;
         qmcd_mbar_wait(bar0 + 8 * s, u & 1);
-        if (j < nk) {
-            // ---- NT: 4 k-groups of 8 columns; fragments are 16-byte vectors (k = 8q + 2c + s on both operands)
-            const double* As = reinterpret_cast<const double*>(stg) + (wid * 16 + g) * 8 + 2 * c;
-            const double* Cs = reinterpret_cast<const double*>(stg + 32768) + g * 8 + 2 * c;
+        if (wid == (j & 7) && lane == 0) issue(j + NS - 1);                          // (j + NS - 1 < total always here)
+        const double* As = reinterpret_cast<const double*>(stg) + (wid * 16 + g) * 8 + 2 * c;
+        const double* Cs = reinterpret_cast<const double*>(stg + 32768) + g * 8 + 2 * c;
+        double2 av[2][2], bv[2][NB];
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                if (q == 2 && tid == 0 && j + 2 < total) issue(j + 2);
-                double2 av[2], bv[NB];
+        for (int a = 0; a < 2; ++a) av[0][a] = qmcd_lds128(As + a * 64);
 #pragma unroll
-                for (int a = 0; a < 2; ++a) av[a] = qmcd_lds128(As + q * (QMCD_TMA_ROWS * 8) + a * 64);
+        for (int bt = 0; bt < NB; ++bt) bv[0][bt] = qmcd_lds128(Cs + bt * 64);
 #pragma unroll
-                for (int bt = 0; bt < NB; ++bt) bv[bt] = qmcd_lds128(Cs + q * (64 * NB) + bt * 64);
+        for (int q = 0; q < 4; ++q) {
+            const int cur = q & 1, nxt = cur ^ 1;
+            if (q < 3) {
 #pragma unroll
-                for (int bt = 0; bt < NB; ++bt)
-                    if (bt < nqm) {
+                for (int a = 0; a < 2; ++a) av[nxt][a] = qmcd_lds128(As + (q + 1) * (QMCD_TMA_ROWS * 8) + a * 64);
 #pragma unroll
-                        for (int a = 0; a < 2; ++a) qmcd_dmma(acc[a][bt][0], acc[a][bt][1], av[a].x, bv[bt].x);
-                    }
-#pragma unroll
-                for (int bt = 0; bt < NB; ++bt)
-                    if (bt < nqm) {
-#pragma unroll
-                        for (int a = 0; a < 2; ++a) qmcd_dmma(acc[a][bt][0], acc[a][bt][1], av[a].y, bv[bt].y);
-                    }
+                for (int bt = 0; bt < NB; ++bt) bv[nxt][bt] = qmcd_lds128(Cs + (q + 1) * (64 * NB) + bt * 64);
             }
-        } else if (j == nk) {
-            if (tid == 0 && j + 2 < total) issue(j + 2);
-            // ---- T = -(B0 C^T) + E_J for this warp's 16 rows, then T <- T M (warp-local)
-            double* Tw = Ts + (size_t)(wid * 16 + g) * QMCD_TMA_LDT + 2 * c;
 #pragma unroll
-            for (int a = 0; a < 2; ++a)
+            for (int bt = 0; bt < NB; ++bt)
 #pragma unroll
-                for (int bt = 0; bt < NB; ++bt)
-                    if (bt < nqm)
-                        *reinterpret_cast<double2*>(Tw + a * 8 * QMCD_TMA_LDT + bt * 8) = make_double2(-acc[a][bt][0], -acc[a][bt][1]);
-            __syncwarp();
-            for (int i = lane; i < m; i += 32) {
-                const int r = __ldcg(Jw + i) - row0 - wid * 16;
-                if (r >= 0 && r < 16) Ts[(size_t)(wid * 16 + r) * QMCD_TMA_LDT + i] += 1.0;
+                for (int a = 0; a < 2; ++a) qmcd_dmma(T[a][bt][0], T[a][bt][1], av[cur][a].x, bv[cur][bt].x);
+#pragma unroll
+            for (int bt = 0; bt < NB; ++bt)
+#pragma unroll
+                for (int a = 0; a < 2; ++a) qmcd_dmma(T[a][bt][0], T[a][bt][1], av[cur][a].y, bv[cur][bt].y);
+        }
+        __syncwarp();
+        if (lane == 0) qmcd_mbar_arrive(bar0 + 8 * NS + 8 * s);                      // this warp has left stage s
+    }
+
+    // ---------------- T = -T + E_J ;  T <- T M   (iteration nk: the stage holds M)
+    {
+        const int j = nk;
+        const unsigned gi = it0 + (unsigned)j, s = gi % NS, u = gi / NS;
+        const unsigned char* stg = st0 + s * QMCD_TMA_STAGE_BYTES;
+        const int* Jw = P.J + (size_t)b * P.K;
+#pragma unroll
+        for (int q = 0; q < NB; ++q)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int i = 8 * q + 2 * c + e;
+                const int jr = (i < m) ? __ldcg(Jw + i) - row0 - wid * 16 - g : -1;      // E_J[j_i, i] = 1
+#pragma unroll
+                for (int a = 0; a < 2; ++a) T[a][q][e] = ((jr == 8 * a) ? 1.0 : 0.0) - T[a][q][e];
             }
-            __syncwarp();
-            double a2[2][NG][2][2];
+        qmcd_mbar_wait(bar0 + 8 * s, u & 1);
+        if (wid == (j & 7) && lane == 0) issue(j + NS - 1);
+        double T2[2][NB][2];
 #pragma unroll
-            for (int a = 0; a < 2; ++a)
+        for (int a = 0; a < 2; ++a)
 #pragma unroll
-                for (int G = 0; G < NG; ++G) { a2[a][G][0][0] = a2[a][G][0][1] = a2[a][G][1][0] = a2[a][G][1][1] = 0.0; }
-            const unsigned char* Ms = stg + (2 * c) * 128;          // row k = 8q + 2c (+1), chunk g ^ (k % 8)
-            const int sw0 = (g ^ (2 * c)) << 4, sw1 = (g ^ (2 * c + 1)) << 4;
+            for (int t = 0; t < NB; ++t) { T2[a][t][0] = 0.0; T2[a][t][1] = 0.0; }
+        // M[k][n] at group (n / 16): row k, 16-byte chunk ((n % 16) / 2) ^ (k % 8), half n % 2;  k = 8q + 2c + s, n = 8t + g
+        const unsigned char* Ms = stg + (2 * c) * 128 + (g & 1) * 8;
+        const int ch0 = (g >> 1) ^ (2 * c), ch1 = (g >> 1) ^ (2 * c + 1);            // chunk of n-tile parity 0; parity 1: ^ 4
 #pragma unroll
-            for (int q = 0; q < NB; ++q) {
-                if (q < nqm) {
-                    double2 av[2];
+        for (int q = 0; q < NB; ++q) {
+            double b0[NB], b1[NB];
 #pragma unroll
-                    for (int a = 0; a < 2; ++a) av[a] = qmcd_lds128(Trow + a * 8 * QMCD_TMA_LDT + 8 * q);
-#pragma unroll
-                    for (int G = 0; G < NG; ++G) {
-                        if (G < nG) {
-                            const double2 x0 = *reinterpret_cast<const double2*>(Ms + G * 8192 + q * 1024 + sw0);
-                            const double2 x1 = *reinterpret_cast<const double2*>(Ms + G * 8192 + q * 1024 + 128 + sw1);
-#pragma unroll
-                            for (int a = 0; a < 2; ++a) {
-                                qmcd_dmma(a2[a][G][0][0], a2[a][G][0][1], av[a].x, x0.x);
-                                qmcd_dmma(a2[a][G][1][0], a2[a][G][1][1], av[a].x, x0.y);
-                                qmcd_dmma(a2[a][G][0][0], a2[a][G][0][1], av[a].y, x1.x);
-                                qmcd_dmma(a2[a][G][1][0], a2[a][G][1][1], av[a].y, x1.y);
-                            }
-                        }
-                    }
-                }
+            for (int t = 0; t < NB; ++t) {
+                const unsigned char* pm = Ms + (t >> 1) * 8192 + q * 1024;
+                b0[t] = *reinterpret_cast<const double*>(pm + ((ch0 ^ ((t & 1) << 2)) << 4));
+                b1[t] = *reinterpret_cast<const double*>(pm + 128 + ((ch1 ^ ((t & 1) << 2)) << 4));
             }
-            __syncwarp();                                // every lane has read this warp's rows of T
-            double* To = Ts + (size_t)(wid * 16 + g) * QMCD_TMA_LDT + 4 * c;
 #pragma unroll
-            for (int a = 0; a < 2; ++a)
+            for (int t = 0; t < NB; ++t)
 #pragma unroll
-                for (int G = 0; G < NG; ++G)
-                    if (G < nG) {                        // columns 16 G + 4 c .. + 3 (n-slot x of tile t is column 16 G + 2 x + t)
-                        *reinterpret_cast<double2*>(To + a * 8 * QMCD_TMA_LDT + 16 * G) = make_double2(a2[a][G][0][0], a2[a][G][1][0]);
-                        *reinterpret_cast<double2*>(To + a * 8 * QMCD_TMA_LDT + 16 * G + 2) = make_double2(a2[a][G][0][1], a2[a][G][1][1]);
-                    }
-            __syncwarp();
-        } else {
-            // ---- NN: B[tile, 32 columns] += T W[:, same]; initial values from the staged tile, results by STG
-            const int n0 = 32 * (j - nk - 1);
-            const double* Ds = reinterpret_cast<const double*>(stg);                 // [4 groups of 8 columns][128 rows][8]
-            const unsigned char* Ws = stg + 32768 + (2 * c) * 128;                    // [2 groups of 16 columns][8 NB rows][128 B]
-            const int sw0 = (g ^ (2 * c)) << 4, sw1 = (g ^ (2 * c + 1)) << 4;
-            double an[2][2][2][2];
+                for (int a = 0; a < 2; ++a) qmcd_dmma(T2[a][t][0], T2[a][t][1], T[a][q][0], b0[t]);
 #pragma unroll
-            for (int a = 0; a < 2; ++a)
+            for (int t = 0; t < NB; ++t)
 #pragma unroll
-                for (int G = 0; G < 2; ++G) {          // this lane's columns 16 G + 4 c .. + 3 of rows 16 wid + 8 a + g
-                    const double* p = Ds + ((2 * G + (c >> 1)) * QMCD_TMA_ROWS + wid * 16 + a * 8 + g) * 8 + 4 * (c & 1);
-                    const double2 v0 = qmcd_lds128(p), v1 = qmcd_lds128(p + 2);
-                    an[a][G][0][0] = v0.x; an[a][G][1][0] = v0.y; an[a][G][0][1] = v1.x; an[a][G][1][1] = v1.y;
-                }
+                for (int a = 0; a < 2; ++a) qmcd_dmma(T2[a][t][0], T2[a][t][1], T[a][q][1], b1[t]);
+        }
 #pragma unroll
-            for (int q = 0; q < NB; ++q) {
-                if (q == (nqm >> 1) && tid == 0 && j + 2 < total) issue(j + 2);
-                if (q < nqm) {
-                    double2 av[2], x0[2], x1[2];
+        for (int a = 0; a < 2; ++a)
 #pragma unroll
-                    for (int a = 0; a < 2; ++a) av[a] = qmcd_lds128(Trow + a * 8 * QMCD_TMA_LDT + 8 * q);
+            for (int t = 0; t < NB; ++t) { T[a][t][0] = T2[a][t][0]; T[a][t][1] = T2[a][t][1]; }
+        __syncwarp();
+        if (lane == 0) qmcd_mbar_arrive(bar0 + 8 * NS + 8 * s);
+    }
+
+    // ---------------- NN: B[tile, 32 columns] += T W[:, same]; initial values from the staged tile, results by STG
+    const int sw0 = (g ^ (2 * c)) << 4, sw1 = (g ^ (2 * c + 1)) << 4;
+    for (int j = nk + 1; j < total; ++j) {
+        const unsigned gi = it0 + (unsigned)j, s = gi % NS, u = gi / NS;
+        const unsigned char* stg = st0 + s * QMCD_TMA_STAGE_BYTES;
+        const int n0 = 32 * (j - nk - 1);
+        qmcd_mbar_wait(bar0 + 8 * s, u & 1);
+        if (wid == (j & 7) && lane == 0 && j + NS - 1 < total) issue(j + NS - 1);
+        const double* Ds = reinterpret_cast<const double*>(stg);                     // [4 groups of 8 columns][128 rows][8]
+        const unsigned char* Ws = stg + 32768 + (2 * c) * 128;                        // [2 groups of 16 columns][8 NB rows][128 B]
+        double an[2][2][2][2];                                                       // [a][G][t][e]
 #pragma unroll
-                    for (int G = 0; G < 2; ++G) {
-                        x0[G] = *reinterpret_cast<const double2*>(Ws + G * (1024 * NB) + q * 1024 + sw0);
-                        x1[G] = *reinterpret_cast<const double2*>(Ws + G * (1024 * NB) + q * 1024 + 128 + sw1);
-                    }
+        for (int a = 0; a < 2; ++a)
 #pragma unroll
-                    for (int G = 0; G < 2; ++G)
+            for (int G = 0; G < 2; ++G) {              // this lane's columns 16 G + 4 c .. + 3 of row 16 wid + 8 a + g
+                const double* p = Ds + ((2 * G + (c >> 1)) * QMCD_TMA_ROWS + wid * 16 + a * 8 + g) * 8 + 4 * (c & 1);
+                const double2 v0 = qmcd_lds128(p), v1 = qmcd_lds128(p + 2);
+                an[a][G][0][0] = v0.x; an[a][G][1][0] = v0.y; an[a][G][0][1] = v1.x; an[a][G][1][1] = v1.y;
+            }
+        double2 x0[2][2], x1[2][2];                                                  // [buffer][G]
 #pragma unroll
-                        for (int a = 0; a < 2; ++a) {
-                            qmcd_dmma(an[a][G][0][0], an[a][G][0][1], av[a].x, x0[G].x);
-                            qmcd_dmma(an[a][G][1][0], an[a][G][1][1], av[a].x, x0[G].y);
-                        }
+        for (int G = 0; G < 2; ++G) {
+            x0[0][G] = *reinterpret_cast<const double2*>(Ws + G * (1024 * NB) + sw0);
+            x1[0][G] = *reinterpret_cast<const double2*>(Ws + G * (1024 * NB) + 128 + sw1);
+        }
 #pragma unroll
-                    for (int G = 0; G < 2; ++G)
+        for (int q = 0; q < NB; ++q) {
+            const int cur = q & 1, nxt = cur ^ 1;
+            if (q + 1 < NB) {
 #pragma unroll
-                        for (int a = 0; a < 2; ++a) {
-                            qmcd_dmma(an[a][G][0][0], an[a][G][0][1], av[a].y, x1[G].x);
-                            qmcd_dmma(an[a][G][1][0], an[a][G][1][1], av[a].y, x1[G].y);
-                        }
+                for (int G = 0; G < 2; ++G) {
+                    x0[nxt][G] = *reinterpret_cast<const double2*>(Ws + G * (1024 * NB) + (q + 1) * 1024 + sw0);
+                    x1[nxt][G] = *reinterpret_cast<const double2*>(Ws + G * (1024 * NB) + (q + 1) * 1024 + 128 + sw1);
                 }
             }
 #pragma unroll
-            for (int a = 0; a < 2; ++a) {
-                const int row = row0 + wid * 16 + a * 8 + g;
-                if (row < N) {
-                    double* d = Bw + (size_t)row * N + n0 + 4 * c;
+            for (int G = 0; G < 2; ++G)
 #pragma unroll
-                    for (int G = 0; G < 2; ++G) {
-                        qmcd_stg128(d + 16 * G, an[a][G][0][0], an[a][G][1][0]);
-                        qmcd_stg128(d + 16 * G + 2, an[a][G][0][1], an[a][G][1][1]);
-                    }
+                for (int a = 0; a < 2; ++a) {
+                    qmcd_dmma(an[a][G][0][0], an[a][G][0][1], T[a][q][0], x0[cur][G].x);
+                    qmcd_dmma(an[a][G][1][0], an[a][G][1][1], T[a][q][0], x0[cur][G].y);
+                }
+#pragma unroll
+            for (int G = 0; G < 2; ++G)
+#pragma unroll
+                for (int a = 0; a < 2; ++a) {
+                    qmcd_dmma(an[a][G][0][0], an[a][G][0][1], T[a][q][1], x1[cur][G].x);
+                    qmcd_dmma(an[a][G][1][0], an[a][G][1][1], T[a][q][1], x1[cur][G].y);
+                }
+        }
+        __syncwarp();
+        if (lane == 0) qmcd_mbar_arrive(bar0 + 8 * NS + 8 * s);                      // every read of stage s is done
+#pragma unroll
+        for (int a = 0; a < 2; ++a) {
+            const int row = row0 + wid * 16 + a * 8 + g;
+            if (row < N) {
+                double* d = Bw + (size_t)row * N + n0 + 4 * c;
+#pragma unroll
+                for (int G = 0; G < 2; ++G) {
+                    qmcd_stg128(d + 16 * G, an[a][G][0][0], an[a][G][1][0]);
+                    qmcd_stg128(d + 16 * G + 2, an[a][G][0][1], an[a][G][1][1]);
                 }
             }
         }
-        __syncwarp();
-        if (lane == 0) qmcd_mbar_arrive(bar0 + 8 * QMCD_TMA_NS + 8 * s);       // this warp has left stage s
     }
     itc = it0 + (unsigned)total;
 }
