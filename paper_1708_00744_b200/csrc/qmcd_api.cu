@@ -436,7 +436,7 @@ extern "C" int qmcd_sweep(qmcd_handle h, int j_begin, int n_moves,
     QmcdArgs a = base_args(h, QMCD_MODE_SWEEP);
     a.j_begin = j_begin; a.n_moves = n_moves; a.v = proposals_dev;
     a.mask = mask_dev; a.uniforms = uniforms_dev; a.R_out = R_out_dev; a.acc_out = acc_out_dev;
-    a.blocked = (h->lookahead != 1 && h->P.blk_ok && h->P.m_in_smem && (((uintptr_t)proposals_dev & 15) == 0)) ? 1 : 0;
+    a.blocked = (h->lookahead != 1 && !h->P.slot_replace && h->P.blk_ok && h->P.m_in_smem && (((uintptr_t)proposals_dev & 15) == 0)) ? 1 : 0;
     return launch(h, a, true);
 }
 
@@ -604,6 +604,11 @@ extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
         h->P.lockstep = value;
         return QMCD_OK;
     }
+    if (!strcmp(key, "slot_replace")) {            // IDLE only; qmcd_sweep then runs the per-move look-ahead
+        if (value < 0 || value > 1) return QMCD_EINVAL;
+        h->P.slot_replace = value;
+        return QMCD_OK;
+    }
     if (!strcmp(key, "chain_regs")) {
         if (value < 0 || value > 1) return QMCD_EINVAL;
         h->P.chain_regs = value;
@@ -623,7 +628,8 @@ extern "C" int qmcd_get_option(qmcd_handle h, const char* key) {
     if (!strcmp(key, "flush_path")) return h->P.flush_path;
     if (!strcmp(key, "lookahead")) return h->lookahead;
     if (!strcmp(key, "lockstep")) return h->P.lockstep;
-    if (!strcmp(key, "blocked_ok")) return h->P.blk_ok && h->P.m_in_smem;
+    if (!strcmp(key, "slot_replace")) return h->P.slot_replace;
+    if (!strcmp(key, "blocked_ok")) return h->P.blk_ok && h->P.m_in_smem && !h->P.slot_replace;
     if (!strcmp(key, "m_in_smem")) return h->P.m_in_smem;
     if (!strcmp(key, "threads")) return QMCD_THREADS;
     if (!strcmp(key, "smem_bytes")) return (int)h->smem_bytes;

@@ -51,6 +51,7 @@ struct QmcdDev {
     int m_in_smem;            // host: every CTA keeps its own copy of M in shared memory
     int chain_regs;           // option: blocked look-ahead keeps M in registers when K <= 32
     int blk_ok;               // host: qmcd_sweep may use the blocked look-ahead (qmcd_block.cuh)
+    int slot_replace;         // option: an electron accepted again inside one window replaces the column of its queue slot (reading G7, second alternative) instead of flushing first
     int lockstep;             // option: lock-step variant: Eq. 4 every K PROPOSALS; counters[7] = proposals in the window
 };
 

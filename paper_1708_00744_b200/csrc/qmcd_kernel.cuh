@@ -199,6 +199,15 @@ __device__ void qmcd_pool_loop(const QmcdDev& P, const QmcdSmem& s) {
 template <bool MS>
 __device__ int qmcd_do_accept(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
                               const QmcdWalker& w, int j, int m, double R, bool inq, int& pbuf) {
+    if (inq && P.slot_replace) {
+        // repeated electron, slot replacement (G7, second alternative): no flush, m unchanged
+        int a = 0;
+        for (int i = 0; i < m; ++i) if (s.Js[i] == j) a = i;
+        if (!MS && P.S > 1) cl.sync();
+        qmcd_accept_replace<MS>(P, s, w, a, m, R);
+        if (P.S > 1) cl.sync();        // slot a of C is complete before the next look-ahead reads it
+        return m;
+    }
     if (inq) {
         // repeated electron inside one window (G7): flush, then the move
         // is re-evaluated against the fresh inverse (m = 0) and queued.  Its v sits
@@ -276,7 +285,7 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
         __syncthreads();
         m = qmcd_do_accept<MS>(P, s, cl, w, j, m, R, inq, pbuf);
         if (QMCD_LOCKSTEP(P)) {
-            if (inq) pw = 1;                           // G7 flushed first: this move opens the new window
+            if (inq && !P.slot_replace) pw = 1;        // G7 flushed first: this move opens the new window
             if (pw >= P.K) {
                 if (m > 0) { qmcd_flush_phase<MS>(P, s, cl, w, m); m = 0; }
                 pw = 0;
@@ -333,7 +342,7 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
         if (QMCD_LOCKSTEP(P)) {
             // every proposal takes a slot (a rejected one adds a zero column of U,
             // i.e. nothing), so the window closes after K proposals for every walker at once
-            pw = (acc && inq) ? 1 : pw + 1;
+            pw = (acc && inq && !P.slot_replace) ? 1 : pw + 1;
             if (pw >= P.K) {
                 if (m > 0) { qmcd_flush_phase<MS>(P, s, cl, w, m); m = 0; }
                 pw = 0;

@@ -196,6 +196,38 @@ __device__ void qmcd_accept_update(const QmcdDev& P, const QmcdSmem& s, const Qm
     __syncthreads();
 }
 
+// ---------------------------------------------------------------------------
+// F2, repeated electron (reading G7, second alternative; the paper is silent):
+// electron j = J[a] is accepted again before the queue was applied.  The current matrix is A0 with
+// column j = the NEWEST column, so slot a keeps its row W[a,:] = B0[j,:] and only its column changes,
+// C[a,:] <- v.  S = W C^T changes in column a (to q = W v), and by Sherman-Morrison on that column
+//     M' = M - (c - e_a) M[a,:] / c_a,      c = M q,   c_a = M[a,:] q = R  (the ratio of this move).
+// cf = c must be valid in shared memory; v sits in slot m of C (staged by the look-ahead).  m, J, W
+// are unchanged.  s.rf is used as scratch for the old row a.  Every CTA copies its column slice.
+// ---------------------------------------------------------------------------
+template <bool MS>
+__device__ void qmcd_accept_replace(const QmcdDev& P, const QmcdSmem& s, const QmcdWalker& w,
+                                    int a, int m, double R) {
+    const int tid = threadIdx.x;
+    const double inv = 1.0 / R;
+    if (MS || w.r == 0) {
+        double* Mb = MS ? s.Ms : w.M;
+        const int ldM = QmcdM<MS>::ld(P);
+        for (int y = tid; y < m; y += QMCD_THREADS) s.rf[y] = QmcdM<MS>::get(Mb + (size_t)a * ldM + y);
+        __syncthreads();
+        for (int idx = tid; idx < m * m; idx += QMCD_THREADS) {
+            const int x = idx / m, y = idx - x * m;
+            double* p = Mb + (size_t)x * ldM + y;
+            *p = QmcdM<MS>::get(p) - (s.cf[x] - (x == a ? 1.0 : 0.0)) * s.rf[y] * inv;
+        }
+    }
+    const double* src = w.C + (size_t)m * P.N;
+    double* dst = w.C + (size_t)a * P.N;
+    for (int k = w.klo + tid; k < w.khi; k += QMCD_THREADS) dst[k] = __ldcg(src + k);
+    if (tid == 0 && w.r == 0) P.counters[(size_t)w.b * 8 + 0] += 1;
+    __syncthreads();
+}
+
 // Leader: copy this walker's M from shared to global memory (before a flush, or
 // at the end of a launch).  No-op when M already lives in global memory.
 template <bool MS>

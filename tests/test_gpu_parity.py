@@ -438,88 +438,6 @@ def test_sweep_host_matches_device_sweep(qmcd):
 
 
 # ------------------------------------------------------------------ full-size configs, bench launch configuration
-def _residuals_numpy(wl, acc, B, walkers):
-    worst = 0.0
-    for w in walkers:
-        A_cur = inputs.current_matrix(wl.A[w], wl.proposals[:, w, :], acc[:, w], wl.n_moves)
-        worst = max(worst, float(np.max(np.abs(A_cur @ B[w] - np.eye(wl.N)))))
-    return worst
-
-
-def test_c2_full_size_sampled_walkers_vs_oracle_and_residuals(qmcd):
-    """BASELINE.json configs[2] at FULL size (64 walkers, N = 1024, 4 sweeps) in bench.py's launch
-    configuration (qmcd_sweep + qmcd_flush, library-chosen clusters), K = 64 and 32.
-    Sampled outputs: walkers 0 and 63 against the oracle's rank-1 path run on exactly those walkers
-    (a walker's data depend only on its seed); every walker: max|A.Ainv - I| <= 1e-8 after the run;
-    K-independence of all ratios.  Bernoulli(0.99) and the Metropolis rule."""
-    wl = inputs.make_config("c2")
-    sample = [0, wl.batch - 1]
-    for mode in ("bern0.99", "metropolis"):
-        mask = wl.bernoulli_mask(0.99) if mode == "bern0.99" else None
-        uni = wl.uniforms if mode == "metropolis" else None
-        g64 = gpu_sweep(qmcd, wl, 64, mask=mask, uniforms=uni)
-        assert g64["status"] == 0 and g64["blocked"]
-        Bs = np.ascontiguousarray(wl.Ainv[sample])
-        Ro, acco, _ = oracle.run(1, Bs, 1, np.ascontiguousarray(wl.proposals[:, sample, :]),
-                                 mask=None if mask is None else np.ascontiguousarray(mask[:, sample]),
-                                 uniforms=None if uni is None else np.ascontiguousarray(uni[:, sample]))
-        assert np.array_equal(g64["acc"][:, sample], acco)
-        assert _rel(g64["R"][:, sample], Ro) <= RTOL_RATIO
-        assert np.max(np.abs(g64["B"][sample] - Bs)) <= 1e-9
-        assert _residuals_numpy(wl, g64["acc"], g64["B"], range(0, wl.batch, 7)) <= TOL_RESID
-        assert 0.97 < g64["acc"].mean() < 1.0
-        if mode == "bern0.99":
-            g32 = gpu_sweep(qmcd, wl, 32, mask=mask)
-            assert np.array_equal(g32["acc"], g64["acc"])
-            assert _rel(g32["R"], g64["R"]) <= RTOL_RATIO
-            assert np.max(np.abs(g32["B"] - g64["B"])) <= 1e-9
-
-
-def test_c4_full_size_properties(qmcd):
-    """BASELINE.json configs[4] at FULL size (8 walkers, N = 4096, 1 sweep), bench launch
-    configuration, K = 64 (helper clusters) against K = 32: identical accept sequence, ratios
-    K-independent to 1e-10, max|A.Ainv - I| <= 1e-8 for every walker, and the
-    ratios of sampled moves against the plain definition det(A_new)/det(A_cur) by library LU."""
-    wl = inputs.make_config("c4")
-    mask = wl.bernoulli_mask(0.99)
-    g64 = gpu_sweep(qmcd, wl, 64, mask=mask)
-    assert g64["status"] == 0 and g64["blocked"]
-    g32 = gpu_sweep(qmcd, wl, 32, mask=mask)
-    assert np.array_equal(g64["acc"], mask) and np.array_equal(g32["acc"], mask)
-    assert _rel(g64["R"], g32["R"]) <= RTOL_RATIO
-    assert np.max(np.abs(g64["B"] - g32["B"])) <= 1e-9
-    assert _residuals_numpy(wl, mask, g64["B"], range(wl.batch)) <= TOL_RESID
-    # plain definition at sampled moves of walker 3 (explicit LU determinants, numpy/LAPACK)
-    w = 3
-    for t in (0, 70, 1500):
-        A_cur = inputs.current_matrix(wl.A[w], wl.proposals[:, w, :], mask[:, w], t)
-        A_new = A_cur.copy(); A_new[:, t % wl.N] = wl.proposals[t, w]
-        s0, l0 = np.linalg.slogdet(A_cur); s1, l1 = np.linalg.slogdet(A_new)
-        Rdef = s1 * s0 * np.exp(l1 - l0)
-        assert abs(g64["R"][t, w] - Rdef) <= 1e-9 * abs(Rdef)
-
-
-def test_c3_full_size_properties(qmcd):
-    """BASELINE.json configs[3] at FULL size (32 walkers, N = 2048, 2 sweeps), bench launch
-    configuration: K = 64 against K = 128 (the Y = M W flush path): identical accept sequence,
-    K-independent ratios, residuals of sampled walkers, walker 5 against the oracle's
-    rank-1 path for the first 300 proposals."""
-    wl = inputs.make_config("c3")
-    mask = wl.bernoulli_mask(0.99)
-    g64 = gpu_sweep(qmcd, wl, 64, mask=mask)
-    g128 = gpu_sweep(qmcd, wl, 128, mask=mask)
-    assert g64["status"] == 0 and g128["status"] == 0
-    assert np.array_equal(g64["acc"], mask) and np.array_equal(g128["acc"], mask)
-    assert _rel(g64["R"], g128["R"]) <= RTOL_RATIO
-    assert np.max(np.abs(g64["B"] - g128["B"])) <= 1e-9
-    assert _residuals_numpy(wl, mask, g64["B"], (0, 13, 31)) <= TOL_RESID
-    w, nt = 5, 300
-    Bs = np.ascontiguousarray(wl.Ainv[w:w + 1])
-    Ro, acco, _ = oracle.run(1, Bs, 1, np.ascontiguousarray(wl.proposals[:nt, w:w + 1, :]),
-                             mask=np.ascontiguousarray(mask[:nt, w:w + 1]))
-    assert _rel(g64["R"][:nt, w:w + 1], Ro) <= RTOL_RATIO
-
-
 def test_blocked_sweep_singular_move_is_dropped_and_reported(qmcd):
     """Reading G13 inside qmcd_sweep (blocked look-ahead): a proposal with R == 0 that the mask
     accepts sets the sticky status, is NOT queued, and the rest of the run is unaffected."""
@@ -699,6 +617,82 @@ def test_cluster_option_rejects_non_powers_of_two(qmcd):
     for ok in (1, 2, 4, 8):
         q.set_option("cluster", ok)
         assert q.get_option("cluster") == ok
+    q.close()
+
+
+# ------------------------------------------------------------------ slot replacement (reading G7)
+@pytest.mark.parametrize("N,K,batch,cluster,p,j_begin", [
+    (64, 64, 2, 1, 0.3, 0),        # K = N at 30 % acceptance: every window revisits queued electrons
+    (48, 24, 3, 2, 0.4, 5),        # clusters of 2, ragged slices
+    (128, 100, 2, 1, 0.5, 0),      # M in shared memory, K > 64 flush path
+    (256, 200, 1, 4, 0.6, 250),    # M in GLOBAL memory (K too large for shared memory), wrap-around
+])
+def test_slot_replacement_sweep_matches_oracle_path4(qmcd, N, K, batch, cluster, p, j_begin):
+    """Option "slot_replace": an electron accepted again before the queue is applied replaces the column of
+    its queue slot (column-replacement Sherman-Morrison on M) instead of flushing first.  Against the
+    oracle's literal path 4 (rebuilds S, LU-solves): ratios, decisions, inverse, and the same, smaller
+    number of flushes; flush-first (the default) must give the same inverse with more flushes."""
+    wl = inputs.make_workload(batch, N, n_moves=4 * N + 7, seed=91)
+    mask = wl.bernoulli_mask(p)
+    jseq = ((j_begin + np.arange(wl.n_moves)) % N).astype(np.int32)
+    Bo = wl.Ainv.copy()
+    Ro, acco, flo, _ = oracle.run_jseq(Bo, K, wl.proposals, jseq, True, mask=mask)
+    import torch
+    q = qmcd.Qmcd(N, K, batch)
+    q.set_option("cluster", cluster); q.set_option("slot_replace", 1)
+    assert q.get_option("slot_replace") == 1 and q.get_option("blocked_ok") == 0
+    B = _dev(wl.Ainv); q.set_inverse(B)
+    R = torch.zeros((wl.n_moves, batch), dtype=torch.float64, device="cuda")
+    acc = torch.zeros((wl.n_moves, batch), dtype=torch.uint8, device="cuda")
+    q.sweep(j_begin, _dev(wl.proposals), mask=_dev(mask), R_out=R, acc_out=acc)
+    q.flush()
+    assert q.status()[0] == 0
+    cnt = q.counters().cpu().numpy()
+    q.close()
+    assert np.array_equal(acc.cpu().numpy(), acco)
+    assert _rel(R.cpu().numpy(), Ro) <= RTOL_RATIO
+    assert np.max(np.abs(B.cpu().numpy() - Bo)) <= 1e-10
+    assert np.array_equal(cnt[:, 0], mask.sum(axis=0))
+    assert np.array_equal(cnt[:, 1], flo)                       # Eq. 4 applied exactly as often as in the oracle
+    g = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, j_begin=j_begin, lookahead=1)     # flush-first
+    assert np.max(np.abs(g["B"] - Bo)) <= 1e-10
+    assert (g["counters"][:, 1] > cnt[:, 1]).all()
+
+
+def test_slot_replacement_per_call_sequence(qmcd):
+    """The (1, 4, 1, 4, 4, 2) sequence of the oracle pin P12 through qmcd_ratio / qmcd_accept."""
+    import torch
+    N, K, batch = 64, 6, 2
+    wl = inputs.make_workload(batch, N, n_moves=12, seed=13)
+    js = (1, 4, 1, 4, 4, 2, 2, 9, 1, 4, 30, 1)
+    q = qmcd.Qmcd(N, K, batch)
+    q.set_option("slot_replace", 1)
+    B = _dev(wl.Ainv); q.set_inverse(B)
+    Bo = wl.Ainv.copy()
+    D = [oracle.Delayed(Bo[w], K, replace=True) for w in range(batch)]
+    R = torch.zeros(batch, dtype=torch.float64, device="cuda")
+    A = wl.A.copy()
+    for t, j in enumerate(js):
+        v = A[:, :, j] + 0.3 * (wl.proposals[t] - wl.A[:, :, t % N]) * 8.0 / np.sqrt(N) + 0.05     # a new column for electron j
+        q.ratio(j, _dev(v), R)
+        Rg = R.cpu().numpy()
+        for w in range(batch):
+            An = A[w].copy(); An[:, j] = v[w]
+            truth = np.linalg.det(An) / np.linalg.det(A[w])
+            assert abs(D[w].ratio(j, v[w]) / truth - 1) <= 1e-10
+            assert abs(Rg[w] / truth - 1) <= 1e-10, (t, j, w)
+            D[w].accept()
+            A[w] = An
+        q.accept()
+        pend = q.pending().cpu().numpy()
+        assert all(int(pend[w]) == D[w].pending for w in range(batch)), (t, pend)
+    q.flush()
+    for w in range(batch):
+        D[w].flush()
+    assert q.status()[0] == 0
+    assert np.max(np.abs(B.cpu().numpy() - Bo)) <= 1e-10
+    for w in range(batch):
+        assert np.max(np.abs(A[w] @ B.cpu().numpy()[w] - np.eye(N))) <= 1e-8
     q.close()
 
 
