@@ -28,7 +28,9 @@ struct qmcd_ctx {
     int coop;                 // option "cooperative": pooled launches ask the driver for co-residency
     QmcdTmaps tmaps;          // 4-D tensor maps of B, C, W, M for the TMA-fed flush (B re-encoded by set_inverse)
     int tma_opt;              // option "tma": 1 = use the TMA-fed flush when the shape allows
-    bool tmaps_ok;            // C, W, M encoded
+    bool tmaps_ok;            // C, W, M, Wk encoded (and B, B16 once an inverse is adopted)
+    int la_opt;               // option "la_tma": 1 = TMA-ring look-ahead in qmcd_sweep when the shape allows
+    bool la_fit;              // the kernel's shared memory was sized with the look-ahead ring
     size_t ctl_off, ctl_bytes;    // job words inside the workspace (zeroed before every pooled launch)
     unsigned char* ws;
     char last_cuda_error[256];
@@ -94,18 +96,29 @@ static qmcd_encode_fn get_encode_fn() {
     }
     return fn;
 }
+static bool encode_4d(CUtensorMap* tm, const void* base, const cuuint64_t gd[4], const cuuint64_t gs[3], const cuuint32_t bd[4], bool swizzle) {
+    qmcd_encode_fn enc = get_encode_fn();
+    if (!enc) return false;
+    cuuint32_t es[4] = {1, 1, 1, 1};
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void*>(base), gd, gs, bd, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               swizzle ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
 // A row-major fp64 array [batch][rows][N] seen as {inner, rows, N / inner, batch}: inner = 8 without swizzle
 // (an 8 x 8 block of doubles lands as 512 contiguous bytes) or 16 with SWIZZLE_128B; box {inner, box_rows, groups, 1}.
 static bool encode_view(CUtensorMap* tm, double* base, int rows, int N, size_t batch_stride_elems, int batch,
                         int inner, int box_rows, int groups, bool swizzle) {
-    qmcd_encode_fn enc = get_encode_fn();
-    if (!enc) return false;
-    cuuint64_t gd[4] = {(cuuint64_t)inner, (cuuint64_t)rows, (cuuint64_t)(N / inner), (cuuint64_t)batch};
-    cuuint64_t gs[3] = {(cuuint64_t)N * 8, (cuuint64_t)inner * 8, (cuuint64_t)batch_stride_elems * 8};
-    cuuint32_t bd[4] = {(cuuint32_t)inner, (cuuint32_t)box_rows, (cuuint32_t)groups, 1}, es[4] = {1, 1, 1, 1};
-    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, gd, gs, bd, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-               swizzle ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    const cuuint64_t gd[4] = {(cuuint64_t)inner, (cuuint64_t)rows, (cuuint64_t)(N / inner), (cuuint64_t)batch};
+    const cuuint64_t gs[3] = {(cuuint64_t)N * 8, (cuuint64_t)inner * 8, (cuuint64_t)batch_stride_elems * 8};
+    const cuuint32_t bd[4] = {(cuuint32_t)inner, (cuuint32_t)box_rows, (cuuint32_t)groups, 1};
+    return encode_4d(tm, base, gd, gs, bd, swizzle);
+}
+// The proposals of one qmcd_sweep launch, [n_moves][batch][N], seen as {8, n_moves, N / 8, batch}: row t of walker b
+static bool encode_proposals(CUtensorMap* tm, const double* base, int n_moves, int N, int batch) {
+    const cuuint64_t gd[4] = {8, (cuuint64_t)n_moves, (cuuint64_t)(N / 8), (cuuint64_t)batch};
+    const cuuint64_t gs[3] = {(cuuint64_t)batch * N * 8, 64, (cuuint64_t)N * 8};
+    const cuuint32_t bd[4] = {8, 16, 4, 1};
+    return encode_4d(tm, base, gd, gs, bd, false);
 }
 static bool tma_shape_ok(int N, int K) { return K <= 64 && N % 64 == 0 && N >= 128; }
 static void encode_queue_tmaps(qmcd_ctx* h) {
@@ -114,22 +127,28 @@ static void encode_queue_tmaps(qmcd_ctx* h) {
     const int N = h->N, K = h->K, rows = 8 * qmcd_tma_NB(K);
     h->tmaps_ok = encode_view(&h->tmaps.C, h->P.C, K, N, (size_t)K * N, h->batch, 8, rows, 4, false) &&
                   encode_view(&h->tmaps.W, h->P.W, K, N, (size_t)K * N, h->batch, 16, rows, 2, true) &&
-                  encode_view(&h->tmaps.M, h->P.M, 64, 64, (size_t)64 * 64, h->batch, 16, 64, 4, true);
+                  encode_view(&h->tmaps.M, h->P.M, 64, 64, (size_t)64 * 64, h->batch, 16, 64, 4, true) &&
+                  encode_view(&h->tmaps.Wk, h->P.W, K, N, (size_t)K * N, h->batch, 8, rows, 4, false);
 }
 static void refresh_use_tma(qmcd_ctx* h) {
     h->P.use_tma = (h->tma_opt && h->tmaps_ok && h->P.B != nullptr && h->P.mma_smem_ok && h->P.flush_path != 1 &&
                     h->smem_bytes >= qmcd_flush_tma_smem_bytes()) ? 1 : 0;
     if (h->P.use_tma) h->P.tile_rows = QMCD_TMA_ROWS;
+    h->P.la_tma = (h->la_opt && h->la_fit && h->tmaps_ok && h->P.B != nullptr && h->P.blk_ok && h->P.m_in_smem) ? 1 : 0;
 }
 
 static int configure_kernel(qmcd_ctx* h, int S) {
     const size_t cap = 227 * 1024;
     // blocked look-ahead: 16-byte vector access to every slice, <= 40 output tiles
     const bool blk_shape = h->N >= QMCD_TB && (h->N % (8 * S) == 0) && (2 * ((h->K + 7) / 8) + 2 <= 8 * QMCD_BLK_MAXU);
-    const size_t blk = blk_shape ? qmcd_blk_smem_bytes(h->K) : 0;
+    // the TMA look-ahead ring: K <= 64 tensor maps, column slices of whole 32-column chunks
+    bool la = blk_shape && h->la_opt && tma_shape_ok(h->N, h->K) && (h->N / S) % 32 == 0 && h->N % S == 0;
+    size_t blk = blk_shape ? qmcd_blk_smem_bytes(h->K, la) : 0;
     size_t base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, blk);
+    if (la && base > cap) { la = false; blk = qmcd_blk_smem_bytes(h->K, false); base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, blk); }
+    h->la_fit = la;
     h->P.m_in_smem = 1; h->P.blk_ok = blk_shape ? 1 : 0;
-    if (base > cap) { base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, 0); h->P.blk_ok = 0; }
+    if (base > cap) { h->la_fit = false; base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, 0); h->P.blk_ok = 0; }
     if (base > cap) { base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, false, 0); h->P.m_in_smem = 0; }
     const size_t mma = QMCD_SMEM_HEADER + qmcd_flush_mma_smem_bytes(h->N, h->K);
     if (base > cap) { snprintf(g_last_error, sizeof(g_last_error), "shared memory need %zu > 227 KB", base); return QMCD_EINVAL; }
@@ -262,7 +281,7 @@ extern "C" int qmcd_create(qmcd_handle* out, int N, int K, int batch,
     P.fin = (unsigned*)(ws + L.fin); P.ctrl = (unsigned*)(ws + L.ctrl);
     P.chain_regs = 1; P.pool = 0;
     P.flush_path = 0; P.use_tma = 0; P.ldMg = qmcd_ldMg_host(K);
-    h->tma_opt = 1;
+    h->tma_opt = 1; h->la_opt = 1; h->la_fit = false;
     encode_queue_tmaps(h);
     P.tile_rows = (K <= 64 && N >= 2048) ? 128 : 64;
     int rc = QMCD_OK;
@@ -312,7 +331,8 @@ extern "C" int qmcd_set_inverse(qmcd_handle h, double* Ainv_dev) {
     if (!h || !Ainv_dev || ((uintptr_t)Ainv_dev & 15)) return QMCD_EINVAL;
     if (h->state != QMCD_IDLE) return QMCD_ESTATE;
     h->P.B = Ainv_dev;
-    if (h->tmaps_ok && !encode_view(&h->tmaps.B, Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, QMCD_TMA_ROWS, 4, false))
+    if (h->tmaps_ok && !(encode_view(&h->tmaps.B, Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, QMCD_TMA_ROWS, 4, false) &&
+                         encode_view(&h->tmaps.B16, Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 16, 4, false)))
         h->tmaps_ok = false;
     refresh_use_tma(h);
     CK(h, cudaMemsetAsync(h->P.m, 0, (size_t)h->batch * 4, h->stream));
@@ -436,6 +456,7 @@ extern "C" int qmcd_sweep(qmcd_handle h, int j_begin, int n_moves,
     QmcdArgs a = base_args(h, QMCD_MODE_SWEEP);
     a.j_begin = j_begin; a.n_moves = n_moves; a.v = proposals_dev;
     a.mask = mask_dev; a.uniforms = uniforms_dev; a.R_out = R_out_dev; a.acc_out = acc_out_dev;
+    if (h->P.la_tma && !encode_proposals(&h->tmaps.V, proposals_dev, n_moves, h->N, h->batch)) { h->la_opt = 0; refresh_use_tma(h); a.P = h->P; }
     a.blocked = (h->lookahead != 1 && !h->P.slot_replace && h->P.blk_ok && h->P.m_in_smem && (((uintptr_t)proposals_dev & 15) == 0)) ? 1 : 0;
     return launch(h, a, true);
 }
@@ -580,6 +601,12 @@ extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
         h->P.tile_rows = value;
         return QMCD_OK;
     }
+    if (!strcmp(key, "la_tma")) {                  // 0: qmcd_sweep's blocked look-ahead through LDG / cp.async instead of the TMA ring
+        if (value < 0 || value > 1) return QMCD_EINVAL;
+        CK(h, cudaStreamSynchronize(h->stream));
+        h->la_opt = value;
+        return configure_kernel(h, h->P.S);
+    }
     if (!strcmp(key, "tma")) {                     // 0: K <= 64 flush tiles through the cp.async kernels instead
         if (value < 0 || value > 1) return QMCD_EINVAL;
         h->tma_opt = value;
@@ -625,6 +652,7 @@ extern "C" int qmcd_get_option(qmcd_handle h, const char* key) {
     if (!strcmp(key, "cooperative")) return h->coop;
     if (!strcmp(key, "tile_rows")) return h->P.tile_rows;
     if (!strcmp(key, "tma")) return h->P.use_tma;
+    if (!strcmp(key, "la_tma")) return h->P.la_tma;
     if (!strcmp(key, "flush_path")) return h->P.flush_path;
     if (!strcmp(key, "lookahead")) return h->lookahead;
     if (!strcmp(key, "lockstep")) return h->P.lockstep;

@@ -24,9 +24,15 @@
 
 __host__ __device__ inline int qmcd_blk_Kp(int K) { return (K + 7) & ~7; }
 __host__ __device__ inline int qmcd_blk_RL(int K) { return 2 * qmcd_blk_Kp(K) + QMCD_TB; }
-// As[2][32][LDA] | recv[16][RL] | G[16][RL] | ub[16] | Rb[16] | Z[2][16][16] | Xm[Kp][16] | Ym[16][Kp] | Um[Kp][16]
-__host__ __device__ inline size_t qmcd_blk_smem_bytes(int K) {
-    return ((size_t)2 * 32 * QMCD_BLK_LDA + (size_t)2 * QMCD_TB * qmcd_blk_RL(K) + 32 + 2 * QMCD_TB * QMCD_TB + 3 * (size_t)QMCD_TB * qmcd_blk_Kp(K) + 8) * 8;
+// As | recv[16][RL] | G[16][RL] | ub[16] | Rb[16] | Z[2][16][16] | Xm[Kp][16] | Ym[16][Kp] | Um[Kp][16]
+// As = [2][32][LDA] (cp.async staging of the left operands) or, with the TMA look-ahead, the ring of
+// QMCD_LA_NS stages of qmcd_la_stage_bytes(K) bytes (all four operands)
+__host__ __device__ inline size_t qmcd_blk_as_doubles(int K, bool la_tma) {
+    const size_t a = (size_t)2 * 32 * QMCD_BLK_LDA, r = la_tma ? QMCD_LA_NS * qmcd_la_stage_bytes(K) / 8 : 0;
+    return r > a ? r : a;
+}
+__host__ __device__ inline size_t qmcd_blk_smem_bytes(int K, bool la_tma) {
+    return (qmcd_blk_as_doubles(K, la_tma) + (size_t)2 * QMCD_TB * qmcd_blk_RL(K) + 32 + 2 * QMCD_TB * QMCD_TB + 3 * (size_t)QMCD_TB * qmcd_blk_Kp(K) + 8) * 8;
 }
 
 struct QmcdBlk {
@@ -42,10 +48,10 @@ struct QmcdBlk {
     double* Rb;     // [16]          ratios of the block (written to R_out at the block's end)
 };
 
-__device__ inline QmcdBlk qmcd_blk_carve(double* base, int K) {
+__device__ inline QmcdBlk qmcd_blk_carve(double* base, int K, bool la_tma) {
     QmcdBlk x;
     const int RL = qmcd_blk_RL(K);
-    x.As = base; base += 2 * 32 * QMCD_BLK_LDA;
+    x.As = base; base += qmcd_blk_as_doubles(K, la_tma);
     x.recv = base; base += QMCD_TB * RL;
     x.G = base; base += QMCD_TB * RL;
     x.ub = base; base += 16;
@@ -106,6 +112,50 @@ __device__ __forceinline__ const double* qmcd_blk_right(const QmcdArgs& A, const
     if (u < 2 * nP) { const int i = (u - nP) * 8 + g; return (i < m0) ? w.W + (size_t)i * N + w.klo : nullptr; }
     const int tl = (u - 2 * nP) * 8 + g;
     return (tl < L) ? A.v + ((size_t)(t0 + tl) * A.P.batch + w.b) * N + w.klo : nullptr;
+}
+
+// Cluster-wide sum of the strips: acc[i][a] = this CTA's partial of unit wid + 8 i, row block a.
+// Reduce-scatter + all-gather through distributed shared memory; on return every CTA holds G.
+__device__ __forceinline__ void qmcd_blk_reduce(const QmcdDev& P, const QmcdBlk& x, cg::cluster_group& cl, const QmcdWalker& w,
+                                             double (&acc)[QMCD_BLK_MAXU][2][2], int nu, int nP) {
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, g = lane >> 2, c = lane & 3;
+    const int S = P.S, K = P.K, Kp = qmcd_blk_Kp(K), RL = qmcd_blk_RL(K);
+    // ---- reduce-scatter: strip row `row` is summed by CTA (row % S); every CTA
+    // sends its partial of that row to slot [my rank][row / S] of the owner's recv
+    const int RPO = (QMCD_TB + S - 1) / S;
+#pragma unroll
+    for (int i = 0; i < QMCD_BLK_MAXU; ++i) {
+        if (i < nu) {
+            const int u = wid + 8 * i;
+            const int off = (u < nP) ? u * 8 : (u < 2 * nP) ? Kp + (u - nP) * 8 : 2 * Kp + (u - 2 * nP) * 8;
+#pragma unroll
+            for (int a = 0; a < 2; ++a) {
+                const int row = a * 8 + g;
+                const int owner = row % S;
+                double* rb = (S > 1) ? cl.map_shared_rank(x.recv, owner) : x.recv;
+                *reinterpret_cast<double2*>(rb + ((size_t)w.r * RPO + row / S) * RL + off + 2 * c) =
+                    make_double2(acc[i][a][0], acc[i][a][1]);
+            }
+        }
+    }
+    if (S > 1) cl.sync(); else __syncthreads();
+    // ---- owner: sum the S partials in rank order, all-gather the result into every CTA's G
+    {
+        const int ncol = 2 * nP * 8 + QMCD_TB;            // active columns: P | Q | D
+        for (int idx = tid; idx < RPO * ncol; idx += QMCD_THREADS) {
+            const int rl = idx / ncol, ci = idx - rl * ncol;
+            const int row = rl * S + w.r;
+            if (row >= QMCD_TB) continue;
+            const int col = (ci < nP * 8) ? ci : (ci < 2 * nP * 8) ? Kp + (ci - nP * 8) : 2 * Kp + (ci - 2 * nP * 8);
+            double v = 0.0;
+            for (int r = 0; r < S; ++r) v += x.recv[((size_t)r * RPO + rl) * RL + col];
+            for (int q = 0; q < S; ++q) {
+                double* gb = (S > 1) ? cl.map_shared_rank(x.G, q) : x.G;
+                gb[(size_t)row * RL + col] = v;
+            }
+        }
+    }
+    if (S > 1) cl.sync(); else __syncthreads();
 }
 
 // ---------------------------------------------------------------------------
@@ -183,42 +233,128 @@ __device__ __noinline__ void qmcd_blk_strips(const QmcdArgs& A, const QmcdSmem& 
         __syncthreads();
     }
 
-    // ---- reduce-scatter: strip row `row` is summed by CTA (row % S); every CTA
-    // sends its partial of that row to slot [my rank][row / S] of the owner's recv
-    const int RPO = (QMCD_TB + S - 1) / S;
+    qmcd_blk_reduce(P, x, cl, w, acc, nu, nP);
+}
+
+// ---------------------------------------------------------------------------
+// The same strips with every operand streamed through a TMA ring (P.la_tma): per chunk of 32 columns of this
+// CTA's slice one stage holds  B0[j0 .. j0+15, chunk] | V[t0 .. t0+15, chunk] | C[0 .. 8NB), chunk] | W[0 .. 8NB), chunk],
+// each as [4 k-groups][rows][8] (conflict-free 16-byte fragment loads).  Thread 0 issues the loads of chunk
+// kc + 2 at the top of chunk kc; the warps only run LDS + DMMA.  The block must not wrap (j0 + L <= N: the
+// caller cuts it) so that the 16 rows of B0 are one box.  `itc` = chunks this CTA has pushed through the ring.
+// ---------------------------------------------------------------------------
+template <int NB>
+__device__ __noinline__ void qmcd_blk_strips_tma(const QmcdArgs& A, const QmcdSmem& s, const QmcdBlk& x, cg::cluster_group& cl,
+                                                 const QmcdWalker& w, int t0, int L, int m0, unsigned& itc) {
+    constexpr int NS = QMCD_LA_NS;
+    constexpr unsigned STAGE = 8192 + 4096 * NB;               // bytes
+    const QmcdDev& P = A.P;
+    const QmcdTmaps& TM = *s.tm;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, g = lane >> 2, c = lane & 3;
+    const int len = w.khi - w.klo, nch = len / 32;
+    const int nP = (m0 + 7) >> 3, U = 2 * nP + 2;
+    const int j0 = (A.j_begin + t0) % P.N;
+    unsigned char* smem = reinterpret_cast<unsigned char*>(s.red);
+    const unsigned bar0 = qmcd_su32(smem + QMCD_LA_BAR_OFF);
+    unsigned char* ring = reinterpret_cast<unsigned char*>(x.As);
+    const unsigned it0 = itc;
+    (void)L;
+    const unsigned long long pol_keep = qmcd_policy_evict_last();
+    auto issue = [&](int kc) {
+        const unsigned gi = it0 + (unsigned)kc, st = gi % NS, u = gi / NS;
+        if (u > 0) qmcd_mbar_wait(bar0 + 8 * NS + 8 * st, (u - 1) & 1);
+        const unsigned dst = qmcd_su32(ring + st * STAGE), fb = bar0 + 8 * st;
+        const int kg = (w.klo >> 3) + 4 * kc;
+        qmcd_mbar_expect_tx(fb, STAGE);
+        qmcd_tma_load4(dst, &TM.B16, 0, j0, kg, w.b, fb);
+        qmcd_tma_load4(dst + 4096, &TM.V, 0, t0, kg, w.b, fb);
+        qmcd_tma_load4_hint(dst + 8192, &TM.C, 0, 0, kg, w.b, fb, pol_keep);
+        qmcd_tma_load4_hint(dst + 8192 + 2048 * NB, &TM.Wk, 0, 0, kg, w.b, fb, pol_keep);
+    };
+    if (tid == 0) {
+        for (int kc = 0; kc < NS - 1 && kc < nch; ++kc) issue(kc);
+    }
+    // my units u = wid + 8 i: right-operand offset (doubles, within a stage, at k-group 0), its k-group stride, left operand
+    int nu = 0, roff[QMCD_BLK_MAXU], rqs[QMCD_BLK_MAXU], lsel[QMCD_BLK_MAXU];
 #pragma unroll
     for (int i = 0; i < QMCD_BLK_MAXU; ++i) {
-        if (i < nu) {
-            const int u = wid + 8 * i;
-            const int off = (u < nP) ? u * 8 : (u < 2 * nP) ? Kp + (u - nP) * 8 : 2 * Kp + (u - 2 * nP) * 8;
+        const int u = wid + 8 * i;
+        roff[i] = 0; rqs[i] = 0; lsel[i] = 0;
+        if (u < U) {
+            nu = i + 1;
+            if (u < nP) { roff[i] = 1024 + (8 * u + g) * 8 + 2 * c; rqs[i] = 64 * NB; lsel[i] = 0; }                         // P: B0 rows x C
+            else if (u < 2 * nP) { roff[i] = 1024 + 256 * NB + (8 * (u - nP) + g) * 8 + 2 * c; rqs[i] = 64 * NB; lsel[i] = 1; }   // Q: V x W
+            else { roff[i] = 512 + (8 * (u - 2 * nP) + g) * 8 + 2 * c; rqs[i] = 128; lsel[i] = 0; }                           // D: B0 rows x V
+        }
+    }
+    double acc[QMCD_BLK_MAXU][2][2];
 #pragma unroll
-            for (int a = 0; a < 2; ++a) {
-                const int row = a * 8 + g;
-                const int owner = row % S;
-                double* rb = (S > 1) ? cl.map_shared_rank(x.recv, owner) : x.recv;
-                *reinterpret_cast<double2*>(rb + ((size_t)w.r * RPO + row / S) * RL + off + 2 * c) =
-                    make_double2(acc[i][a][0], acc[i][a][1]);
+    for (int i = 0; i < QMCD_BLK_MAXU; ++i) { acc[i][0][0] = acc[i][0][1] = acc[i][1][0] = acc[i][1][1] = 0.0; }
+    for (int kc = 0; kc < nch; ++kc) {
+        const unsigned gi = it0 + (unsigned)kc, st = gi % NS, u = gi / NS;
+        const double* stg = reinterpret_cast<const double*>(ring + st * STAGE);
+        qmcd_mbar_wait(bar0 + 8 * st, u & 1);
+        if (tid == 0 && kc + NS - 1 < nch) issue(kc + NS - 1);
+        const double* Ls = stg + g * 8 + 2 * c;                 // left operands: B0 rows at +0, V rows at +512; row block a at +64
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            double2 lb[2], lv[2];
+#pragma unroll
+            for (int a = 0; a < 2; ++a) { lb[a] = qmcd_lds128(Ls + q * 128 + a * 64); lv[a] = qmcd_lds128(Ls + 512 + q * 128 + a * 64); }
+#pragma unroll
+            for (int i = 0; i < QMCD_BLK_MAXU; ++i) {
+                if (i < nu) {
+                    const double2 bv = qmcd_lds128(stg + roff[i] + q * rqs[i]);
+                    const double2 l0 = lsel[i] ? lv[0] : lb[0], l1 = lsel[i] ? lv[1] : lb[1];
+                    qmcd_dmma(acc[i][0][0], acc[i][0][1], l0.x, bv.x);
+                    qmcd_dmma(acc[i][1][0], acc[i][1][1], l1.x, bv.x);
+                    qmcd_dmma(acc[i][0][0], acc[i][0][1], l0.y, bv.y);
+                    qmcd_dmma(acc[i][1][0], acc[i][1][1], l1.y, bv.y);
+                }
             }
         }
+        __syncwarp();
+        if (lane == 0) qmcd_mbar_arrive(bar0 + 8 * NS + 8 * st);
     }
-    if (S > 1) cl.sync(); else __syncthreads();
-    // ---- owner: sum the S partials in rank order, all-gather the result into every CTA's G
-    {
-        const int ncol = 2 * nP * 8 + QMCD_TB;            // active columns: P | Q | D
-        for (int idx = tid; idx < RPO * ncol; idx += QMCD_THREADS) {
-            const int rl = idx / ncol, ci = idx - rl * ncol;
-            const int row = rl * S + w.r;
-            if (row >= QMCD_TB) continue;
-            const int col = (ci < nP * 8) ? ci : (ci < 2 * nP * 8) ? Kp + (ci - nP * 8) : 2 * Kp + (ci - 2 * nP * 8);
-            double v = 0.0;
-            for (int r = 0; r < S; ++r) v += x.recv[((size_t)r * RPO + rl) * RL + col];
-            for (int q = 0; q < S; ++q) {
-                double* gb = (S > 1) ? cl.map_shared_rank(x.G, q) : x.G;
-                gb[(size_t)row * RL + col] = v;
-            }
+    itc = it0 + (unsigned)nch;
+    __syncthreads();
+    qmcd_blk_reduce(P, x, cl, w, acc, nu, nP);
+}
+
+// Queue append of a block's accepted moves by bulk asynchronous copies (P.la_tma): rows v -> C[slot] and
+// B0[j,:] -> W[slot] (this CTA's column slice of each) bounce through the look-ahead ring's memory, several
+// rows per wave.  Thread 0 only; the caller barriers afterwards.  `phase` = waves this CTA has issued so far.
+__device__ __noinline__ void qmcd_blk_append_bulk(const QmcdArgs& A, const QmcdSmem& s, const QmcdBlk& x, const QmcdWalker& w,
+                                                     int t, int j0, int m0, unsigned accmask, int na, unsigned& phase) {
+    const QmcdDev& P = A.P;
+    const int N = P.N, len = w.khi - w.klo;
+    const unsigned rowbytes = (unsigned)len * 8u;
+    const unsigned ring_bytes = (unsigned)(QMCD_LA_NS * qmcd_la_stage_bytes(P.K));
+    const int per_wave = max(1, (int)(ring_bytes / rowbytes));
+    const unsigned bar = qmcd_su32(reinterpret_cast<unsigned char*>(s.red) + QMCD_LA_APP_BAR_OFF);
+    const unsigned ring = qmcd_su32(x.As);
+    const int nrows = 2 * na;
+    for (int r0 = 0; r0 < nrows; r0 += per_wave) {
+        const int cnt = min(per_wave, nrows - r0);
+        qmcd_mbar_expect_tx(bar, (unsigned)cnt * rowbytes);
+        for (int i = 0; i < cnt; ++i) {
+            const int r = r0 + i, e = r >> 1;
+            const int al = __fns(accmask, 0, e + 1);
+            const double* src = (r & 1) ? w.B + (size_t)((j0 + al) % N) * N + w.klo
+                                        : A.v + ((size_t)(t + al) * P.batch + w.b) * N + w.klo;
+            qmcd_bulk_load(ring + (unsigned)i * rowbytes, src, rowbytes, bar);
         }
+        qmcd_mbar_wait(bar, phase & 1);
+        ++phase;
+        for (int i = 0; i < cnt; ++i) {
+            const int r = r0 + i, e = r >> 1;
+            double* dst = ((r & 1) ? w.W : w.C) + (size_t)(m0 + e) * N + w.klo;
+            qmcd_bulk_store(dst, ring + (unsigned)i * rowbytes, rowbytes);
+        }
+        qmcd_bulk_commit();
+        qmcd_bulk_wait_read0();             // the ring may be overwritten by the next wave / the next block's loads
     }
-    if (S > 1) cl.sync(); else __syncthreads();
+    qmcd_bulk_wait0();                      // the rows are written before the caller's barrier
 }
 
 // ---------------------------------------------------------------------------
@@ -249,7 +385,7 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
     const int tid = threadIdx.x;
     const int N = P.N, K = P.K, Kp = qmcd_blk_Kp(K), RL = qmcd_blk_RL(K), ldM = qmcd_ldM(K);
     const int len = w.khi - w.klo;
-    const QmcdBlk x = qmcd_blk_carve(s.rs, K);
+    const QmcdBlk x = qmcd_blk_carve(s.rs, K, P.la_tma != 0);
     // cycle accounting by one thread of the leader CTA (every phase boundary is a barrier)
     const bool prof = (w.r == 0 && tid == 0);
     long long cy_la = 0, cy_chain = 0, cy_app = 0, cy_fl = 0, c0 = prof ? clock64() : 0, c_start = c0;
@@ -260,6 +396,7 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
     while (t < A.n_moves) {
         const int j0 = (A.j_begin + t) % N;
         int L = min(min(QMCD_TB, LS ? min(K - pw, K - m) : K - m), A.n_moves - t);
+        if (P.la_tma) L = min(L, N - j0);              // the TMA ring takes the block's rows of B0 as one box: no wrap-around
         // an electron already queued may not be proposed inside a block (G7):
         // cut the block before it, or flush first when it is the block's first move
         {
@@ -296,7 +433,18 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
                 qmcd_prefetch_l2(w.B + (size_t)((A.j_begin + tn) % N) * N + w.klo + k);
             }
         }
-        qmcd_blk_strips(A, s, x, cl, w, t, L, m);
+        if (P.la_tma) {
+            unsigned itc = (unsigned)s.iflag[12];
+            switch (qmcd_tma_NB(K)) {
+                case 1: qmcd_blk_strips_tma<1>(A, s, x, cl, w, t, L, m, itc); break;
+                case 2: qmcd_blk_strips_tma<2>(A, s, x, cl, w, t, L, m, itc); break;
+                case 4: qmcd_blk_strips_tma<4>(A, s, x, cl, w, t, L, m, itc); break;
+                default: qmcd_blk_strips_tma<8>(A, s, x, cl, w, t, L, m, itc); break;
+            }
+            if (tid == 0) s.iflag[12] = (int)itc;      // (read again only after the barriers below)
+        } else {
+            qmcd_blk_strips(A, s, x, cl, w, t, L, m);
+        }
         QMCD_TICK(cy_la);
 
         const int m0 = m;
@@ -393,27 +541,35 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
         QMCD_TICK(cy_chain);
         // ---- append the block's accepted moves to the queue: C[slot] = v, W[slot] = B0[j,:]
         {
-            // four 16-byte vectors of each source row in flight per thread (the copy is a latency chain otherwise)
-            const int vpr = len >> 1, total = na * vpr;
-            for (int i0 = tid; i0 < total; i0 += 4 * QMCD_THREADS) {
-                double2 vv[4], bb[4];
-                size_t off[4];
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int idx = i0 + u * QMCD_THREADS;
-                    if (idx < total) {
-                        const int e = idx / vpr, k = (idx - e * vpr) * 2;
-                        const int al = __fns(accmask, 0, e + 1);
-                        vv[u] = qmcd_ldcg128(A.v + ((size_t)(t + al) * P.batch + w.b) * N + w.klo + k);
-                        bb[u] = qmcd_ldcg128(w.B + (size_t)((j0 + al) % N) * N + w.klo + k);
-                        off[u] = (size_t)(m0 + e) * N + w.klo + k;
-                    }
+            if (P.la_tma) {
+                if (tid == 0 && na > 0) {
+                    unsigned ph = (unsigned)s.iflag[13];
+                    qmcd_blk_append_bulk(A, s, x, w, t, j0, m0, accmask, na, ph);
+                    s.iflag[13] = (int)ph;
                 }
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    if (i0 + u * QMCD_THREADS < total) {
-                        qmcd_stg128(w.C + off[u], vv[u].x, vv[u].y);
-                        qmcd_stg128(w.W + off[u], bb[u].x, bb[u].y);
+            } else {
+                // four 16-byte vectors of each source row in flight per thread (the copy is a latency chain otherwise)
+                const int vpr = len >> 1, total = na * vpr;
+                for (int i0 = tid; i0 < total; i0 += 4 * QMCD_THREADS) {
+                    double2 vv[4], bb[4];
+                    size_t off[4];
+    #pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int idx = i0 + u * QMCD_THREADS;
+                        if (idx < total) {
+                            const int e = idx / vpr, k = (idx - e * vpr) * 2;
+                            const int al = __fns(accmask, 0, e + 1);
+                            vv[u] = qmcd_ldcg128(A.v + ((size_t)(t + al) * P.batch + w.b) * N + w.klo + k);
+                            bb[u] = qmcd_ldcg128(w.B + (size_t)((j0 + al) % N) * N + w.klo + k);
+                            off[u] = (size_t)(m0 + e) * N + w.klo + k;
+                        }
+                    }
+    #pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        if (i0 + u * QMCD_THREADS < total) {
+                            qmcd_stg128(w.C + off[u], vv[u].x, vv[u].y);
+                            qmcd_stg128(w.W + off[u], bb[u].x, bb[u].y);
+                        }
                     }
                 }
             }

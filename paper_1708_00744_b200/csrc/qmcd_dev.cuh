@@ -24,6 +24,7 @@ struct QmcdDev {
     int pool;                 // pool CTAs (flush workers serving every walker) in THIS launch, set per launch
     int tile_rows;            // rows of B per flush tile (64 or 128), host choice
     int use_tma;              // host: K <= 64 flush tiles through qmcd_flush_tma.cuh (TMA-fed, 128-row tiles)
+    int la_tma;               // host: qmcd_sweep's blocked look-ahead streams its operands through a TMA ring (qmcd_block.cuh)
     int ldMg;                 // row stride of M in GLOBAL memory: 64 when K <= 64 (a 64 x 64 tile, TMA box), else K
     // ---- flush jobs (leader cluster of walker b -> every worker: its own CTAs and the pool)
     unsigned long long* ticket;   // [batch]  (job number << 32) | next tile; tiles are taken by CAS
@@ -121,7 +122,7 @@ __host__ __device__ inline size_t qmcd_smem_fixed_bytes(int K, bool with_M) {
     b += qmcd_align16((size_t)QMCD_WARPS * K * 8);             // Ts
     b += qmcd_align16((size_t)K * 4);                          // Js
     if (with_M) b += qmcd_align16((size_t)K * qmcd_ldM(K) * 8);  // Ms
-    return b;
+    return (b + 127) & ~(size_t)127;                            // the union area starts 128-byte aligned (TMA destination)
 }
 __host__ __device__ inline size_t qmcd_smem_base_bytes(int N, int K, int S, bool with_M, size_t blk_bytes) {
     size_t ns = (size_t)(N + S - 1) / S + 1;
@@ -146,6 +147,7 @@ __device__ inline QmcdSmem qmcd_carve(unsigned char* base, int N, int K, int S, 
     s.Ts = (double*)p; p += qmcd_align16((size_t)QMCD_WARPS * K * 8);
     s.Js = (int*)p; p += qmcd_align16((size_t)K * 4);
     s.Ms = (double*)p; if (with_M) p += qmcd_align16((size_t)K * qmcd_ldM(K) * 8);
+    p = s.dyn + qmcd_smem_fixed_bytes(K, with_M);          // 128-byte aligned
     s.rs = (double*)p; p += qmcd_align16(ns * 8);          // union starts here (blocked area aliases it)
     s.vs = (double*)p; p += qmcd_align16(ns * 8);
     s.part = (double*)p;

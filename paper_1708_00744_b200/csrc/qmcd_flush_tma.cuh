@@ -24,7 +24,9 @@
 #include <cuda.h>
 #include "qmcd_flush_mma.cuh"
 
-struct QmcdTmaps { CUtensorMap B, C, W, M; };      // 4-D views, see qmcd_api.cu (encode_tmaps)
+// 4-D views, see qmcd_api.cu.  B, C, W, M: the flush (this file).  B16, V, Wk (+ C): the look-ahead ring of
+// qmcd_block.cuh -- B with 16-row boxes, the proposals of the current qmcd_sweep launch, W in the k-major view.
+struct QmcdTmaps { CUtensorMap B, C, W, M, B16, V, Wk; };
 
 #define QMCD_TMA_NS 4
 #define QMCD_TMA_STAGE_BYTES 49152
@@ -54,7 +56,47 @@ __device__ __forceinline__ void qmcd_tma_load4(unsigned dst, const CUtensorMap* 
     asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
                  :: "r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar) : "memory");
 }
+// 1-D bulk copies (rows of the queue append): global -> shared with mbarrier completion, shared -> global as a bulk group
+__device__ __forceinline__ void qmcd_bulk_load(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void qmcd_bulk_store(void* dst, unsigned src, unsigned bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" :: "l"(dst), "r"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void qmcd_bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void qmcd_bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void qmcd_bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+// L2 eviction policies: the flush streams each tile of B once per pass (evict first: do not push the queues
+// out of L2); the queue rows C, W and M are re-read by every tile and every look-ahead block (evict last)
+__device__ __forceinline__ unsigned long long qmcd_policy_evict_first() {
+    unsigned long long p; asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p)); return p;
+}
+__device__ __forceinline__ unsigned long long qmcd_policy_evict_last() {
+    unsigned long long p; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p;
+}
+__device__ __forceinline__ void qmcd_tma_load4_hint(unsigned dst, const CUtensorMap* tm, int c0, int c1, int c2, int c3, unsigned bar,
+                                                    unsigned long long policy) {
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4, %5}], [%6], %7;"
+                 :: "r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar), "l"(policy) : "memory");
+}
 __device__ __forceinline__ void qmcd_fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
+// look-ahead ring (qmcd_block.cuh): 3 stages; full[3] at +576, empty[3] at +600, the append's barrier at +624
+#define QMCD_LA_NS 3
+#define QMCD_LA_BAR_OFF 576
+#define QMCD_LA_APP_BAR_OFF 624
+__host__ __device__ inline size_t qmcd_la_stage_bytes(int K) { return 8192 + 4096 * (size_t)qmcd_tma_NB(K); }
+__device__ __forceinline__ void qmcd_la_init_barriers(unsigned char* smem) {
+    const unsigned bar0 = qmcd_su32(smem + QMCD_LA_BAR_OFF);
+#pragma unroll
+    for (int s = 0; s < QMCD_LA_NS; ++s) {
+        qmcd_mbar_init(bar0 + 8 * s, 1);
+        qmcd_mbar_init(bar0 + 8 * QMCD_LA_NS + 8 * s, QMCD_WARPS);
+    }
+    qmcd_mbar_init(qmcd_su32(smem + QMCD_LA_APP_BAR_OFF), 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
 
 // once per kernel, by one thread, before the CTA's first barrier
 __device__ __forceinline__ void qmcd_tma_init_barriers(unsigned char* smem) {
@@ -82,22 +124,23 @@ __device__ __noinline__ void qmcd_flush_tile_tma(const QmcdDev& P, const QmcdTma
     const unsigned it0 = itc;
     double* Bw = P.B + (size_t)b * N * N;
 
+    const unsigned long long pol_stream = qmcd_policy_evict_first(), pol_keep = qmcd_policy_evict_last();
     auto issue = [&](int j) {                     // one thread: the loads of iteration j of this tile
         const unsigned gi = it0 + (unsigned)j, s = gi % NS, u = gi / NS;
         if (u > 0) qmcd_mbar_wait(bar0 + 8 * NS + 8 * s, (u - 1) & 1);               // every warp has left the stage
         const unsigned dst = qmcd_su32(st0 + s * QMCD_TMA_STAGE_BYTES), fb = bar0 + 8 * s;
         if (j < nk) {
             qmcd_mbar_expect_tx(fb, TX_ROWS);
-            qmcd_tma_load4(dst, &TM.B, 0, row0, 4 * j, b, fb);
-            qmcd_tma_load4(dst + 32768, &TM.C, 0, 0, 4 * j, b, fb);
+            qmcd_tma_load4_hint(dst, &TM.B, 0, row0, 4 * j, b, fb, pol_stream);
+            qmcd_tma_load4_hint(dst + 32768, &TM.C, 0, 0, 4 * j, b, fb, pol_keep);
         } else if (j == nk) {
             qmcd_mbar_expect_tx(fb, 32768u);
-            qmcd_tma_load4(dst, &TM.M, 0, 0, 0, b, fb);
+            qmcd_tma_load4_hint(dst, &TM.M, 0, 0, 0, b, fb, pol_keep);
         } else {
             const int jj = j - nk - 1;
             qmcd_mbar_expect_tx(fb, TX_ROWS);
-            qmcd_tma_load4(dst, &TM.B, 0, row0, 4 * jj, b, fb);
-            qmcd_tma_load4(dst + 32768, &TM.W, 0, 0, 2 * jj, b, fb);
+            qmcd_tma_load4_hint(dst, &TM.B, 0, row0, 4 * jj, b, fb, pol_stream);
+            qmcd_tma_load4_hint(dst + 32768, &TM.W, 0, 0, 2 * jj, b, fb, pol_keep);
         }
     };
     if (tid == 0) {
