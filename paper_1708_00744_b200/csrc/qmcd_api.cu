@@ -142,7 +142,10 @@ static int configure_kernel(qmcd_ctx* h, int S) {
     // blocked look-ahead: 16-byte vector access to every slice, <= 40 output tiles
     const bool blk_shape = h->N >= QMCD_TB && (h->N % (8 * S) == 0) && (2 * ((h->K + 7) / 8) + 2 <= 8 * QMCD_BLK_MAXU);
     // the TMA look-ahead ring: K <= 64 tensor maps, column slices of whole 32-column chunks
-    bool la = blk_shape && h->la_opt && tma_shape_ok(h->N, h->K) && (h->N / S) % 32 == 0 && h->N % S == 0;
+    // (measured: it pays when a CTA's slice is long -- c2/c3/c4: +3 ... +8 % -- and costs on short ones, where the ring's
+    // fill latency per block dominates: c1, N = 512, -16 %; la_opt = 2 forces it on for any shape that fits)
+    bool la = blk_shape && h->la_opt && tma_shape_ok(h->N, h->K) && (h->N / S) % 32 == 0 && h->N % S == 0 &&
+              (h->N / S >= 1024 || h->la_opt == 2);
     size_t blk = blk_shape ? qmcd_blk_smem_bytes(h->K, la) : 0;
     size_t base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, blk);
     if (la && base > cap) { la = false; blk = qmcd_blk_smem_bytes(h->K, false); base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, blk); }
@@ -601,8 +604,8 @@ extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
         h->P.tile_rows = value;
         return QMCD_OK;
     }
-    if (!strcmp(key, "la_tma")) {                  // 0: qmcd_sweep's blocked look-ahead through LDG / cp.async instead of the TMA ring
-        if (value < 0 || value > 1) return QMCD_EINVAL;
+    if (!strcmp(key, "la_tma")) {                  // 0: blocked look-ahead through LDG / cp.async; 1: TMA ring for long slices; 2: whenever it fits
+        if (value < 0 || value > 2) return QMCD_EINVAL;
         CK(h, cudaStreamSynchronize(h->stream));
         h->la_opt = value;
         return configure_kernel(h, h->P.S);

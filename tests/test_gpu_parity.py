@@ -24,7 +24,7 @@ def _rel(a, b):
 
 
 def gpu_sweep(qmcd, wl, K, mask=None, uniforms=None, final_flush=True, cluster=None, j_begin=0,
-              flush_path=None, lookahead=None, lockstep=None, G=None, split=None, tile_rows=None, pool=None, tma=None):
+              flush_path=None, lookahead=None, lockstep=None, G=None, split=None, tile_rows=None, pool=None, tma=None, la_tma=None):
     import torch
     q = qmcd.Qmcd(wl.N, K, wl.batch)
     if lockstep is not None:
@@ -41,6 +41,9 @@ def gpu_sweep(qmcd, wl, K, mask=None, uniforms=None, final_flush=True, cluster=N
         q.set_option("pool", pool)
     if tma is not None:
         q.set_option("tma", tma)                     # 0: the cp.async flush kernels also for K <= 64
+        q.set_option("la_tma", 2 if tma else 0)      # ... and the TMA-ring look-ahead on every shape that fits / never
+    if la_tma is not None:
+        q.set_option("la_tma", la_tma)
     if tile_rows is not None:
         q.set_option("tile_rows", tile_rows)
     blocked = bool(q.get_option("blocked_ok")) and q.get_option("lookahead") == 0
@@ -62,7 +65,7 @@ def gpu_sweep(qmcd, wl, K, mask=None, uniforms=None, final_flush=True, cluster=N
     pend = q.pending().cpu().numpy()
     out = dict(R=R.cpu().numpy(), acc=acc.cpu().numpy(), B=B.cpu().numpy(), status=st, info=info,
                counters=cnt, pending=pend, S=q.get_option("cluster"), blocked=blocked, pool=q.get_option("pool"),
-               tma=q.get_option("tma"))
+               tma=q.get_option("tma"), la_tma=q.get_option("la_tma"))
     q.close()
     return out
 
@@ -257,6 +260,14 @@ def test_blocked_lookahead_matches_oracle_and_per_move(qmcd, N, K, batch, cluste
     assert not pm["blocked"]
     assert np.max(np.abs(g["R"] - pm["R"])) <= 1e-11
     assert np.max(np.abs(g["B"] - pm["B"])) <= 1e-11
+    # the same blocks with the operands streamed through the TMA ring (forced on: by default only long slices use
+    # it) -- wrap-around cuts the block, a repeated electron cuts it or flushes first; K <= 64, slices of 32-column chunks
+    if K <= 64 and N >= 128 and N % 64 == 0 and (N // cluster) % 32 == 0:
+        gt = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, j_begin=j_begin, la_tma=2)
+        assert gt["la_tma"] == 1 and gt["blocked"] and gt["status"] == 0
+        assert np.array_equal(gt["acc"], acco)
+        assert _rel(gt["R"], Ro) <= RTOL_RATIO
+        assert np.max(np.abs(gt["B"] - Bo)) <= 1e-10
 
 
 @pytest.mark.parametrize("K", [1, 16, 32])
@@ -726,6 +737,7 @@ def _windows_with_accepts(acc, K):
     (512, 64, 2, 4, None, 0.3, 0, [5]),         # DMMA flush of low, varying rank
     (96, 7, 2, 1, None, 0.1, 0, None),          # windows with no accepted move at all
     (64, 1, 2, 1, None, 0.5, 0, None),          # K = 1
+    (256, 24, 3, 2, 2, 0.5, 0, [100]),          # TMA-ring look-ahead (la_tma forced on below) + pool, windows of 16 + 8
 ])
 def test_lockstep_sweep_matches_oracle_path3(qmcd, N, K, batch, cluster, G, p, lookahead, split):
     """Option "lockstep" against the oracle's literal path 3 (a rejected move
@@ -736,9 +748,10 @@ def test_lockstep_sweep_matches_oracle_path3(qmcd, N, K, batch, cluster, G, p, l
     mask = wl.bernoulli_mask(p)
     Ao, Bo = wl.A.copy(), wl.Ainv.copy()
     Ro, acco, flo, _ = oracle.run_lockstep(Ao, Bo, K, wl.proposals, mask=mask, final_flush=False)
+    la = 2 if (N, K) == (256, 24) else None       # that case: the TMA-ring look-ahead, forced on
     g = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, G=G, lookahead=lookahead, lockstep=1,
-                  split=split, final_flush=False)
-    assert g["status"] == 0
+                  split=split, final_flush=False, la_tma=la)
+    assert g["status"] == 0 and (la is None or g["la_tma"] == 1)
     if lookahead == 1:
         assert not g["blocked"]
     assert np.array_equal(g["acc"], acco)
