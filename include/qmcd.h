@@ -129,7 +129,7 @@ int qmcd_worker_stats(qmcd_handle h, long long* stats_dev, long long* flush_rank
 
 /* Device-resident run of n_moves proposals with no host round trip (the same
  * ratio -> accept -> flush-when-full sequence, one persistent launch; results
- * equal the call-by-call sequence -- bit for bit with option "lookahead" = 1,
+ * equal the call-by-call sequence -- bit for bit with options "lookahead" = 1 and "ratio_kernel" = 0,
  * to rounding (another summation order, and an already-queued electron is
  * flushed before its block instead of at its accept) with the default blocked
  * look-ahead, which needs proposals_dev 16-byte aligned; the blocked sweep also

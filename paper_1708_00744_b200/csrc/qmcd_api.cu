@@ -10,6 +10,7 @@
 #include "../../include/qmcd.h"
 #include "qmcd_kernel.cuh"
 #include "qmcd_invert.cuh"
+#include "qmcd_ratio.cuh"
 
 enum { QMCD_IDLE = 0, QMCD_PROPOSED = 1 };
 
@@ -29,6 +30,8 @@ struct qmcd_ctx {
     QmcdTmaps tmaps;          // 4-D tensor maps of B, C, W, M for the TMA-fed flush (B re-encoded by set_inverse)
     int tma_opt;              // option "tma": 1 = use the TMA-fed flush when the shape allows
     bool tmaps_ok;            // C, W, M, Wk encoded (and B, B16 once an inverse is adopted)
+    double* rpart; unsigned* rcnt;   // qmcd_ratio kernel scratch
+    int ratio_opt;            // option "ratio_kernel": 1 = qmcd_ratio through the dedicated kernel (qmcd_ratio.cuh)
     int la_opt;               // option "la_tma": 1 = TMA-ring look-ahead in qmcd_sweep when the shape allows
     bool la_fit;              // the kernel's shared memory was sized with the look-ahead ring
     size_t ctl_off, ctl_bytes;    // job words inside the workspace (zeroed before every pooled launch)
@@ -48,7 +51,9 @@ static int cuda_fail(qmcd_ctx* h, cudaError_t e, const char* what) {
 static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
 static int qmcd_ldMg_host(int K) { return K <= 64 ? 64 : K; }
 
-struct WsLayout { size_t C, W, Y, M, J, m, sj, sR, sp, sc, sr, counters, fstat, wstat, status, ticket, jdesc, fin, ctrl, ctl_end, total; };
+struct WsLayout { size_t C, W, Y, M, J, m, sj, sR, sp, sc, sr, counters, fstat, wstat, rpart, rcnt, status, ticket, jdesc, fin, ctrl, ctl_end, total; };
+
+static int ratio_gmax(int N) { int g = (N + 63) / 64; return g > 128 ? 128 : g; }
 
 static WsLayout ws_layout(int N, int K, int batch) {
     WsLayout L; size_t o = 0;
@@ -67,6 +72,8 @@ static WsLayout ws_layout(int N, int K, int batch) {
     L.counters = o; o += al256((size_t)batch * 8 * 8);
     L.fstat = o; o += al256((size_t)batch * 2 * 8);
     L.wstat = o; o += al256((size_t)QMCD_WSTAT_CTAS * 4 * 8);
+    L.rpart = o; o += al256((size_t)batch * ratio_gmax(N) * (2 * (size_t)K + 2) * 8);   // qmcd_ratio partial sums
+    L.rcnt = o; o += al256((size_t)batch * 4);
     L.status = o; o += 256;
     L.ticket = o; o += al256((size_t)batch * 8);                  // job words: one block, zeroed per launch
     L.jdesc = o; o += al256((size_t)batch * 8);
@@ -284,7 +291,8 @@ extern "C" int qmcd_create(qmcd_handle* out, int N, int K, int batch,
     P.fin = (unsigned*)(ws + L.fin); P.ctrl = (unsigned*)(ws + L.ctrl);
     P.chain_regs = 1; P.pool = 0;
     P.flush_path = 0; P.use_tma = 0; P.ldMg = qmcd_ldMg_host(K);
-    h->tma_opt = 1; h->la_opt = 1; h->la_fit = false;
+    h->tma_opt = 1; h->la_opt = 1; h->la_fit = false; h->ratio_opt = 1;
+    h->rpart = (double*)(ws + L.rpart); h->rcnt = (unsigned*)(ws + L.rcnt);
     encode_queue_tmaps(h);
     P.tile_rows = (K <= 64 && N >= 2048) ? 128 : 64;
     int rc = QMCD_OK;
@@ -356,12 +364,45 @@ static QmcdArgs base_args(qmcd_ctx* h, int mode) {
     return a;
 }
 
+// The dedicated ratio kernel: slices of <= 256 columns (128 when N is odd: 8-byte loads), as many row groups as it
+// takes to put ~6 CTAs on every SM.
+static int launch_ratio(qmcd_ctx* h, int j, const int* jv, const double* v_dev, double* R_dev) {
+    const int N = h->N, K = h->K;
+    const bool vec2 = (N % 2 == 0) && (((uintptr_t)v_dev & 15) == 0);
+    const int per = 32 * (vec2 ? 2 : 1);                 // columns per lane round
+    int slice = QMCD_RATIO_NU * per;                     // at most 8 rounds per lane
+    const int gmax = ratio_gmax(N);
+    while (slice > per && (size_t)h->batch * ((N + slice - 1) / slice) * 8 < 148 * 6 && (N + slice / 2 - 1) / (slice / 2) <= gmax) slice /= 2;
+    int G = (N + slice - 1) / slice;
+    if (G > gmax) { G = gmax; slice = ((N + G - 1) / G + per - 1) / per * per; G = (N + slice - 1) / slice; }
+    int GR = 1;
+    while (GR < 8 && (size_t)h->batch * G * GR < 148 * 6 && 8 * GR < K) GR *= 2;
+    QmcdRatioArgs a;
+    a.P = h->P; a.j = j; a.jv = jv; a.v = v_dev; a.R_out = R_dev; a.part = h->rpart; a.cnt = h->rcnt;
+    a.G = G; a.GR = GR; a.slice = slice;
+    const size_t smem = (size_t)4 * K * 8;
+    dim3 grid((unsigned)G, (unsigned)GR, (unsigned)h->batch);
+    if (vec2) {
+        if (smem > 48 * 1024) CK(h, cudaFuncSetAttribute(qmcd_ratio_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        qmcd_ratio_kernel<2><<<grid, QMCD_THREADS, smem, h->stream>>>(a);
+    } else {
+        if (smem > 48 * 1024) CK(h, cudaFuncSetAttribute(qmcd_ratio_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        qmcd_ratio_kernel<1><<<grid, QMCD_THREADS, smem, h->stream>>>(a);
+    }
+    CK(h, cudaGetLastError());
+    return QMCD_OK;
+}
+
 extern "C" int qmcd_ratio(qmcd_handle h, int j, const double* v_dev, double* R_dev) {
     if (!h || !v_dev || !R_dev || j < 0 || j >= h->N) return QMCD_EINVAL;
     if (!h->has_inverse) return QMCD_ESTATE;
-    QmcdArgs a = base_args(h, QMCD_MODE_RATIO);
-    a.j = j; a.v = v_dev; a.R_out = R_dev;
-    int rc = launch(h, a, false);
+    int rc;
+    if (h->ratio_opt) rc = launch_ratio(h, j, nullptr, v_dev, R_dev);
+    else {
+        QmcdArgs a = base_args(h, QMCD_MODE_RATIO);
+        a.j = j; a.v = v_dev; a.R_out = R_dev;
+        rc = launch(h, a, false);
+    }
     if (rc == QMCD_OK) h->state = QMCD_PROPOSED;
     return rc;
 }
@@ -369,9 +410,13 @@ extern "C" int qmcd_ratio(qmcd_handle h, int j, const double* v_dev, double* R_d
 extern "C" int qmcd_ratio_jv(qmcd_handle h, const int* j_dev, const double* v_dev, double* R_dev) {
     if (!h || !j_dev || !v_dev || !R_dev) return QMCD_EINVAL;
     if (!h->has_inverse) return QMCD_ESTATE;
-    QmcdArgs a = base_args(h, QMCD_MODE_RATIO);
-    a.jv = j_dev; a.v = v_dev; a.R_out = R_dev;
-    int rc = launch(h, a, false);
+    int rc;
+    if (h->ratio_opt) rc = launch_ratio(h, 0, j_dev, v_dev, R_dev);
+    else {
+        QmcdArgs a = base_args(h, QMCD_MODE_RATIO);
+        a.jv = j_dev; a.v = v_dev; a.R_out = R_dev;
+        rc = launch(h, a, false);
+    }
     if (rc == QMCD_OK) h->state = QMCD_PROPOSED;
     return rc;
 }
@@ -604,6 +649,11 @@ extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
         h->P.tile_rows = value;
         return QMCD_OK;
     }
+    if (!strcmp(key, "ratio_kernel")) {            // 0: qmcd_ratio through the cluster kernel's look-ahead (the per-move sweep's arithmetic)
+        if (value < 0 || value > 1) return QMCD_EINVAL;
+        h->ratio_opt = value;
+        return QMCD_OK;
+    }
     if (!strcmp(key, "la_tma")) {                  // 0: blocked look-ahead through LDG / cp.async; 1: TMA ring for long slices; 2: whenever it fits
         if (value < 0 || value > 2) return QMCD_EINVAL;
         CK(h, cudaStreamSynchronize(h->stream));
@@ -656,6 +706,7 @@ extern "C" int qmcd_get_option(qmcd_handle h, const char* key) {
     if (!strcmp(key, "tile_rows")) return h->P.tile_rows;
     if (!strcmp(key, "tma")) return h->P.use_tma;
     if (!strcmp(key, "la_tma")) return h->P.la_tma;
+    if (!strcmp(key, "ratio_kernel")) return h->ratio_opt;
     if (!strcmp(key, "flush_path")) return h->P.flush_path;
     if (!strcmp(key, "lookahead")) return h->lookahead;
     if (!strcmp(key, "lockstep")) return h->P.lockstep;

@@ -169,7 +169,6 @@ __device__ __noinline__ void qmcd_blk_strips(const QmcdArgs& A, const QmcdSmem& 
                                 const QmcdWalker& w, int t0, int L, int m0) {
     const QmcdDev& P = A.P;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, g = lane >> 2, c = lane & 3;
-    const int S = P.S, K = P.K, Kp = qmcd_blk_Kp(K), RL = qmcd_blk_RL(K);
     const int len = w.khi - w.klo;
     const int nP = (m0 + 7) >> 3, U = 2 * nP + 2;
     const int nchunks = (len + QMCD_BLK_KC - 1) / QMCD_BLK_KC;

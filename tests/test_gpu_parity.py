@@ -70,10 +70,12 @@ def gpu_sweep(qmcd, wl, K, mask=None, uniforms=None, final_flush=True, cluster=N
     return out
 
 
-def gpu_calls(qmcd, wl, K, mask, flush_every=None, residual_cb=None):
+def gpu_calls(qmcd, wl, K, mask, flush_every=None, residual_cb=None, ratio_kernel=None):
     """The per-call API: ratio -> accept(mask) per move."""
     import torch
     q = qmcd.Qmcd(wl.N, K, wl.batch)
+    if ratio_kernel is not None:
+        q.set_option("ratio_kernel", ratio_kernel)
     B = _dev(wl.Ainv)
     q.set_inverse(B)
     P = _dev(wl.proposals)
@@ -216,11 +218,13 @@ def test_sweep_equals_call_by_call(qmcd):
     """qmcd_sweep must reproduce the ratio -> accept(mask) sequence (include/qmcd.h)."""
     wl = inputs.make_workload(4, 128, 200, seed=3)
     mask = wl.bernoulli_mask(0.7)
-    a = gpu_sweep(qmcd, wl, 8, mask=mask, lookahead=1)      # per-move look-ahead: same arithmetic
-    b = gpu_calls(qmcd, wl, 8, mask)
+    a = gpu_sweep(qmcd, wl, 8, mask=mask, lookahead=1)      # per-move look-ahead ...
+    b = gpu_calls(qmcd, wl, 8, mask, ratio_kernel=0)        # ... and qmcd_ratio through the same device function: same arithmetic
     assert not a["blocked"]
     assert np.array_equal(a["R"], b["R"])
     assert np.array_equal(a["B"], b["B"])
+    b = gpu_calls(qmcd, wl, 8, mask)                        # the dedicated ratio kernel (default): another summation order
+    assert _rel(b["R"], a["R"]) <= 1e-12 and np.max(np.abs(a["B"] - b["B"])) <= 1e-12
     c = gpu_sweep(qmcd, wl, 8, mask=mask)                   # blocked look-ahead: other summation order
     assert c["blocked"]
     assert _rel(c["R"], b["R"]) <= 1e-12
@@ -629,6 +633,54 @@ def test_cluster_option_rejects_non_powers_of_two(qmcd):
         q.set_option("cluster", ok)
         assert q.get_option("cluster") == ok
     q.close()
+
+
+# ------------------------------------------------------------------ the dedicated ratio kernel (per-call API)
+@pytest.mark.parametrize("N,K,batch,n_moves", [
+    (33, 5, 7, 40),          # odd N: 8-byte loads, one slice
+    (100, 7, 3, 60),         # even, ragged slice
+    (257, 33, 2, 80),        # odd N, several slices, K not a multiple of 8
+    (1024, 64, 4, 150),      # several slices x row groups, two full windows
+    (2048, 200, 1, 230),     # one walker: 8 row groups; M (200 x 200) read from global memory by the last CTA
+])
+def test_ratio_kernel_per_call_vs_oracle(qmcd, N, K, batch, n_moves):
+    """qmcd_ratio through the dedicated kernel (qmcd_ratio.cuh): every ratio of a call-by-call run against the
+    oracle's delayed path at every queue length 0 ... K-1, with accepts and rejects in between; and the
+    same calls through the cluster kernel's look-ahead (option ratio_kernel = 0) agree to rounding."""
+    import torch
+    wl = inputs.make_workload(batch, N, n_moves, seed=29)
+    mask = wl.bernoulli_mask(0.85)
+    Bo = wl.Ainv.copy()
+    D = [oracle.Delayed(Bo[w], K) for w in range(batch)]
+    runs = {}
+    for opt in (1, 0):
+        q = qmcd.Qmcd(N, K, batch)
+        q.set_option("ratio_kernel", opt)
+        B = _dev(wl.Ainv); q.set_inverse(B)
+        P, Md = _dev(wl.proposals), _dev(mask)
+        R = torch.zeros(batch, dtype=torch.float64, device="cuda")
+        Rs = np.zeros((n_moves, batch))
+        for t in range(n_moves):
+            q.ratio(t % N, P[t], R)
+            q.accept(Md[t])
+            Rs[t] = R.cpu().numpy()
+        q.flush()
+        assert q.status()[0] == 0
+        runs[opt] = (Rs, B.cpu().numpy())
+        q.close()
+    for t in range(n_moves):
+        for w in range(batch):
+            Ro = D[w].ratio(t % N, wl.proposals[t, w])
+            assert abs(runs[1][0][t, w] / Ro - 1) <= RTOL_RATIO, (t, w)
+            if mask[t, w]:
+                D[w].accept()
+            else:
+                D[w].reject()
+    for w in range(batch):
+        D[w].flush()
+    assert np.max(np.abs(runs[1][1] - Bo)) <= 1e-10
+    assert np.max(np.abs(runs[1][0] / runs[0][0] - 1)) <= 1e-11
+    assert np.max(np.abs(runs[1][1] - runs[0][1])) <= 1e-11
 
 
 # ------------------------------------------------------------------ slot replacement (SURVEY 8(f4), reading G7)
