@@ -250,10 +250,14 @@ static int launch(qmcd_ctx* h, QmcdArgs& a, bool with_pool) {
 // that do not shrink with S), while flush tiles go to any free CTA.  With many walkers the pool
 // hides one walker's look-ahead behind the others' flushes, so small clusters (more pool CTAs,
 // no DSMEM exchange) win; with few walkers the chain is exposed and a larger S shortens it.
-static int default_S(int N, int batch, int cap) {
+static int default_S(int N, int K, int batch, int cap) {
     int s = 1;
     if (batch <= 4) s = 8; else if (batch <= 16) s = 2;
     if ((long long)N * batch <= 16384) s *= 2;     // small problems: the flush is short, the chain dominates
+    // K > 64 runs the per-move look-ahead (one cluster barrier per proposal, 2m + 2 streamed rows): it is a latency
+    // chain that shortens with S (measured: c3 K=128 S=1/2/4 -> 0.27/0.38/0.33 of the DMMA peak; c4 K=128 S=2/4/8 ->
+    // 0.31/0.42/0.32; c4 K=256 S=2/4/8 -> 0.12/0.16/0.18)
+    if (K > 128) s *= 4; else if (K > 64) s *= 2;
     while (s > 1 && (N / s < 64 || N % (8 * s) != 0)) s /= 2;
     if (s > cap) s = cap;
     return s < 1 ? 1 : s;
@@ -311,7 +315,7 @@ extern "C" int qmcd_create(qmcd_handle* out, int N, int K, int batch,
         h->max_cluster = 16;
         // S = CTAs per leader cluster: the default of default_S, halved until `batch` clusters of it
         // are co-resident (so that a pool can be attached) or S = 1
-        int S = default_S(N, batch, h->max_cluster);
+        int S = default_S(N, K, batch, h->max_cluster);
         for (;; S /= 2) {
             rc = configure_kernel(h, S);
             if (rc != QMCD_OK || S == 1) break;
