@@ -158,8 +158,17 @@ static int configure_kernel(qmcd_ctx* h, int S) {
     if (la && base > cap) { la = false; blk = qmcd_blk_smem_bytes(h->K, false); base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, blk); }
     h->la_fit = la;
     h->P.m_in_smem = 1; h->P.blk_ok = blk_shape ? 1 : 0;
-    if (base > cap) { h->la_fit = false; base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, 0); h->P.blk_ok = 0; }
-    if (base > cap) { base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, false, 0); h->P.m_in_smem = 0; }
+    if (base > cap) {
+        // M does not fit beside the blocked look-ahead's area: keep the blocked look-ahead and leave M in global memory
+        // (staged 16 rows at a time, qmcd_blk_xy_global) when K is even and small enough for its register tile
+        h->la_fit = false;
+        const size_t nb = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, false, qmcd_blk_smem_bytes(h->K, false));
+        if (blk_shape && h->K % 2 == 0 && h->K <= 16 * QMCD_BLK_YU && nb <= cap) { base = nb; h->P.m_in_smem = 0; h->P.blk_ok = 1; }
+        else {
+            base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, 0); h->P.blk_ok = 0;
+            if (base > cap) { base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, false, 0); h->P.m_in_smem = 0; }
+        }
+    }
     const size_t mma = QMCD_SMEM_HEADER + qmcd_flush_mma_smem_bytes(h->N, h->K);
     if (base > cap) { snprintf(g_last_error, sizeof(g_last_error), "shared memory need %zu > 227 KB", base); return QMCD_EINVAL; }
     h->P.mma_smem_ok = (mma <= cap) ? 1 : 0;
@@ -172,6 +181,8 @@ static int configure_kernel(qmcd_ctx* h, int S) {
     CK(h, cudaFuncSetAttribute(qmcd_kernel_sweep, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     CK(h, cudaFuncSetAttribute(qmcd_kernel_sweep_ls, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     CK(h, cudaFuncSetAttribute(qmcd_kernel_sweep_ls, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    CK(h, cudaFuncSetAttribute(qmcd_kernel_sweep_gm, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    CK(h, cudaFuncSetAttribute(qmcd_kernel_sweep_gm, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     h->smem_bytes = smem;
     h->P.S = S;
     if (h->K > 64) h->P.tile_rows = 64;          // T for 128 rows does not fit beside the chunk ring
@@ -229,7 +240,9 @@ static int launch(qmcd_ctx* h, QmcdArgs& a, bool with_pool) {
         cfg.numAttrs = (pool > 0 && h->coop) ? 2 : 1;
         cudaError_t e = cudaMemsetAsync(h->ws + h->ctl_off, 0, h->ctl_bytes, h->stream);   // job words of this launch
         if (e != cudaSuccess) return e;
-        if (a.mode == QMCD_MODE_SWEEP && a.blocked && h->P.m_in_smem)
+        if (a.mode == QMCD_MODE_SWEEP && a.blocked && !h->P.m_in_smem)
+            return cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep_gm, a, h->tmaps);
+        if (a.mode == QMCD_MODE_SWEEP && a.blocked)
             return h->P.lockstep ? cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep_ls, a, h->tmaps) : cudaLaunchKernelEx(&cfg, qmcd_kernel_sweep, a, h->tmaps);
         return cudaLaunchKernelEx(&cfg, qmcd_kernel, a, h->tmaps);
     };
@@ -254,10 +267,11 @@ static int default_S(int N, int K, int batch, int cap) {
     int s = 1;
     if (batch <= 4) s = 8; else if (batch <= 16) s = 2;
     if ((long long)N * batch <= 16384) s *= 2;     // small problems: the flush is short, the chain dominates
-    // K > 64 runs the per-move look-ahead (one cluster barrier per proposal, 2m + 2 streamed rows): it is a latency
-    // chain that shortens with S (measured: c3 K=128 S=1/2/4 -> 0.27/0.38/0.33 of the DMMA peak; c4 K=128 S=2/4/8 ->
-    // 0.31/0.42/0.32; c4 K=256 S=2/4/8 -> 0.12/0.16/0.18)
-    if (K > 128) s *= 4; else if (K > 64) s *= 2;
+    // K > 152 (or odd K > 64) runs the per-move look-ahead (one cluster barrier per proposal, 2m + 2 streamed rows): a
+    // latency chain that shortens with S (measured with it: c3 K=128 S=1/2/4 -> 0.27/0.38/0.33 of the DMMA peak; c4 K=256
+    // S=2/4/8 -> 0.12/0.16/0.18).  64 < K <= 152, K even, keeps the blocked look-ahead with M in global memory (c3 K=128
+    // S=1/2/4 -> 0.48/0.46/0.39; c4 K=128 S=1/2/4 -> 0.41/0.51/0.45) and the cluster size of the small delays.
+    if (K > 152 || (K > 64 && (K & 1))) s *= (K > 128) ? 4 : 2;
     while (s > 1 && (N / s < 64 || N % (8 * s) != 0)) s /= 2;
     if (s > cap) s = cap;
     return s < 1 ? 1 : s;
@@ -509,7 +523,9 @@ extern "C" int qmcd_sweep(qmcd_handle h, int j_begin, int n_moves,
     a.j_begin = j_begin; a.n_moves = n_moves; a.v = proposals_dev;
     a.mask = mask_dev; a.uniforms = uniforms_dev; a.R_out = R_out_dev; a.acc_out = acc_out_dev;
     if (h->P.la_tma && !encode_proposals(&h->tmaps.V, proposals_dev, n_moves, h->N, h->batch)) { h->la_opt = 0; refresh_use_tma(h); a.P = h->P; }
-    a.blocked = (h->lookahead != 1 && !h->P.slot_replace && h->P.blk_ok && h->P.m_in_smem && (((uintptr_t)proposals_dev & 15) == 0)) ? 1 : 0;
+    // (the blocked look-ahead with M in global memory has no lock-step variant: that combination runs per move)
+    a.blocked = (h->lookahead != 1 && !h->P.slot_replace && h->P.blk_ok && (h->P.m_in_smem || !h->P.lockstep) &&
+                 (((uintptr_t)proposals_dev & 15) == 0)) ? 1 : 0;
     return launch(h, a, true);
 }
 
@@ -715,7 +731,7 @@ extern "C" int qmcd_get_option(qmcd_handle h, const char* key) {
     if (!strcmp(key, "lookahead")) return h->lookahead;
     if (!strcmp(key, "lockstep")) return h->P.lockstep;
     if (!strcmp(key, "slot_replace")) return h->P.slot_replace;
-    if (!strcmp(key, "blocked_ok")) return h->P.blk_ok && h->P.m_in_smem && !h->P.slot_replace;
+    if (!strcmp(key, "blocked_ok")) return h->P.blk_ok && (h->P.m_in_smem || !h->P.lockstep) && !h->P.slot_replace;
     if (!strcmp(key, "m_in_smem")) return h->P.m_in_smem;
     if (!strcmp(key, "threads")) return QMCD_THREADS;
     if (!strcmp(key, "smem_bytes")) return (int)h->smem_bytes;

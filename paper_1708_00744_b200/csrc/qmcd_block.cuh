@@ -356,6 +356,55 @@ __device__ __noinline__ void qmcd_blk_append_bulk(const QmcdArgs& A, const QmcdS
     qmcd_bulk_wait0();                      // the rows are written before the caller's barrier
 }
 
+// X = M0 Q^T and Y = P M0 of one block with M in GLOBAL memory (K too large for a shared-memory copy): M0 is staged
+// 16 rows at a time into the (idle) operand area x.As; thread (il, tl) forms X[p0 + il][tl], thread (t, bq) keeps
+// Y[t][bq + 16 u] in registers over all panels.  Needs K even (16-byte row alignment) and K <= 16 * QMCD_BLK_YU.
+#define QMCD_BLK_YU 10
+__device__ __noinline__ void qmcd_blk_xy_global(const QmcdDev& P, const QmcdBlk& x, const QmcdWalker& w, int m0, int L) {
+    const int tid = threadIdx.x, K = P.K, Kp = qmcd_blk_Kp(K), RL = qmcd_blk_RL(K), ldg = P.ldMg;
+    const int ldp = Kp + 2, m0e = (m0 + 1) & ~1, vpr = m0e >> 1;
+    double* Mp = x.As;
+    const int t = tid >> 4, bq = tid & 15;
+    double ya[QMCD_BLK_YU];
+#pragma unroll
+    for (int u = 0; u < QMCD_BLK_YU; ++u) ya[u] = 0.0;
+    const double* Gq = x.G + (size_t)bq * RL + Kp;         // Q[tl = bq][:]  (X part: il = t, tl = bq)
+    const double* Gp = x.G + (size_t)t * RL;               // P[t][:]        (Y part)
+    for (int p0 = 0; p0 < m0; p0 += 16) {
+        const int pr = min(16, m0 - p0);
+        __syncthreads();                                   // the previous panel has been consumed
+        for (int i0 = tid; i0 < pr * vpr; i0 += 4 * QMCD_THREADS) {
+            double2 v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int idx = i0 + u * QMCD_THREADS;
+                if (idx < pr * vpr) { const int r = idx / vpr, c2 = (idx - r * vpr) * 2; v[u] = qmcd_ldcg128(w.M + (size_t)(p0 + r) * ldg + c2); }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int idx = i0 + u * QMCD_THREADS;
+                if (idx < pr * vpr) { const int r = idx / vpr, c2 = (idx - r * vpr) * 2; *reinterpret_cast<double2*>(Mp + r * ldp + c2) = v[u]; }
+            }
+        }
+        __syncthreads();
+        if (t < pr) {                                      // X[p0 + t][bq]
+            double xa = 0.0;
+            if (bq < L) { const double* row = Mp + t * ldp; for (int b = 0; b < m0; ++b) xa += row[b] * Gq[b]; }
+            x.Xm[(p0 + t) * QMCD_TB + bq] = xa;
+        }
+        if (t < L) {
+            for (int il = 0; il < pr; ++il) {
+                const double pv = Gp[p0 + il];
+                const double* row = Mp + il * ldp + bq;
+#pragma unroll
+                for (int u = 0; u < QMCD_BLK_YU; ++u) if (bq + 16 * u < m0) ya[u] += pv * row[16 * u];
+            }
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < QMCD_BLK_YU; ++u) if (bq + 16 * u < m0) x.Ym[t * Kp + bq + 16 * u] = ya[u];
+}
+
 // ---------------------------------------------------------------------------
 // The sweep loop in blocks (M in shared memory, replicated in every CTA).
 // Returns the queue length at the end.  Every CTA of the cluster runs the same
@@ -377,7 +426,7 @@ __device__ __noinline__ void qmcd_blk_append_bulk(const QmcdArgs& A, const QmcdS
 // ---------------------------------------------------------------------------
 // LS: the lock-step variant, a compile-time flag: a run-time test in this loop cost the
 // default scheme 12 % on c1 (measured A/B on one box), so each reading has its own kernel entry.
-template <bool LS>
+template <bool LS, bool MS>
 __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group& cl,
                                   const QmcdWalker& w, int m) {
     const QmcdDev& P = A.P;
@@ -412,7 +461,7 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
                 __syncthreads();
                 if (L == 0) {
                     QMCD_TICK(cy_la);
-                    qmcd_flush_phase<true>(P, s, cl, w, m);
+                    qmcd_flush_phase<MS>(P, s, cl, w, m);
                     QMCD_TICK(cy_fl);
                     m = 0; pw = 0;
                     continue;
@@ -448,19 +497,23 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
 
         const int m0 = m;
         // ---- X = M0 Q^T (Xm[i][t]) and Y = P M0 (Ym[t][b]) for every move of the block
-        for (int idx = tid; idx < m0 * QMCD_TB; idx += QMCD_THREADS) {
-            const int i = idx >> 4, tl = idx & 15;
-            double xa = 0.0, ya = 0.0;
-            if (tl < L) {
-                const double* Gq = x.G + (size_t)tl * RL + Kp;      // Q[tl][:]
-                const double* Gp = x.G + (size_t)tl * RL;           // P[tl][:]
-                for (int b = 0; b < m0; ++b) {
-                    xa += s.Ms[(size_t)i * ldM + b] * Gq[b];
-                    ya += Gp[b] * s.Ms[(size_t)b * ldM + i];
+        if (MS) {
+            for (int idx = tid; idx < m0 * QMCD_TB; idx += QMCD_THREADS) {
+                const int i = idx >> 4, tl = idx & 15;
+                double xa = 0.0, ya = 0.0;
+                if (tl < L) {
+                    const double* Gq = x.G + (size_t)tl * RL + Kp;      // Q[tl][:]
+                    const double* Gp = x.G + (size_t)tl * RL;           // P[tl][:]
+                    for (int b = 0; b < m0; ++b) {
+                        xa += s.Ms[(size_t)i * ldM + b] * Gq[b];
+                        ya += Gp[b] * s.Ms[(size_t)b * ldM + i];
+                    }
                 }
+                x.Xm[i * QMCD_TB + tl] = xa;
+                x.Ym[tl * Kp + i] = ya;
             }
-            x.Xm[i * QMCD_TB + tl] = xa;
-            x.Ym[tl * Kp + i] = ya;
+        } else {
+            qmcd_blk_xy_global(P, x, w, m0, L);
         }
         __syncthreads();
         // ---- Z0 = D - P X : one element per thread
@@ -519,11 +572,10 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
             __syncthreads();
             // M11 += U Y_acc ; M12 = -U ; M21 = -W1 Y_acc ; M22 = W1
             const int mn = m0 + na;
-            for (int idx = tid; idx < mn * mn; idx += QMCD_THREADS) {
-                const int a = idx / mn, b = idx - a * mn;
+            auto newM = [&](int a, int b, double mold) -> double {
                 double v;
                 if (a < m0 && b < m0) {
-                    v = s.Ms[(size_t)a * ldM + b];
+                    v = mold;
                     for (int f = 0; f < na; ++f) v += x.Um[a * QMCD_TB + f] * x.Ym[al_s[f] * Kp + b];
                 } else if (a < m0) {
                     v = -x.Um[a * QMCD_TB + (b - m0)];
@@ -533,7 +585,31 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
                 } else {
                     v = Zc[al_s[a - m0] * QMCD_TB + al_s[b - m0]];
                 }
-                s.Ms[(size_t)a * ldM + b] = v;
+                return v;
+            };
+            if (MS) {
+                for (int idx = tid; idx < mn * mn; idx += QMCD_THREADS) {
+                    const int a = idx / mn, b = idx - a * mn;
+                    s.Ms[(size_t)a * ldM + b] = newM(a, b, (a < m0 && b < m0) ? s.Ms[(size_t)a * ldM + b] : 0.0);
+                }
+            } else if (w.r == 0) {
+                // M in global memory (row stride P.ldMg), written by the leader CTA only; four elements per thread in flight
+                const int ldg = P.ldMg;
+                for (int i0 = tid; i0 < mn * mn; i0 += 4 * QMCD_THREADS) {
+                    double mo[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int idx = i0 + u * QMCD_THREADS;
+                        const int a = idx / mn, b = idx - a * mn;
+                        mo[u] = (idx < mn * mn && a < m0 && b < m0) ? __ldcg(w.M + (size_t)a * ldg + b) : 0.0;
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int idx = i0 + u * QMCD_THREADS;
+                        if (idx < mn * mn) { const int a = idx / mn, b = idx - a * mn; w.M[(size_t)a * ldg + b] = newM(a, b, mo[u]); }
+                    }
+                }
+                __threadfence();
             }
             if (tid < na) s.Js[m0 + tid] = (j0 + al_s[tid]) % N;
         }
@@ -592,10 +668,10 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
         if (LS) {
             pw += L;
             if (pw >= K) {                             // every walker closes its window here, rank m <= K
-                if (m > 0) { qmcd_flush_phase<true>(P, s, cl, w, m); m = 0; QMCD_TICK(cy_fl); }
+                if (m > 0) { qmcd_flush_phase<MS>(P, s, cl, w, m); m = 0; QMCD_TICK(cy_fl); }
                 pw = 0;
             }
-        } else if (K - m < max(1, min(QMCD_TB / 2, K / 4))) { qmcd_flush_phase<true>(P, s, cl, w, m); m = 0; QMCD_TICK(cy_fl); }
+        } else if (K - m < max(1, min(QMCD_TB / 2, K / 4))) { qmcd_flush_phase<MS>(P, s, cl, w, m); m = 0; QMCD_TICK(cy_fl); }
     }
     if (LS && w.r == 0 && tid == 0) P.counters[(size_t)w.b * 8 + 7] = pw;
     if (prof) {

@@ -363,7 +363,7 @@ __device__ void qmcd_run(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group
 
 // Common prologue / epilogue of the entry points.  BLOCKED != 0: the blocked sweep only (its
 // own register allocation: the per-move look-ahead of the generic entry is not compiled in).
-template <int BLOCKED>      // 0 generic, 1 blocked sweep, 2 blocked sweep in lock-step
+template <int BLOCKED>      // 0 generic, 1 blocked sweep, 2 blocked sweep in lock-step, 3 blocked sweep with M in global memory
 __device__ __forceinline__ void qmcd_kernel_body(const QmcdArgs& A, const QmcdTmaps& TM) {
     extern __shared__ __align__(1024) unsigned char qmcd_smem_raw[];
     const QmcdDev& P = A.P;
@@ -383,10 +383,15 @@ __device__ __forceinline__ void qmcd_kernel_body(const QmcdArgs& A, const QmcdTm
     const QmcdWalker w = qmcd_walker(P, b, r);
     const long long c_launch = clock64();
     if (S > 1) cl.sync();                            // every CTA of the cluster runs before any remote shared-memory access
-    if (BLOCKED) {
+    if (BLOCKED == 3) {                              // blocked sweep with M in global memory (K too large for shared memory)
+        int m = __ldcg(P.m + b);
+        qmcd_load_state<false>(P, s, w, m);
+        m = qmcd_sweep_blocked<false, false>(A, s, cl, w, m);
+        if (r == 0 && threadIdx.x == 0) { P.sj[b] = -1; P.m[b] = m; }
+    } else if (BLOCKED) {
         int m = __ldcg(P.m + b);
         qmcd_load_state<true>(P, s, w, m);
-        m = qmcd_sweep_blocked<BLOCKED == 2>(A, s, cl, w, m);
+        m = qmcd_sweep_blocked<BLOCKED == 2, true>(A, s, cl, w, m);
         qmcd_writeback_M<true>(P, s, w, m);
         if (r == 0 && threadIdx.x == 0) { P.sj[b] = -1; P.m[b] = m; }
     } else {
@@ -403,3 +408,4 @@ __device__ __forceinline__ void qmcd_kernel_body(const QmcdArgs& A, const QmcdTm
 __global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel(const QmcdArgs A, const __grid_constant__ QmcdTmaps TM) { qmcd_kernel_body<0>(A, TM); }
 __global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel_sweep(const QmcdArgs A, const __grid_constant__ QmcdTmaps TM) { qmcd_kernel_body<1>(A, TM); }
 __global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel_sweep_ls(const QmcdArgs A, const __grid_constant__ QmcdTmaps TM) { qmcd_kernel_body<2>(A, TM); }
+__global__ void __launch_bounds__(QMCD_THREADS, 1) qmcd_kernel_sweep_gm(const QmcdArgs A, const __grid_constant__ QmcdTmaps TM) { qmcd_kernel_body<3>(A, TM); }

@@ -239,6 +239,9 @@ def test_sweep_equals_call_by_call(qmcd):
     (64, 64, 2, 1, 0.3, 0),        # K = N with many rejections: electrons repeat inside a window
     (48, 24, 2, 2, 0.4, 5),        # ragged chunk (24 columns per CTA), repeats
     (1024, 32, 2, 16, 0.99, 0),    # 16 CTAs per walker, one strip row per owner
+    (512, 128, 2, 2, 0.9, 0),      # K = 128: M stays in GLOBAL memory, staged 16 rows at a time (qmcd_blk_xy_global)
+    (256, 150, 2, 1, 0.5, 3),      # K = 150 (ragged panels, K not a multiple of 8), many rejections
+    (1024, 128, 3, 4, 0.99, 1000), # clusters of 4: the leader CTA alone writes M, the others read it after the barrier
 ])
 def test_blocked_lookahead_matches_oracle_and_per_move(qmcd, N, K, batch, cluster, p, j_begin):
     """qmcd_sweep's blocked look-ahead (qmcd_block.cuh) against the oracle's delayed path and
