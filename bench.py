@@ -60,6 +60,8 @@ def parse_args():
     ap.add_argument("--no-dgemm", action="store_true", help="skip the library fp64 GEMM ceiling (checker only)")
     ap.add_argument("--quick", action="store_true", help="= --no-cpu-baseline --no-e2e --no-k1 --no-phases --no-dgemm")
     ap.add_argument("--nvtx", action="store_true", help="NVTX ranges around each part of the run")
+    ap.add_argument("--Ks", default="", help="comma-separated delays: one JSON line per K on ONE generated workload "
+                                             "(K sweeps / the paper's grid; overrides --K)")
     a = ap.parse_args()
     if a.quick:
         a.no_cpu_baseline = a.no_e2e = a.no_k1 = a.no_phases = a.no_dgemm = True
@@ -286,7 +288,7 @@ def load_peaks():
         return {}
 
 
-def run_ours(args):
+def run_ours(args, wl_cache=None):
     import torch
     import torch.distributed as dist
     from paper_1708_00744_b200 import binding, buildlib, inputs
@@ -299,7 +301,7 @@ def run_ours(args):
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference "
                          "for the CPU oracle)")
     torch.cuda.set_device(local)
-    if world > 1:
+    if world > 1 and not dist.is_initialized():
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     if rank == 0:
@@ -310,8 +312,13 @@ def run_ours(args):
     nvtx = Nvtx(args.nvtx)
 
     cfg = get_config(args)
-    wl = inputs.make_workload(cfg["batch"], cfg["N"], cfg["sweeps"] * cfg["N"],
-                              seed=qdist.rank_seed(cfg["seed"], rank, cfg["batch"]), want_A=False)     # per-rank walkers
+    if wl_cache is not None and "wl" in wl_cache:
+        wl = wl_cache["wl"]
+    else:
+        wl = inputs.make_workload(cfg["batch"], cfg["N"], cfg["sweeps"] * cfg["N"],
+                                  seed=qdist.rank_seed(cfg["seed"], rank, cfg["batch"]), want_A=False)     # per-rank walkers
+        if wl_cache is not None:
+            wl_cache["wl"] = wl
     N, K, batch, n_moves = wl.N, args.K, wl.batch, wl.n_moves
     mask, uniforms = mode_inputs(wl, args.mode)
     big = inputs_exceed_l2(batch, N, n_moves)
@@ -416,7 +423,7 @@ def run_ours(args):
             del Ph, Bh, Rh, Ah, staging
 
     if rank != 0:
-        if world > 1:
+        if world > 1 and wl_cache is None:
             dist.destroy_process_group()
         return
 
@@ -489,8 +496,8 @@ def run_ours(args):
         assert np.array_equal(acc_o, acc_h[:n]), "accept sequence differs from the oracle"
         out["cpu_baseline"] = {"value": int(acc_o.sum()) / dt, "unit": UNIT, "cores": thr, "kind": "oracle",
                                "sample": sample_text(args, batch, n, n_moves) + f", {dt:.2f} s wall"}
-    print(json.dumps(out))
-    if world > 1:
+    print(json.dumps(out), flush=True)
+    if world > 1 and wl_cache is None:
         dist.destroy_process_group()
 
 
@@ -624,6 +631,11 @@ def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.Ks:
+        cache = {}
+        for k in [int(x) for x in args.Ks.split(",")]:
+            args.K = k
+            run_ours(args, cache)
     else:
         run_ours(args)
 
