@@ -19,7 +19,9 @@
  *
  * Conventions common to every call
  *   - All `*_dev` pointers are DEVICE pointers, fp64 unless stated, owned by the
- *     caller (e.g. torch tensors).  The library never allocates device memory.
+ *     caller (e.g. torch tensors).  The library never allocates device memory
+ *     (one exception, outside the method: qmcd_probe_fp64 allocates and frees an
+ *     8-byte scratch).
  *   - Every call only ENQUEUES work on the handle's CUDA stream and returns; no
  *     call synchronises except qmcd_status, qmcd_destroy and qmcd_sweep_host.
  *   - Return value: QMCD_OK (0) or a negative QMCD_E* code.  Argument and state
@@ -55,7 +57,8 @@ size_t qmcd_workspace_bytes(int N, int K, int batch);
 /* Create a handle.  workspace_dev: >= qmcd_workspace_bytes bytes, 256-byte
  * aligned, caller-owned, must outlive the handle; it is zero-filled here
  * (enqueued).  cuda_stream: a cudaStream_t (may be NULL = default stream).
- * Errors: QMCD_EINVAL (ranges, K > N, NULL, too small, misaligned), QMCD_ECUDA. */
+ * Errors: QMCD_EINVAL (ranges, K > N, K > 4095, NULL, too small, misaligned), QMCD_ENOMEM
+ * (host allocation of the handle failed), QMCD_ECUDA. */
 int qmcd_create(qmcd_handle* out, int N, int K, int batch,
                 void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
 
@@ -171,21 +174,36 @@ size_t qmcd_invert_scratch_bytes(int N, int batch);
 int qmcd_invert(qmcd_handle h, const double* A_dev, double* Ainv_dev,
                 void* scratch_dev, size_t scratch_bytes, int* info_dev);
 
-/* Tuning / introspection.  set: "cluster" (CTAs per cluster, 1..16; resets
- * "clusters_per_walker" to 1), "clusters_per_walker" (1..16, 1..4 when K > 64: cluster 0 of a walker
- * runs the look-ahead, all of them share the rows of a flush; they must all fit
- * on the device at once, else QMCD_EINVAL; such launches are cooperative, and when the driver
- * refuses one at launch time the same step runs with the leader clusters alone), "flush_path"
- * (0 auto, 1 CUDA-core, 2 DMMA), "lookahead" (qmcd_sweep: 0 auto = blocked
- * look-ahead when the shape allows, 1 = per move, the arithmetic of the per-call
- * API), "lockstep" (0/1, IDLE only: the lock-step variant of PAPER.md:97-99 --
- * every proposal, accepted or not, takes one of the K slots of the window (a rejected
- * one stands for the unchanged column, a zero column of U in Eq. 4, so it adds no
- * arithmetic), and Eq. 4 is applied after every K-th PROPOSAL with rank m = the
- * moves accepted in the window, 0 <= m <= K: all walkers flush in the same move.
- * Holds for qmcd_accept* / qmcd_reject and both sweeps; qmcd_flush and
- * qmcd_set_inverse open a new window).  get: those plus "threads", "smem_bytes", "m_in_smem", "blocked_ok",
- * "max_active_clusters".
+/* Tuning / introspection (IDLE only).  set:
+ *   "cluster"       CTAs per LEADER cluster (1, 2, 4, 8, 16; other values: QMCD_EINVAL).  Cluster b of the grid leads
+ *                   walker b: look-ahead, accept, posting of its flush jobs.
+ *   "pool"          -1 auto (default): qmcd_sweep / qmcd_flush launches fill every SM the leader clusters leave free
+ *                   with POOL CTAs that take flush tiles of any walker; 0 = leaders only; n > 0 = at most n pool CTAs.
+ *                   The pool needs all leader clusters co-resident (else it is 0).  "clusters_per_walker" is the
+ *                   round-1 name: 1 = pool off, > 1 = pool auto.
+ *   "cooperative"   1 (default): pooled launches are cooperative launches (the driver guarantees co-residency or the
+ *                   launch fails, and the step then runs with the leaders alone); 0 = plain launches (profilers that
+ *                   cannot replay cooperative cluster launches; safe on an otherwise idle device: one CTA per SM).
+ *   "tma"           1 (default): flush tiles for K <= 64, N >= 128, N % 64 == 0 through the TMA-fed kernel
+ *                   (128-row tiles); 0 = the cp.async DMMA kernels.  "tile_rows" (64 / 128) applies to the latter.
+ *   "la_tma"        qmcd_sweep's blocked look-ahead streams its operands through a TMA ring: 1 (default) when a CTA's
+ *                   column slice has >= 1024 columns, 2 whenever the shape allows (K <= 64, slices of whole 32-column
+ *                   chunks), 0 never.
+ *   "ratio_kernel"  1 (default): qmcd_ratio runs the dedicated bandwidth kernel; 0 = the cluster kernel's look-ahead
+ *                   (the arithmetic of the per-move sweep, bit for bit).
+ *   "flush_path"    0 auto, 1 CUDA-core, 2 DMMA.
+ *   "lookahead"     qmcd_sweep: 0 auto = blocked look-ahead when the shape allows (N % (8 cluster) == 0, K <= 152; for
+ *                   K > ~100 the K x K inverse then stays in global memory, which needs K even), 1 = per move.
+ *   "slot_replace"  0 (default): accepting an electron that is already queued flushes first (reading G7); 1: it
+ *                   replaces the column of its queue slot (M updated by a column-replacement Sherman-Morrison step),
+ *                   nothing is flushed; qmcd_sweep then runs the per-move look-ahead.
+ *   "lockstep"      0/1: the lock-step variant of PAPER.md:97-99 -- every proposal, accepted or not, takes one of the K
+ *                   slots of the window (a rejected one stands for the unchanged column, a zero column of U in Eq. 4, so
+ *                   it adds no arithmetic), and Eq. 4 is applied after every K-th PROPOSAL with rank m = the moves
+ *                   accepted in the window, 0 <= m <= K: all walkers flush in the same move.  Holds for qmcd_accept* /
+ *                   qmcd_reject and the sweeps; qmcd_flush and qmcd_set_inverse open a new window.
+ * get: those plus "threads", "smem_bytes", "m_in_smem", "blocked_ok", "max_active_clusters"; "pool" returns the pool
+ * CTAs the next sweep / flush launch gets, "tma" / "la_tma" whether that path is active for this handle.
  * get returns the value (>= 0) or a negative error. */
 int qmcd_set_option(qmcd_handle h, const char* key, int value);
 int qmcd_get_option(qmcd_handle h, const char* key);
