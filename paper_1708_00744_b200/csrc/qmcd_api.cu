@@ -28,6 +28,7 @@ struct qmcd_ctx {
     int pool_opt;             // option "pool": -1 auto (every SM the leaders leave free), 0 off, > 0 that many CTAs
     int coop;                 // option "cooperative": pooled launches ask the driver for co-residency
     QmcdTmaps tmaps;          // 4-D tensor maps of B, C, W, M for the TMA-fed flush (B re-encoded by set_inverse)
+    int tile_opt;             // option "tile_rows" for the TMA-fed flush: 0 auto, 64, 128
     int tma_opt;              // option "tma": 1 = use the TMA-fed flush when the shape allows
     bool tmaps_ok;            // C, W, M, Wk encoded (and B, B16 once an inverse is adopted)
     double* rpart; unsigned* rcnt;   // qmcd_ratio kernel scratch
@@ -127,20 +128,26 @@ static bool encode_proposals(CUtensorMap* tm, const double* base, int n_moves, i
     const cuuint32_t bd[4] = {8, 16, 4, 1};
     return encode_4d(tm, base, gd, gs, bd, false);
 }
-static bool tma_shape_ok(int N, int K) { return K <= 64 && N % 64 == 0 && N >= 128; }
+static bool tma_shape_ok(int N, int K) { return K <= 128 && N % 64 == 0 && N >= 128; }
+static bool la_shape_ok(int N, int K) { return K <= 64 && N % 64 == 0 && N >= 128; }
 static void encode_queue_tmaps(qmcd_ctx* h) {
     h->tmaps_ok = false;
     if (!tma_shape_ok(h->N, h->K)) return;
     const int N = h->N, K = h->K, rows = 8 * qmcd_tma_NB(K);
-    h->tmaps_ok = encode_view(&h->tmaps.C, h->P.C, K, N, (size_t)K * N, h->batch, 8, rows, 4, false) &&
-                  encode_view(&h->tmaps.W, h->P.W, K, N, (size_t)K * N, h->batch, 16, rows, 2, true) &&
-                  encode_view(&h->tmaps.M, h->P.M, 64, 64, (size_t)64 * 64, h->batch, 16, 64, 4, true) &&
-                  encode_view(&h->tmaps.Wk, h->P.W, K, N, (size_t)K * N, h->batch, 8, rows, 4, false);
+    h->tmaps_ok = encode_view(&h->tmaps.C, h->P.C, K, N, (size_t)K * N, h->batch, 8, rows, 4, false);
+    if (K <= 64)
+        h->tmaps_ok = h->tmaps_ok && encode_view(&h->tmaps.W, h->P.W, K, N, (size_t)K * N, h->batch, 16, rows, 2, true) &&
+                      encode_view(&h->tmaps.M, h->P.M, 64, 64, (size_t)64 * 64, h->batch, 16, 64, 4, true) &&
+                      encode_view(&h->tmaps.Wk, h->P.W, K, N, (size_t)K * N, h->batch, 8, rows, 4, false);
+    else                                       // 64 < K <= 128: the tile multiplies by Y = M W (formed by the job's first phase)
+        h->tmaps_ok = h->tmaps_ok && encode_view(&h->tmaps.Y, h->P.Y, K, N, (size_t)K * N, h->batch, 16, rows, 2, true);
 }
 static void refresh_use_tma(qmcd_ctx* h) {
     h->P.use_tma = (h->tma_opt && h->tmaps_ok && h->P.B != nullptr && h->P.mma_smem_ok && h->P.flush_path != 1 &&
                     h->smem_bytes >= qmcd_flush_tma_smem_bytes()) ? 1 : 0;
-    if (h->P.use_tma) h->P.tile_rows = QMCD_TMA_ROWS;
+    // 128-row tiles when a job then still has >= 8 of them, else 64-row tiles (more workers per job: a short flush is
+    // latency, not throughput); K > 64 runs 64-row tiles (the registers hold T for 8 rows x 128 columns per warp)
+    if (h->P.use_tma) h->P.tile_rows = (h->K <= 64 && h->N >= 1024 && h->tile_opt != 64) || (h->K <= 64 && h->tile_opt == 128) ? 128 : 64;
     h->P.la_tma = (h->la_opt && h->la_fit && h->tmaps_ok && h->P.B != nullptr && h->P.blk_ok && h->P.m_in_smem) ? 1 : 0;
 }
 
@@ -151,7 +158,7 @@ static int configure_kernel(qmcd_ctx* h, int S) {
     // the TMA look-ahead ring: K <= 64 tensor maps, column slices of whole 32-column chunks
     // (measured: it pays when a CTA's slice is long -- c2/c3/c4: +3 ... +8 % -- and costs on short ones, where the ring's
     // fill latency per block dominates: c1, N = 512, -16 %; la_opt = 2 forces it on for any shape that fits)
-    bool la = blk_shape && h->la_opt && tma_shape_ok(h->N, h->K) && (h->N / S) % 32 == 0 && h->N % S == 0 &&
+    bool la = blk_shape && h->la_opt && la_shape_ok(h->N, h->K) && (h->N / S) % 32 == 0 && h->N % S == 0 &&
               (h->N / S >= 1024 || h->la_opt == 2);
     size_t blk = blk_shape ? qmcd_blk_smem_bytes(h->K, la) : 0;
     size_t base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, blk);
@@ -360,7 +367,8 @@ extern "C" int qmcd_set_inverse(qmcd_handle h, double* Ainv_dev) {
     if (!h || !Ainv_dev || ((uintptr_t)Ainv_dev & 15)) return QMCD_EINVAL;
     if (h->state != QMCD_IDLE) return QMCD_ESTATE;
     h->P.B = Ainv_dev;
-    if (h->tmaps_ok && !(encode_view(&h->tmaps.B, Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, QMCD_TMA_ROWS, 4, false) &&
+    if (h->tmaps_ok && !(encode_view(&h->tmaps.B, Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 128, 4, false) &&
+                         encode_view(&h->tmaps.B64, Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 64, 4, false) &&
                          encode_view(&h->tmaps.B16, Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 16, 4, false)))
         h->tmaps_ok = false;
     refresh_use_tma(h);
@@ -665,8 +673,9 @@ extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
     }
     if (!strcmp(key, "tile_rows")) {               // cp.async flush only (the TMA-fed flush works on 128-row tiles)
         if ((value != 64 && value != 128) || (value == 128 && h->K > 64)) return QMCD_EINVAL;
-        if (h->P.use_tma && value != QMCD_TMA_ROWS) return QMCD_EINVAL;
+        h->tile_opt = value;
         h->P.tile_rows = value;
+        refresh_use_tma(h);
         return QMCD_OK;
     }
     if (!strcmp(key, "ratio_kernel")) {            // 0: qmcd_ratio through the cluster kernel's look-ahead (the per-move sweep's arithmetic)
@@ -684,7 +693,7 @@ extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
         if (value < 0 || value > 1) return QMCD_EINVAL;
         h->tma_opt = value;
         refresh_use_tma(h);
-        if (!h->P.use_tma && h->K <= 64) h->P.tile_rows = (h->N >= 2048) ? 128 : 64;
+        if (!h->P.use_tma && h->K <= 64) h->P.tile_rows = h->tile_opt ? h->tile_opt : ((h->N >= 2048) ? 128 : 64);
         return QMCD_OK;
     }
     if (!strcmp(key, "flush_path")) {

@@ -26,7 +26,7 @@
 
 // 4-D views, see qmcd_api.cu.  B, C, W, M: the flush (this file).  B16, V, Wk (+ C): the look-ahead ring of
 // qmcd_block.cuh -- B with 16-row boxes, the proposals of the current qmcd_sweep launch, W in the k-major view.
-struct QmcdTmaps { CUtensorMap B, C, W, M, B16, V, Wk; };
+struct QmcdTmaps { CUtensorMap B, C, W, M, B16, V, Wk, B64, Y; };   // B64: 64-row boxes of B; Y = M W (K > 64), viewed like W
 
 #define QMCD_TMA_NS 4
 #define QMCD_TMA_STAGE_BYTES 49152
@@ -36,7 +36,7 @@ struct QmcdTmaps { CUtensorMap B, C, W, M, B16, V, Wk; };
 __host__ __device__ inline size_t qmcd_flush_tma_smem_bytes() {
     return (size_t)QMCD_TMA_STAGE_OFF + QMCD_TMA_NS * QMCD_TMA_STAGE_BYTES;
 }
-__host__ __device__ inline int qmcd_tma_NB(int K) { return K <= 8 ? 1 : K <= 16 ? 2 : K <= 32 ? 4 : 8; }
+__host__ __device__ inline int qmcd_tma_NB(int K) { return K <= 8 ? 1 : K <= 16 ? 2 : K <= 32 ? 4 : K <= 64 ? 8 : 16; }
 
 __device__ __forceinline__ unsigned qmcd_su32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void qmcd_mbar_init(unsigned bar, unsigned count) {
@@ -109,20 +109,28 @@ __device__ __forceinline__ void qmcd_tma_init_barriers(unsigned char* smem) {
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 }
 
-// One tile.  `itc` = iterations this CTA has pushed through the ring so far (the same in every thread; it
-// fixes stage and mbarrier parity), updated on return.  All 256 threads; ends without a CTA barrier.
-template <int NB>
+// One tile of 64 A_T rows.  `itc` = iterations this CTA has pushed through the ring so far (the same in every
+// thread; it fixes stage and mbarrier parity), updated on return.  All 256 threads; ends without a CTA barrier.
+//   YP = false (K <= 64): the three parts above, M applied in registers.
+//   YP = true  (64 < K <= 128, NB = 16, A_T = 1): Y = M W was formed by the job's first phase; part 2 is only
+//              T = -T + E_J and part 3 multiplies by Y (tensor map TM.Y) -- 2 nk iterations, no M stage.
+template <int NB, int A_T, bool YP>
 __device__ __noinline__ void qmcd_flush_tile_tma(const QmcdDev& P, const QmcdTmaps& TM, unsigned char* smem, int b, int m, int tile,
                                                  unsigned& itc) {
-    constexpr unsigned TX_ROWS = 32768u + 2048u * NB;
+    constexpr int ROWS = 64 * A_T;
+    constexpr unsigned OFF2 = 256u * ROWS;                     // second operand of a stage, after the B tile
+    constexpr unsigned TX_ROWS = OFF2 + 2048u * NB;
     constexpr int NS = QMCD_TMA_NS;
+    constexpr bool DB = (NB <= 8);                             // double-buffered fragments while the registers allow
+    static_assert(OFF2 + 2048u * NB <= QMCD_TMA_STAGE_BYTES, "stage too small");
     const int N = P.N, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, g = lane >> 2, c = lane & 3;
-    const int nk = N / 32, total = 2 * nk + 1;
-    const int row0 = tile * QMCD_TMA_ROWS;
+    const int nk = N / 32, total = YP ? 2 * nk : 2 * nk + 1, nn0 = YP ? nk : nk + 1;
+    const int row0 = tile * ROWS, wrow = wid * 8 * A_T;
     const unsigned bar0 = qmcd_su32(smem + QMCD_TMA_BAR_OFF);
     unsigned char* st0 = smem + QMCD_TMA_STAGE_OFF;
     const unsigned it0 = itc;
     double* Bw = P.B + (size_t)b * N * N;
+    const CUtensorMap* tmB = (A_T == 2) ? &TM.B : &TM.B64;
 
     const unsigned long long pol_stream = qmcd_policy_evict_first(), pol_keep = qmcd_policy_evict_last();
     auto issue = [&](int j) {                     // one thread: the loads of iteration j of this tile
@@ -131,27 +139,27 @@ __device__ __noinline__ void qmcd_flush_tile_tma(const QmcdDev& P, const QmcdTma
         const unsigned dst = qmcd_su32(st0 + s * QMCD_TMA_STAGE_BYTES), fb = bar0 + 8 * s;
         if (j < nk) {
             qmcd_mbar_expect_tx(fb, TX_ROWS);
-            qmcd_tma_load4_hint(dst, &TM.B, 0, row0, 4 * j, b, fb, pol_stream);
-            qmcd_tma_load4_hint(dst + 32768, &TM.C, 0, 0, 4 * j, b, fb, pol_keep);
-        } else if (j == nk) {
+            qmcd_tma_load4_hint(dst, tmB, 0, row0, 4 * j, b, fb, pol_stream);
+            qmcd_tma_load4_hint(dst + OFF2, &TM.C, 0, 0, 4 * j, b, fb, pol_keep);
+        } else if (!YP && j == nk) {
             qmcd_mbar_expect_tx(fb, 32768u);
             qmcd_tma_load4_hint(dst, &TM.M, 0, 0, 0, b, fb, pol_keep);
         } else {
-            const int jj = j - nk - 1;
+            const int jj = j - nn0;
             qmcd_mbar_expect_tx(fb, TX_ROWS);
-            qmcd_tma_load4_hint(dst, &TM.B, 0, row0, 4 * jj, b, fb, pol_stream);
-            qmcd_tma_load4_hint(dst + 32768, &TM.W, 0, 0, 2 * jj, b, fb, pol_keep);
+            qmcd_tma_load4_hint(dst, tmB, 0, row0, 4 * jj, b, fb, pol_stream);
+            qmcd_tma_load4_hint(dst + OFF2, YP ? &TM.Y : &TM.W, 0, 0, 2 * jj, b, fb, pol_keep);
         }
     };
     if (tid == 0) {
 #pragma unroll
-        for (int j = 0; j < NS - 1; ++j) issue(j);            // total >= 2 * 4 + 1 > NS - 1
+        for (int j = 0; j < NS - 1; ++j) issue(j);            // total >= 2 * 4 > NS - 1
     }
 
-    // T for this warp's 16 rows: T[a][q][e] = T[row 16 wid + 8 a + g][column 8 q + 2 c + e]
-    double T[2][NB][2];
+    // T for this warp's 8 A_T rows: T[a][q][e] = T[row wrow + 8 a + g][column 8 q + 2 c + e]
+    double T[A_T][NB][2];
 #pragma unroll
-    for (int a = 0; a < 2; ++a)
+    for (int a = 0; a < A_T; ++a)
 #pragma unroll
         for (int q = 0; q < NB; ++q) { T[a][q][0] = 0.0; T[a][q][1] = 0.0; }
 
@@ -160,56 +168,82 @@ __device__ __noinline__ void qmcd_flush_tile_tma(const QmcdDev& P, const QmcdTma
         const unsigned gi = it0 + (unsigned)j, s = gi % NS, u = gi / NS;
         const unsigned char* stg = st0 + s * QMCD_TMA_STAGE_BYTES;
         qmcd_mbar_wait(bar0 + 8 * s, u & 1);
-        if (wid == (j & 7) && lane == 0) issue(j + NS - 1);                          // (j + NS - 1 < total always here)
-        const double* As = reinterpret_cast<const double*>(stg) + (wid * 16 + g) * 8 + 2 * c;
-        const double* Cs = reinterpret_cast<const double*>(stg + 32768) + g * 8 + 2 * c;
-        double2 av[2][2], bv[2][NB];
+        if (wid == (j & 7) && lane == 0 && j + NS - 1 < total) issue(j + NS - 1);
+        const double* As = reinterpret_cast<const double*>(stg) + (wrow + g) * 8 + 2 * c;
+        const double* Cs = reinterpret_cast<const double*>(stg + OFF2) + g * 8 + 2 * c;
+        if (DB) {
+            double2 av[2][A_T], bv[2][NB];
 #pragma unroll
-        for (int a = 0; a < 2; ++a) av[0][a] = qmcd_lds128(As + a * 64);
+            for (int a = 0; a < A_T; ++a) av[0][a] = qmcd_lds128(As + a * 64);
 #pragma unroll
-        for (int bt = 0; bt < NB; ++bt) bv[0][bt] = qmcd_lds128(Cs + bt * 64);
+            for (int bt = 0; bt < NB; ++bt) bv[0][bt] = qmcd_lds128(Cs + bt * 64);
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const int cur = q & 1, nxt = cur ^ 1;
-            if (q < 3) {
+            for (int q = 0; q < 4; ++q) {
+                const int cur = q & 1, nxt = cur ^ 1;
+                if (q < 3) {
 #pragma unroll
-                for (int a = 0; a < 2; ++a) av[nxt][a] = qmcd_lds128(As + (q + 1) * (QMCD_TMA_ROWS * 8) + a * 64);
+                    for (int a = 0; a < A_T; ++a) av[nxt][a] = qmcd_lds128(As + (q + 1) * (ROWS * 8) + a * 64);
 #pragma unroll
-                for (int bt = 0; bt < NB; ++bt) bv[nxt][bt] = qmcd_lds128(Cs + (q + 1) * (64 * NB) + bt * 64);
+                    for (int bt = 0; bt < NB; ++bt) bv[nxt][bt] = qmcd_lds128(Cs + (q + 1) * (64 * NB) + bt * 64);
+                }
+#pragma unroll
+                for (int bt = 0; bt < NB; ++bt)
+#pragma unroll
+                    for (int a = 0; a < A_T; ++a) qmcd_dmma(T[a][bt][0], T[a][bt][1], av[cur][a].x, bv[cur][bt].x);
+#pragma unroll
+                for (int bt = 0; bt < NB; ++bt)
+#pragma unroll
+                    for (int a = 0; a < A_T; ++a) qmcd_dmma(T[a][bt][0], T[a][bt][1], av[cur][a].y, bv[cur][bt].y);
             }
+        } else {
 #pragma unroll
-            for (int bt = 0; bt < NB; ++bt)
+            for (int q = 0; q < 4; ++q) {
+                double2 av[A_T];
 #pragma unroll
-                for (int a = 0; a < 2; ++a) qmcd_dmma(T[a][bt][0], T[a][bt][1], av[cur][a].x, bv[cur][bt].x);
+                for (int a = 0; a < A_T; ++a) av[a] = qmcd_lds128(As + q * (ROWS * 8) + a * 64);
 #pragma unroll
-            for (int bt = 0; bt < NB; ++bt)
+                for (int h = 0; h < NB; h += 8) {          // 8 n-tiles at a time: 8 fragment registers pairs live
+                    double2 bv[8];
 #pragma unroll
-                for (int a = 0; a < 2; ++a) qmcd_dmma(T[a][bt][0], T[a][bt][1], av[cur][a].y, bv[cur][bt].y);
+                    for (int bt = 0; bt < 8; ++bt) bv[bt] = qmcd_lds128(Cs + q * (64 * NB) + (h + bt) * 64);
+#pragma unroll
+                    for (int bt = 0; bt < 8; ++bt)
+#pragma unroll
+                        for (int a = 0; a < A_T; ++a) qmcd_dmma(T[a][h + bt][0], T[a][h + bt][1], av[a].x, bv[bt].x);
+#pragma unroll
+                    for (int bt = 0; bt < 8; ++bt)
+#pragma unroll
+                        for (int a = 0; a < A_T; ++a) qmcd_dmma(T[a][h + bt][0], T[a][h + bt][1], av[a].y, bv[bt].y);
+                }
+            }
         }
         __syncwarp();
         if (lane == 0) qmcd_mbar_arrive(bar0 + 8 * NS + 8 * s);                      // this warp has left stage s
     }
 
-    // ---------------- T = -T + E_J ;  T <- T M   (iteration nk: the stage holds M)
+    // ---------------- T = -T + E_J  (and, K <= 64, T <- T M: iteration nk, the stage holds M)
     {
-        const int j = nk;
-        const unsigned gi = it0 + (unsigned)j, s = gi % NS, u = gi / NS;
-        const unsigned char* stg = st0 + s * QMCD_TMA_STAGE_BYTES;
         const int* Jw = P.J + (size_t)b * P.K;
 #pragma unroll
         for (int q = 0; q < NB; ++q)
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
                 const int i = 8 * q + 2 * c + e;
-                const int jr = (i < m) ? __ldcg(Jw + i) - row0 - wid * 16 - g : -1;      // E_J[j_i, i] = 1
+                const int jr = (i < m) ? __ldcg(Jw + i) - row0 - wrow - g : -1;          // E_J[j_i, i] = 1
 #pragma unroll
-                for (int a = 0; a < 2; ++a) T[a][q][e] = ((jr == 8 * a) ? 1.0 : 0.0) - T[a][q][e];
+                for (int a = 0; a < A_T; ++a)
+                    T[a][q][e] = (YP && i >= m) ? 0.0 : ((jr == 8 * a) ? 1.0 : 0.0) - T[a][q][e];   // (YP: rows >= m of Y are stale)
             }
+    }
+    if (!YP) {
+        const int j = nk;
+        const unsigned gi = it0 + (unsigned)j, s = gi % NS, u = gi / NS;
+        const unsigned char* stg = st0 + s * QMCD_TMA_STAGE_BYTES;
         qmcd_mbar_wait(bar0 + 8 * s, u & 1);
-        if (wid == (j & 7) && lane == 0) issue(j + NS - 1);
-        double T2[2][NB][2];
+        if (wid == (j & 7) && lane == 0 && j + NS - 1 < total) issue(j + NS - 1);
+        double T2[A_T][NB][2];
 #pragma unroll
-        for (int a = 0; a < 2; ++a)
+        for (int a = 0; a < A_T; ++a)
 #pragma unroll
             for (int t = 0; t < NB; ++t) { T2[a][t][0] = 0.0; T2[a][t][1] = 0.0; }
         // M[k][n] at group (n / 16): row k, 16-byte chunk ((n % 16) / 2) ^ (k % 8), half n % 2;  k = 8q + 2c + s, n = 8t + g
@@ -227,36 +261,37 @@ __device__ __noinline__ void qmcd_flush_tile_tma(const QmcdDev& P, const QmcdTma
 #pragma unroll
             for (int t = 0; t < NB; ++t)
 #pragma unroll
-                for (int a = 0; a < 2; ++a) qmcd_dmma(T2[a][t][0], T2[a][t][1], T[a][q][0], b0[t]);
+                for (int a = 0; a < A_T; ++a) qmcd_dmma(T2[a][t][0], T2[a][t][1], T[a][q][0], b0[t]);
 #pragma unroll
             for (int t = 0; t < NB; ++t)
 #pragma unroll
-                for (int a = 0; a < 2; ++a) qmcd_dmma(T2[a][t][0], T2[a][t][1], T[a][q][1], b1[t]);
+                for (int a = 0; a < A_T; ++a) qmcd_dmma(T2[a][t][0], T2[a][t][1], T[a][q][1], b1[t]);
         }
 #pragma unroll
-        for (int a = 0; a < 2; ++a)
+        for (int a = 0; a < A_T; ++a)
 #pragma unroll
             for (int t = 0; t < NB; ++t) { T[a][t][0] = T2[a][t][0]; T[a][t][1] = T2[a][t][1]; }
         __syncwarp();
         if (lane == 0) qmcd_mbar_arrive(bar0 + 8 * NS + 8 * s);
     }
 
-    // ---------------- NN: B[tile, 32 columns] += T W[:, same]; initial values from the staged tile, results by STG
+    // ---------------- NN: B[tile, 32 columns] += T X[:, same] (X = W, or Y when YP); initial values from the staged
+    // tile, results by STG
     const int sw0 = (g ^ (2 * c)) << 4, sw1 = (g ^ (2 * c + 1)) << 4;
-    for (int j = nk + 1; j < total; ++j) {
+    for (int j = nn0; j < total; ++j) {
         const unsigned gi = it0 + (unsigned)j, s = gi % NS, u = gi / NS;
         const unsigned char* stg = st0 + s * QMCD_TMA_STAGE_BYTES;
-        const int n0 = 32 * (j - nk - 1);
+        const int n0 = 32 * (j - nn0);
         qmcd_mbar_wait(bar0 + 8 * s, u & 1);
         if (wid == (j & 7) && lane == 0 && j + NS - 1 < total) issue(j + NS - 1);
-        const double* Ds = reinterpret_cast<const double*>(stg);                     // [4 groups of 8 columns][128 rows][8]
-        const unsigned char* Ws = stg + 32768 + (2 * c) * 128;                        // [2 groups of 16 columns][8 NB rows][128 B]
-        double an[2][2][2][2];                                                       // [a][G][t][e]
+        const double* Ds = reinterpret_cast<const double*>(stg);                     // [4 groups of 8 columns][ROWS][8]
+        const unsigned char* Ws = stg + OFF2 + (2 * c) * 128;                         // [2 groups of 16 columns][8 NB rows][128 B]
+        double an[A_T][2][2][2];                                                     // [a][G][t][e]
 #pragma unroll
-        for (int a = 0; a < 2; ++a)
+        for (int a = 0; a < A_T; ++a)
 #pragma unroll
-            for (int G = 0; G < 2; ++G) {              // this lane's columns 16 G + 4 c .. + 3 of row 16 wid + 8 a + g
-                const double* p = Ds + ((2 * G + (c >> 1)) * QMCD_TMA_ROWS + wid * 16 + a * 8 + g) * 8 + 4 * (c & 1);
+            for (int G = 0; G < 2; ++G) {              // this lane's columns 16 G + 4 c .. + 3 of row wrow + 8 a + g
+                const double* p = Ds + ((2 * G + (c >> 1)) * ROWS + wrow + a * 8 + g) * 8 + 4 * (c & 1);
                 const double2 v0 = qmcd_lds128(p), v1 = qmcd_lds128(p + 2);
                 an[a][G][0][0] = v0.x; an[a][G][1][0] = v0.y; an[a][G][0][1] = v1.x; an[a][G][1][1] = v1.y;
             }
@@ -279,14 +314,14 @@ __device__ __noinline__ void qmcd_flush_tile_tma(const QmcdDev& P, const QmcdTma
 #pragma unroll
             for (int G = 0; G < 2; ++G)
 #pragma unroll
-                for (int a = 0; a < 2; ++a) {
+                for (int a = 0; a < A_T; ++a) {
                     qmcd_dmma(an[a][G][0][0], an[a][G][0][1], T[a][q][0], x0[cur][G].x);
                     qmcd_dmma(an[a][G][1][0], an[a][G][1][1], T[a][q][0], x0[cur][G].y);
                 }
 #pragma unroll
             for (int G = 0; G < 2; ++G)
 #pragma unroll
-                for (int a = 0; a < 2; ++a) {
+                for (int a = 0; a < A_T; ++a) {
                     qmcd_dmma(an[a][G][0][0], an[a][G][0][1], T[a][q][1], x1[cur][G].x);
                     qmcd_dmma(an[a][G][1][0], an[a][G][1][1], T[a][q][1], x1[cur][G].y);
                 }
@@ -294,8 +329,8 @@ __device__ __noinline__ void qmcd_flush_tile_tma(const QmcdDev& P, const QmcdTma
         __syncwarp();
         if (lane == 0) qmcd_mbar_arrive(bar0 + 8 * NS + 8 * s);                      // every read of stage s is done
 #pragma unroll
-        for (int a = 0; a < 2; ++a) {
-            const int row = row0 + wid * 16 + a * 8 + g;
+        for (int a = 0; a < A_T; ++a) {
+            const int row = row0 + wrow + a * 8 + g;
             if (row < N) {
                 double* d = Bw + (size_t)row * N + n0 + 4 * c;
 #pragma unroll

@@ -45,14 +45,20 @@ __device__ __forceinline__ void qmcd_tile_done(const QmcdDev& P, int b) {
 // (s.iflag[15] = iterations this CTA has pushed through the TMA ring), else the cp.async kernels.
 __device__ void qmcd_do_tile(const QmcdDev& P, const QmcdSmem& s, int b, int phase, int m, int tile,
                              unsigned long long job_key, unsigned long long& mf_key) {
-    if (P.use_tma && phase == QMCD_JOB_LOCAL) {
+    if (P.use_tma && (phase == QMCD_JOB_LOCAL || phase == QMCD_JOB_ROWS_Y)) {
         unsigned char* base = reinterpret_cast<unsigned char*>(s.red);
         unsigned itc = (unsigned)s.iflag[15];
-        switch (qmcd_tma_NB(P.K)) {
-            case 1: qmcd_flush_tile_tma<1>(P, *s.tm, base, b, m, tile, itc); break;
-            case 2: qmcd_flush_tile_tma<2>(P, *s.tm, base, b, m, tile, itc); break;
-            case 4: qmcd_flush_tile_tma<4>(P, *s.tm, base, b, m, tile, itc); break;
-            default: qmcd_flush_tile_tma<8>(P, *s.tm, base, b, m, tile, itc); break;
+        const int key = qmcd_tma_NB(P.K) * 4 + (P.tile_rows == 128 ? 2 : 1);
+        switch (key) {
+            case 1 * 4 + 2: qmcd_flush_tile_tma<1, 2, false>(P, *s.tm, base, b, m, tile, itc); break;
+            case 2 * 4 + 2: qmcd_flush_tile_tma<2, 2, false>(P, *s.tm, base, b, m, tile, itc); break;
+            case 4 * 4 + 2: qmcd_flush_tile_tma<4, 2, false>(P, *s.tm, base, b, m, tile, itc); break;
+            case 8 * 4 + 2: qmcd_flush_tile_tma<8, 2, false>(P, *s.tm, base, b, m, tile, itc); break;
+            case 1 * 4 + 1: qmcd_flush_tile_tma<1, 1, false>(P, *s.tm, base, b, m, tile, itc); break;
+            case 2 * 4 + 1: qmcd_flush_tile_tma<2, 1, false>(P, *s.tm, base, b, m, tile, itc); break;
+            case 4 * 4 + 1: qmcd_flush_tile_tma<4, 1, false>(P, *s.tm, base, b, m, tile, itc); break;
+            case 8 * 4 + 1: qmcd_flush_tile_tma<8, 1, false>(P, *s.tm, base, b, m, tile, itc); break;
+            default: qmcd_flush_tile_tma<16, 1, true>(P, *s.tm, base, b, m, tile, itc); break;      // 64 < K <= 128, tile_rows 64
         }
         __syncthreads();                  // every warp has left the ring (and read iflag[15])
         if (threadIdx.x == 0) s.iflag[15] = (int)itc;
@@ -113,7 +119,7 @@ template <bool MS>
 __device__ void qmcd_flush_phase(const QmcdDev& P, const QmcdSmem& s, cg::cluster_group& cl,
                                  const QmcdWalker& w, int m, bool writeback = true) {
     if (writeback) qmcd_writeback_M<MS>(P, s, w, m);
-    if (P.use_tma && qmcd_flush_use_mma(P)) qmcd_zero_pad_M(P, w, m);
+    if (P.use_tma && P.K <= 64 && qmcd_flush_use_mma(P)) qmcd_zero_pad_M(P, w, m);
     __threadfence();
     qmcd_fence_proxy_async();              // queue rows / M written above are read through TMA by the flush
     if (P.S > 1) cl.sync(); else __syncthreads();

@@ -566,6 +566,11 @@ def test_randomized_shapes_seeds_modes_and_launch_splits(qmcd):
     (192, 5, 3, 1, "tma", -1, 1.0),         # K not a multiple of 8: queue rows past K are zero-filled by TMA
     (1024, 64, 2, 8, "tma", -1, 0.99),      # clusters of 8: 15 fit, 13 of them pool
     (1024, 40, 2, 2, "tma", -1, 0.3),       # NB = 8 with ranks 33 ... 40 and low-rank final flushes
+    (512, 32, 4, 2, "tma128", -1, 0.9),     # TMA-fed tiles of 128 rows forced on a small N (default there: 64 rows)
+    (2048, 64, 2, 1, "tma64", -1, 0.99),    # ... and 64-row TMA tiles forced on a large N
+    (512, 96, 2, 4, "tma", -1, 0.9),        # 64 < K <= 128: Y = M W job (cp.async), then 64-row TMA tiles multiplying by Y
+    (1024, 128, 3, 1, "tma", -1, 0.99),     # K = 128, full rank, blocked look-ahead with M in global memory
+    (256, 100, 2, 2, "tma", -1, 0.5),       # K = 100 (not a multiple of 8), ranks 93 ... 100
     (128, 32, 140, 1, "tma", -1, 0.8),      # 140 leaders + 8 pool CTAs, one tile per job
     (128, 32, 140, 1, "cp64", -1, 0.8),
 ])
@@ -577,11 +582,11 @@ def test_pool_flush_jobs_match_oracle(qmcd, N, K, batch, cluster, path, pool, p)
     wl = inputs.make_workload(batch, N, n_moves=min(2 * N, 700) + K + 3, seed=61)
     mask = wl.bernoulli_mask(p)
     Bo = wl.Ainv.copy(); Ro, acco, _ = oracle.run(2, Bo, K, wl.proposals, mask=mask)
-    kw = dict(tma=1) if path == "tma" else dict(tma=0, tile_rows=int(path[2:]))
+    kw = dict(tma=1) if path == "tma" else dict(tma=1, tile_rows=int(path[3:])) if path.startswith("tma") else dict(tma=0, tile_rows=int(path[2:]))
     g = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, pool=pool,
                   split=[wl.n_moves // 3, wl.n_moves // 3 + 5], **kw)
     assert g["status"] == 0 and g["S"] == cluster
-    assert g["tma"] == (1 if path == "tma" else 0)
+    assert g["tma"] == (1 if path.startswith("tma") else 0)
     assert g["pool"] > 0 and g["pool"] % cluster == 0
     assert np.array_equal(g["acc"], acco)
     assert _rel(g["R"], Ro) <= RTOL_RATIO
