@@ -45,6 +45,7 @@ extern "C" {
 #define QMCD_ECUDA     (-3)   /* CUDA runtime/driver error (see qmcd_strerror)     */
 #define QMCD_ESINGULAR (-4)   /* device status: accept of a move with R==0/non-finite */
 #define QMCD_ENOMEM    (-5)   /* host allocation failed                             */
+#define QMCD_ELIMIT    (-6)   /* size beyond a fixed limit of the entry point (qmcd_invert_static) */
 
 typedef struct qmcd_ctx* qmcd_handle;   /* opaque */
 
@@ -173,6 +174,19 @@ size_t qmcd_sweep_host_min_staging(int N, int batch);
 size_t qmcd_invert_scratch_bytes(int N, int batch);
 int qmcd_invert(qmcd_handle h, const double* A_dev, double* Ainv_dev,
                 void* scratch_dev, size_t scratch_bytes, int* info_dev);
+
+/* qmcd_invert for callers that may not allocate device memory at all (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): the same kernel, with its scratch in a file-scope
+ * `static __device__` array of qmcd_invert_static_max_bytes() = 1 MiB that every GPU loading the library holds
+ * until exit.  Inputs and outputs are still the caller's.  Shapes whose qmcd_invert_scratch_bytes(N, batch)
+ * exceed the array are rejected with QMCD_ELIMIT (qmcd_strerror names the sizes); every BASELINE.json shape
+ * fits.  The call allocates nothing (no cudaMalloc / cudaFree / allocating library routine) and, like
+ * qmcd_invert, only enqueues work on the handle's stream.  ALL calls on a device share the one array, which
+ * keeps the last call's contents (this call clears what it uses first): two calls that overlap on the GPU --
+ * different streams or handles without an ordering between them -- RACE; serialise them.  The handle's device
+ * must be current.  Other errors as qmcd_invert. */
+size_t qmcd_invert_static_max_bytes(void);
+int qmcd_invert_static(qmcd_handle h, const double* A_dev, double* Ainv_dev, int* info_dev);
 
 /* Tuning / introspection (IDLE only).  set:
  *   "cluster"       CTAs per LEADER cluster (1, 2, 4, 8, 16; other values: QMCD_EINVAL).  Cluster b of the grid leads

@@ -10,7 +10,7 @@ import os
 
 from . import buildlib
 
-OK, EINVAL, ESTATE, ECUDA, ESINGULAR, ENOMEM = 0, -1, -2, -3, -4, -5
+OK, EINVAL, ESTATE, ECUDA, ESINGULAR, ENOMEM, ELIMIT = 0, -1, -2, -3, -4, -5, -6
 
 # name -> (restype, argtypes); mirrors include/qmcd.h one to one
 _vp, _ci, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
@@ -34,6 +34,8 @@ SYMBOLS = {
     "qmcd_sweep_host_min_staging": (_sz, [_ci, _ci]),
     "qmcd_invert_scratch_bytes": (_sz, [_ci, _ci]),
     "qmcd_invert": (_ci, [_vp, _vp, _vp, _vp, _sz, _vp]),
+    "qmcd_invert_static_max_bytes": (_sz, []),
+    "qmcd_invert_static": (_ci, [_vp, _vp, _vp, _vp]),
     "qmcd_set_option": (_ci, [_vp, ctypes.c_char_p, _ci]),
     "qmcd_get_option": (_ci, [_vp, ctypes.c_char_p]),
     "qmcd_probe_fp64": (_ci, [_ci, _ci, _vp, ctypes.POINTER(ctypes.c_double)]),
@@ -238,6 +240,15 @@ class Qmcd:
                                  scratch.data_ptr() + off, need, _ptr(info, torch.int32)), "qmcd_invert")
         self._keep = scratch          # alive until the next call (the work is only enqueued)
         return Ainv, info
+
+    def invert_static(self, A, Ainv, info):
+        """qmcd_invert_static: the same inversion with the library's static device scratch (allocates nothing --
+        neither does this wrapper: Ainv and info come from the caller).  Raises QmcdError(ELIMIT) past 1 MiB."""
+        import torch
+        if tuple(A.shape) != (self.batch, self.N, self.N) or tuple(Ainv.shape) != tuple(A.shape):
+            raise ValueError("A and Ainv must be [batch][N][N]")
+        _chk(self._L.qmcd_invert_static(self._h, _ptr(A, torch.float64), _ptr(Ainv, torch.float64),
+                                        _ptr(info, torch.int32)), "qmcd_invert_static")
 
     def set_option(self, key: str, value: int):
         _chk(self._L.qmcd_set_option(self._h, key.encode(), int(value)), f"qmcd_set_option({key})")

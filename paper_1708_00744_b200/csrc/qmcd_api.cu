@@ -5,6 +5,7 @@
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
+#include <mutex>
 #include <new>
 
 #include "../../include/qmcd.h"
@@ -595,6 +596,49 @@ extern "C" int qmcd_invert(qmcd_handle h, const double* A_dev, double* Ainv_dev,
     return QMCD_OK;
 }
 
+// ---- qmcd_invert_static: the same inversion for callers that may not allocate (CUDA graph capture, serving loops,
+// harnesses that forbid cudaMalloc): the scratch of qmcd_invert lives in a file-scope device array instead of a
+// caller buffer.  Every GPU that loads the library holds the array until exit.  In HOST code the array's name is
+// a host-side stand-in, not a device address: the address is resolved once per device, with that device current,
+// by cudaGetSymbolAddress, and that pointer is what the kernel gets.
+#define QMCD_INVERT_STATIC_BYTES (1 << 20)        // 1 MiB: every BASELINE.json shape fits (c2, the largest, needs 459 KB)
+#define QMCD_MAX_DEVICES 64
+static __device__ __align__(256) unsigned char qmcd_invert_static_scratch[QMCD_INVERT_STATIC_BYTES];
+static void* g_static_scratch_ptr[QMCD_MAX_DEVICES];        // per device; nullptr = not resolved yet
+static std::mutex g_static_scratch_mutex;
+
+extern "C" size_t qmcd_invert_static_max_bytes(void) { return QMCD_INVERT_STATIC_BYTES; }
+
+extern "C" int qmcd_invert_static(qmcd_handle h, const double* A_dev, double* Ainv_dev, int* info_dev) {
+    if (!h || !A_dev || !Ainv_dev) return QMCD_EINVAL;
+    const size_t need = qmcd_invert_scratch_bytes(h->N, h->batch);
+    if (need == 0) return QMCD_EINVAL;
+    if (need > QMCD_INVERT_STATIC_BYTES) {
+        snprintf(g_last_error, sizeof(g_last_error),
+                 "qmcd_invert_static: N = %d, batch = %d needs %zu bytes of scratch, the static array holds %d "
+                 "(use qmcd_invert with a caller buffer)", h->N, h->batch, need, QMCD_INVERT_STATIC_BYTES);
+        memcpy(h->last_cuda_error, g_last_error, sizeof(g_last_error));
+        return QMCD_ELIMIT;
+    }
+    int dev = 0;
+    CK(h, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= QMCD_MAX_DEVICES) return QMCD_EINVAL;
+    void* ptr = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_static_scratch_mutex);
+        if (!g_static_scratch_ptr[dev]) {                     // set-up, once per device, that device current
+            void* p = nullptr;
+            CK(h, cudaGetSymbolAddress(&p, qmcd_invert_static_scratch));
+            g_static_scratch_ptr[dev] = p;
+        }
+        ptr = g_static_scratch_ptr[dev];
+    }
+    // the array keeps the last call's contents: clear the part this call uses (the kernel writes its pivot and
+    // candidate arrays before reading them; the per-walker info words must start at zero)
+    CK(h, cudaMemsetAsync(ptr, 0, need, h->stream));
+    return qmcd_invert(h, A_dev, Ainv_dev, ptr, need, info_dev);
+}
+
 extern "C" size_t qmcd_sweep_host_min_staging(int N, int batch) {
     if (N < 1 || batch < 1) return 0;
     // two buffers of one move each
@@ -756,6 +800,7 @@ extern "C" const char* qmcd_strerror(int code) {
         case QMCD_ECUDA: return g_last_error[0] ? g_last_error : "CUDA error";
         case QMCD_ESINGULAR: return "accepted a move with R == 0 or non-finite R (singular)";
         case QMCD_ENOMEM: return "out of host memory";
+        case QMCD_ELIMIT: return g_last_error[0] ? g_last_error : "size exceeds a fixed limit of this entry point";
         default: return "unknown error";
     }
 }

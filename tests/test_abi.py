@@ -39,6 +39,15 @@ def test_invert_scratch_bytes_validation(lib):
     assert lib.qmcd_invert_scratch_bytes(20000, 1) == 0     # two rows + the gather no longer fit in shared memory
 
 
+def test_invert_static_host_side(lib):
+    assert lib.qmcd_invert_static_max_bytes() == 1 << 20
+    assert lib.qmcd_invert_static(None, None, None, None) == binding.EINVAL
+    assert b"limit" in lib.qmcd_strerror(binding.ELIMIT)
+    # every BASELINE.json shape fits the static array
+    for N, batch in [(64, 1), (512, 16), (1024, 64), (2048, 32), (4096, 8)]:
+        assert 0 < lib.qmcd_invert_scratch_bytes(N, batch) <= lib.qmcd_invert_static_max_bytes()
+
+
 def test_workspace_bytes_validation(lib):
     assert lib.qmcd_workspace_bytes(64, 4, 1) > 2 * 4 * 64 * 8
     assert lib.qmcd_workspace_bytes(0, 1, 1) == 0
