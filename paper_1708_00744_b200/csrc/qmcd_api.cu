@@ -123,10 +123,10 @@ static bool encode_view(CUtensorMap* tm, double* base, int rows, int N, size_t b
     return encode_4d(tm, base, gd, gs, bd, swizzle);
 }
 // The proposals of one qmcd_sweep launch, [n_moves][batch][N], seen as {8, n_moves, N / 8, batch}: row t of walker b
-static bool encode_proposals(CUtensorMap* tm, const double* base, int n_moves, int N, int batch) {
+static bool encode_proposals(CUtensorMap* tm, const double* base, int n_moves, int N, int batch, int box_rows) {
     const cuuint64_t gd[4] = {8, (cuuint64_t)n_moves, (cuuint64_t)(N / 8), (cuuint64_t)batch};
     const cuuint64_t gs[3] = {(cuuint64_t)batch * N * 8, 64, (cuuint64_t)N * 8};
-    const cuuint32_t bd[4] = {8, 16, 4, 1};
+    const cuuint32_t bd[4] = {8, (cuuint32_t)box_rows, 2, 1};
     return encode_4d(tm, base, gd, gs, bd, false);
 }
 static bool tma_shape_ok(int N, int K) { return K <= 128 && N % 64 == 0 && N >= 128; }
@@ -139,7 +139,8 @@ static void encode_queue_tmaps(qmcd_ctx* h) {
     if (K <= 64)
         h->tmaps_ok = h->tmaps_ok && encode_view(&h->tmaps.W, h->P.W, K, N, (size_t)K * N, h->batch, 16, rows, 2, true) &&
                       encode_view(&h->tmaps.M, h->P.M, 64, 64, (size_t)64 * 64, h->batch, 16, 64, 4, true) &&
-                      encode_view(&h->tmaps.Wk, h->P.W, K, N, (size_t)K * N, h->batch, 8, rows, 4, false);
+                      encode_view(&h->tmaps.W32, h->P.W, K, N, (size_t)K * N, h->batch, 8, 32, 2, false) &&
+                      encode_view(&h->tmaps.C32, h->P.C, K, N, (size_t)K * N, h->batch, 8, 32, 2, false);
     else                                       // 64 < K <= 128: the tile multiplies by Y = M W (formed by the job's first phase)
         h->tmaps_ok = h->tmaps_ok && encode_view(&h->tmaps.Y, h->P.Y, K, N, (size_t)K * N, h->batch, 16, rows, 2, true);
 }
@@ -156,21 +157,19 @@ static int configure_kernel(qmcd_ctx* h, int S) {
     const size_t cap = 227 * 1024;
     // blocked look-ahead: 16-byte vector access to every slice, <= 40 output tiles
     const bool blk_shape = h->N >= QMCD_TB && (h->N % (8 * S) == 0) && (2 * ((h->K + 7) / 8) + 2 <= 8 * QMCD_BLK_MAXU);
-    // the TMA look-ahead ring: K <= 64 tensor maps, column slices of whole 32-column chunks
-    // (measured: it pays when a CTA's slice is long -- c2/c3/c4: +3 ... +8 % -- and costs on short ones, where the ring's
-    // fill latency per block dominates: c1, N = 512, -16 %; la_opt = 2 forces it on for any shape that fits)
-    bool la = blk_shape && h->la_opt && la_shape_ok(h->N, h->K) && (h->N / S) % 32 == 0 && h->N % S == 0 &&
-              (h->N / S >= 1024 || h->la_opt == 2);
-    size_t blk = blk_shape ? qmcd_blk_smem_bytes(h->K, la) : 0;
+    // the TMA look-ahead ring (super-blocks, qmcd_superblock.cuh): K <= 64 tensor maps, column slices of whole 16-column chunks
+    // (measured against the LDG / cp.async strips of qmcd_block.cuh: c1 +11 %, c2 +21 %, c3 +8 %, c4 +13 %)
+    bool la = blk_shape && h->la_opt && la_shape_ok(h->N, h->K) && (h->N / S) % QMCD_SB_CW == 0 && h->N % S == 0;
+    size_t blk = blk_shape ? (la ? qmcd_sb_smem_bytes(h->K) : qmcd_blk_smem_bytes(h->K)) : 0;
     size_t base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, blk);
-    if (la && base > cap) { la = false; blk = qmcd_blk_smem_bytes(h->K, false); base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, blk); }
+    if (la && base > cap) { la = false; blk = qmcd_blk_smem_bytes(h->K); base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, blk); }
     h->la_fit = la;
     h->P.m_in_smem = 1; h->P.blk_ok = blk_shape ? 1 : 0;
     if (base > cap) {
         // M does not fit beside the blocked look-ahead's area: keep the blocked look-ahead and leave M in global memory
         // (staged 16 rows at a time, qmcd_blk_xy_global) when K is even and small enough for its register tile
         h->la_fit = false;
-        const size_t nb = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, false, qmcd_blk_smem_bytes(h->K, false));
+        const size_t nb = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, false, qmcd_blk_smem_bytes(h->K));
         if (blk_shape && h->K % 2 == 0 && h->K <= 16 * QMCD_BLK_YU && nb <= cap) { base = nb; h->P.m_in_smem = 0; h->P.blk_ok = 1; }
         else {
             base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, 0); h->P.blk_ok = 0;
@@ -272,9 +271,19 @@ static int launch(qmcd_ctx* h, QmcdArgs& a, bool with_pool) {
 // hides one walker's look-ahead behind the others' flushes, so small clusters (more pool CTAs,
 // no DSMEM exchange) win; with few walkers the chain is exposed and a larger S shortens it.
 static int default_S(int N, int K, int batch, int cap) {
+    // measured with the super-block look-ahead (K = 64, 99 % acceptance, fraction of the DMMA peak for S = 1/2/4/8/16):
+    // 1 walker N = 2048: .058/.065/.070/.072/.073, N = 8192: .26/.29/.32/.34/.34; 4 walkers N = 2048: .22/.24/.26/.27;
+    // 16 walkers N = 1024: .38/.39/.41, N = 512 (c1, K = 32): .18/.19/.20; 8 walkers N = 4096 (c4): .84/.66/.70 -- there a
+    // tile takes longer than a window's look-ahead and larger clusters lock the walkers' flushes in step (pool idle
+    // during the look-aheads); 32 and 64 walkers (c3, c2): the pool hides the look-ahead, S = 1
     int s = 1;
-    if (batch <= 4) s = 8; else if (batch <= 16) s = 2;
-    if ((long long)N * batch <= 16384) s *= 2;     // small problems: the flush is short, the chain dominates
+    if (K <= 64) {
+        if (batch <= 4) s = 8; else if (batch <= 16) s = 4;
+        if (batch > 4 && (long long)N * batch >= 32768) s = 1;
+    } else {                                       // the 16-proposal blocks of qmcd_block.cuh / the per-move look-ahead
+        if (batch <= 4) s = 8; else if (batch <= 16) s = 2;
+        if ((long long)N * batch <= 16384) s *= 2;
+    }
     // K > 152 (or odd K > 64) runs the per-move look-ahead (one cluster barrier per proposal, 2m + 2 streamed rows): a
     // latency chain that shortens with S (measured with it: c3 K=128 S=1/2/4 -> 0.27/0.38/0.33 of the DMMA peak; c4 K=256
     // S=2/4/8 -> 0.12/0.16/0.18).  64 < K <= 152, K even, keeps the blocked look-ahead with M in global memory (c3 K=128
@@ -370,7 +379,9 @@ extern "C" int qmcd_set_inverse(qmcd_handle h, double* Ainv_dev) {
     h->P.B = Ainv_dev;
     if (h->tmaps_ok && !(encode_view(&h->tmaps.B, Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 128, 4, false) &&
                          encode_view(&h->tmaps.B64, Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 64, 4, false) &&
-                         encode_view(&h->tmaps.B16, Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 16, 4, false)))
+                         encode_view(&h->tmaps.Bs[0], Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 16, 2, false) &&
+                         encode_view(&h->tmaps.Bs[1], Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 32, 2, false) &&
+                         encode_view(&h->tmaps.Bs[2], Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 64, 2, false)))
         h->tmaps_ok = false;
     refresh_use_tma(h);
     CK(h, cudaMemsetAsync(h->P.m, 0, (size_t)h->batch * 4, h->stream));
@@ -531,7 +542,9 @@ extern "C" int qmcd_sweep(qmcd_handle h, int j_begin, int n_moves,
     QmcdArgs a = base_args(h, QMCD_MODE_SWEEP);
     a.j_begin = j_begin; a.n_moves = n_moves; a.v = proposals_dev;
     a.mask = mask_dev; a.uniforms = uniforms_dev; a.R_out = R_out_dev; a.acc_out = acc_out_dev;
-    if (h->P.la_tma && !encode_proposals(&h->tmaps.V, proposals_dev, n_moves, h->N, h->batch)) { h->la_opt = 0; refresh_use_tma(h); a.P = h->P; }
+    if (h->P.la_tma && !(encode_proposals(&h->tmaps.Vs[0], proposals_dev, n_moves, h->N, h->batch, 16) &&
+                         encode_proposals(&h->tmaps.Vs[1], proposals_dev, n_moves, h->N, h->batch, 32) &&
+                         encode_proposals(&h->tmaps.Vs[2], proposals_dev, n_moves, h->N, h->batch, 64))) { h->la_opt = 0; refresh_use_tma(h); a.P = h->P; }
     // (the blocked look-ahead with M in global memory has no lock-step variant: that combination runs per move)
     a.blocked = (h->lookahead != 1 && !h->P.slot_replace && h->P.blk_ok && (h->P.m_in_smem || !h->P.lockstep) &&
                  (((uintptr_t)proposals_dev & 15) == 0)) ? 1 : 0;

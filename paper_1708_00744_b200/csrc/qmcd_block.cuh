@@ -25,14 +25,10 @@
 __host__ __device__ inline int qmcd_blk_Kp(int K) { return (K + 7) & ~7; }
 __host__ __device__ inline int qmcd_blk_RL(int K) { return 2 * qmcd_blk_Kp(K) + QMCD_TB; }
 // As | recv[16][RL] | G[16][RL] | ub[16] | Rb[16] | Z[2][16][16] | Xm[Kp][16] | Ym[16][Kp] | Um[Kp][16]
-// As = [2][32][LDA] (cp.async staging of the left operands) or, with the TMA look-ahead, the ring of
-// QMCD_LA_NS stages of qmcd_la_stage_bytes(K) bytes (all four operands)
-__host__ __device__ inline size_t qmcd_blk_as_doubles(int K, bool la_tma) {
-    const size_t a = (size_t)2 * 32 * QMCD_BLK_LDA, r = la_tma ? QMCD_LA_NS * qmcd_la_stage_bytes(K) / 8 : 0;
-    return r > a ? r : a;
-}
-__host__ __device__ inline size_t qmcd_blk_smem_bytes(int K, bool la_tma) {
-    return (qmcd_blk_as_doubles(K, la_tma) + (size_t)2 * QMCD_TB * qmcd_blk_RL(K) + 32 + 2 * QMCD_TB * QMCD_TB + 3 * (size_t)QMCD_TB * qmcd_blk_Kp(K) + 8) * 8;
+// As = [2][32][LDA] (cp.async staging of the left operands)
+__host__ __device__ inline size_t qmcd_blk_as_doubles() { return (size_t)2 * 32 * QMCD_BLK_LDA; }
+__host__ __device__ inline size_t qmcd_blk_smem_bytes(int K) {
+    return (qmcd_blk_as_doubles() + (size_t)2 * QMCD_TB * qmcd_blk_RL(K) + 32 + 2 * QMCD_TB * QMCD_TB + 3 * (size_t)QMCD_TB * qmcd_blk_Kp(K) + 8) * 8;
 }
 
 struct QmcdBlk {
@@ -48,10 +44,10 @@ struct QmcdBlk {
     double* Rb;     // [16]          ratios of the block (written to R_out at the block's end)
 };
 
-__device__ inline QmcdBlk qmcd_blk_carve(double* base, int K, bool la_tma) {
+__device__ inline QmcdBlk qmcd_blk_carve(double* base, int K) {
     QmcdBlk x;
     const int RL = qmcd_blk_RL(K);
-    x.As = base; base += qmcd_blk_as_doubles(K, la_tma);
+    x.As = base; base += qmcd_blk_as_doubles();
     x.recv = base; base += QMCD_TB * RL;
     x.G = base; base += QMCD_TB * RL;
     x.ub = base; base += 16;
@@ -235,133 +231,12 @@ __device__ __noinline__ void qmcd_blk_strips(const QmcdArgs& A, const QmcdSmem& 
     qmcd_blk_reduce(P, x, cl, w, acc, nu, nP);
 }
 
-// ---------------------------------------------------------------------------
-// The same strips with every operand streamed through a TMA ring (P.la_tma): per chunk of 32 columns of this
-// CTA's slice one stage holds  B0[j0 .. j0+15, chunk] | V[t0 .. t0+15, chunk] | C[0 .. 8NB), chunk] | W[0 .. 8NB), chunk],
-// each as [4 k-groups][rows][8] (conflict-free 16-byte fragment loads).  Thread 0 issues the loads of chunk
-// kc + 2 at the top of chunk kc; the warps only run LDS + DMMA.  The block must not wrap (j0 + L <= N: the
-// caller cuts it) so that the 16 rows of B0 are one box.  `itc` = chunks this CTA has pushed through the ring.
-// ---------------------------------------------------------------------------
-template <int NB>
-__device__ __noinline__ void qmcd_blk_strips_tma(const QmcdArgs& A, const QmcdSmem& s, const QmcdBlk& x, cg::cluster_group& cl,
-                                                 const QmcdWalker& w, int t0, int L, int m0, unsigned& itc) {
-    constexpr int NS = QMCD_LA_NS;
-    constexpr unsigned STAGE = 8192 + 4096 * NB;               // bytes
-    const QmcdDev& P = A.P;
-    const QmcdTmaps& TM = *s.tm;
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, g = lane >> 2, c = lane & 3;
-    const int len = w.khi - w.klo, nch = len / 32;
-    const int nP = (m0 + 7) >> 3, U = 2 * nP + 2;
-    const int j0 = (A.j_begin + t0) % P.N;
-    unsigned char* smem = reinterpret_cast<unsigned char*>(s.red);
-    const unsigned bar0 = qmcd_su32(smem + QMCD_LA_BAR_OFF);
-    unsigned char* ring = reinterpret_cast<unsigned char*>(x.As);
-    const unsigned it0 = itc;
-    (void)L;
-    const unsigned long long pol_keep = qmcd_policy_evict_last();
-    auto issue = [&](int kc) {
-        const unsigned gi = it0 + (unsigned)kc, st = gi % NS, u = gi / NS;
-        if (u > 0) qmcd_mbar_wait(bar0 + 8 * NS + 8 * st, (u - 1) & 1);
-        const unsigned dst = qmcd_su32(ring + st * STAGE), fb = bar0 + 8 * st;
-        const int kg = (w.klo >> 3) + 4 * kc;
-        qmcd_mbar_expect_tx(fb, STAGE);
-        qmcd_tma_load4(dst, &TM.B16, 0, j0, kg, w.b, fb);
-        qmcd_tma_load4(dst + 4096, &TM.V, 0, t0, kg, w.b, fb);
-        qmcd_tma_load4_hint(dst + 8192, &TM.C, 0, 0, kg, w.b, fb, pol_keep);
-        qmcd_tma_load4_hint(dst + 8192 + 2048 * NB, &TM.Wk, 0, 0, kg, w.b, fb, pol_keep);
-    };
-    if (tid == 0) {
-        for (int kc = 0; kc < NS - 1 && kc < nch; ++kc) issue(kc);
-    }
-    // my units u = wid + 8 i: right-operand offset (doubles, within a stage, at k-group 0), its k-group stride, left operand
-    int nu = 0, roff[QMCD_BLK_MAXU], rqs[QMCD_BLK_MAXU], lsel[QMCD_BLK_MAXU];
-#pragma unroll
-    for (int i = 0; i < QMCD_BLK_MAXU; ++i) {
-        const int u = wid + 8 * i;
-        roff[i] = 0; rqs[i] = 0; lsel[i] = 0;
-        if (u < U) {
-            nu = i + 1;
-            if (u < nP) { roff[i] = 1024 + (8 * u + g) * 8 + 2 * c; rqs[i] = 64 * NB; lsel[i] = 0; }                         // P: B0 rows x C
-            else if (u < 2 * nP) { roff[i] = 1024 + 256 * NB + (8 * (u - nP) + g) * 8 + 2 * c; rqs[i] = 64 * NB; lsel[i] = 1; }   // Q: V x W
-            else { roff[i] = 512 + (8 * (u - 2 * nP) + g) * 8 + 2 * c; rqs[i] = 128; lsel[i] = 0; }                           // D: B0 rows x V
-        }
-    }
-    double acc[QMCD_BLK_MAXU][2][2];
-#pragma unroll
-    for (int i = 0; i < QMCD_BLK_MAXU; ++i) { acc[i][0][0] = acc[i][0][1] = acc[i][1][0] = acc[i][1][1] = 0.0; }
-    for (int kc = 0; kc < nch; ++kc) {
-        const unsigned gi = it0 + (unsigned)kc, st = gi % NS, u = gi / NS;
-        const double* stg = reinterpret_cast<const double*>(ring + st * STAGE);
-        qmcd_mbar_wait(bar0 + 8 * st, u & 1);
-        if (tid == 0 && kc + NS - 1 < nch) issue(kc + NS - 1);
-        const double* Ls = stg + g * 8 + 2 * c;                 // left operands: B0 rows at +0, V rows at +512; row block a at +64
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            double2 lb[2], lv[2];
-#pragma unroll
-            for (int a = 0; a < 2; ++a) { lb[a] = qmcd_lds128(Ls + q * 128 + a * 64); lv[a] = qmcd_lds128(Ls + 512 + q * 128 + a * 64); }
-#pragma unroll
-            for (int i = 0; i < QMCD_BLK_MAXU; ++i) {
-                if (i < nu) {
-                    const double2 bv = qmcd_lds128(stg + roff[i] + q * rqs[i]);
-                    const double2 l0 = lsel[i] ? lv[0] : lb[0], l1 = lsel[i] ? lv[1] : lb[1];
-                    qmcd_dmma(acc[i][0][0], acc[i][0][1], l0.x, bv.x);
-                    qmcd_dmma(acc[i][1][0], acc[i][1][1], l1.x, bv.x);
-                    qmcd_dmma(acc[i][0][0], acc[i][0][1], l0.y, bv.y);
-                    qmcd_dmma(acc[i][1][0], acc[i][1][1], l1.y, bv.y);
-                }
-            }
-        }
-        __syncwarp();
-        if (lane == 0) qmcd_mbar_arrive(bar0 + 8 * NS + 8 * st);
-    }
-    itc = it0 + (unsigned)nch;
-    __syncthreads();
-    qmcd_blk_reduce(P, x, cl, w, acc, nu, nP);
-}
-
-// Queue append of a block's accepted moves by bulk asynchronous copies (P.la_tma): rows v -> C[slot] and
-// B0[j,:] -> W[slot] (this CTA's column slice of each) bounce through the look-ahead ring's memory, several
-// rows per wave.  Thread 0 only; the caller barriers afterwards.  `phase` = waves this CTA has issued so far.
-__device__ __noinline__ void qmcd_blk_append_bulk(const QmcdArgs& A, const QmcdSmem& s, const QmcdBlk& x, const QmcdWalker& w,
-                                                     int t, int j0, int m0, unsigned accmask, int na, unsigned& phase) {
-    const QmcdDev& P = A.P;
-    const int N = P.N, len = w.khi - w.klo;
-    const unsigned rowbytes = (unsigned)len * 8u;
-    const unsigned ring_bytes = (unsigned)(QMCD_LA_NS * qmcd_la_stage_bytes(P.K));
-    const int per_wave = max(1, (int)(ring_bytes / rowbytes));
-    const unsigned bar = qmcd_su32(reinterpret_cast<unsigned char*>(s.red) + QMCD_LA_APP_BAR_OFF);
-    const unsigned ring = qmcd_su32(x.As);
-    const int nrows = 2 * na;
-    for (int r0 = 0; r0 < nrows; r0 += per_wave) {
-        const int cnt = min(per_wave, nrows - r0);
-        qmcd_mbar_expect_tx(bar, (unsigned)cnt * rowbytes);
-        for (int i = 0; i < cnt; ++i) {
-            const int r = r0 + i, e = r >> 1;
-            const int al = __fns(accmask, 0, e + 1);
-            const double* src = (r & 1) ? w.B + (size_t)((j0 + al) % N) * N + w.klo
-                                        : A.v + ((size_t)(t + al) * P.batch + w.b) * N + w.klo;
-            qmcd_bulk_load(ring + (unsigned)i * rowbytes, src, rowbytes, bar);
-        }
-        qmcd_mbar_wait(bar, phase & 1);
-        ++phase;
-        for (int i = 0; i < cnt; ++i) {
-            const int r = r0 + i, e = r >> 1;
-            double* dst = ((r & 1) ? w.W : w.C) + (size_t)(m0 + e) * N + w.klo;
-            qmcd_bulk_store(dst, ring + (unsigned)i * rowbytes, rowbytes);
-        }
-        qmcd_bulk_commit();
-        qmcd_bulk_wait_read0();             // the ring may be overwritten by the next wave / the next block's loads
-    }
-    qmcd_bulk_wait0();                      // the rows are written before the caller's barrier
-}
-
 // X = M0 Q^T and Y = P M0 of one block with M in GLOBAL memory (K too large for a shared-memory copy): M0 is staged
 // 16 rows at a time into the (idle) operand area x.As; thread (il, tl) forms X[p0 + il][tl], thread (t, bq) keeps
 // Y[t][bq + 16 u] in registers over all panels.  Needs K even (16-byte row alignment) and K <= 16 * QMCD_BLK_YU.
 #define QMCD_BLK_YU 10
-__device__ __noinline__ void qmcd_blk_xy_global(const QmcdDev& P, const QmcdBlk& x, const QmcdWalker& w, int m0, int L) {
-    const int tid = threadIdx.x, K = P.K, Kp = qmcd_blk_Kp(K), RL = qmcd_blk_RL(K), ldg = P.ldMg;
+__device__ __noinline__ void qmcd_blk_xy_global(const QmcdDev& P, const QmcdBlk& x, const QmcdWalker& w, int m0, int L, int RL) {
+    const int tid = threadIdx.x, K = P.K, Kp = qmcd_blk_Kp(K), ldg = P.ldMg;
     const int ldp = Kp + 2, m0e = (m0 + 1) & ~1, vpr = m0e >> 1;
     double* Mp = x.As;
     const int t = tid >> 4, bq = tid & 15;
@@ -406,12 +281,9 @@ __device__ __noinline__ void qmcd_blk_xy_global(const QmcdDev& P, const QmcdBlk&
 }
 
 // ---------------------------------------------------------------------------
-// The sweep loop in blocks (M in shared memory, replicated in every CTA).
-// Returns the queue length at the end.  Every CTA of the cluster runs the same
-// code on the same reduced numbers, so decisions agree without communication.
-//
-// Inside a block the look-ahead of Eq. 3 is a 16 x 16 elimination.  With M0 the
-// inverse of S at the block's start,
+// The per-move part of one block of L <= 16 proposals, from the reduced strips to the decisions
+// and to M = S^-1 of the grown queue.  x.G (row stride RL) holds P at column 0, Q at Kp, D at
+// 2 Kp; x.ub the decision inputs.  With M0 the inverse of S at the block's start,
 //     Z[t][s] = D[t][s] - P[t,:] M0 Q[s,:]^T  =  e_{j_t}^T A_cur^-1 v_s     (t, s < L)
 // is formed for ALL moves of the block at once; the ratio of move t is Z[t][t]
 // (the Schur complement of the bordered S), and accepting move e
@@ -423,6 +295,141 @@ __device__ __noinline__ void qmcd_blk_xy_global(const QmcdDev& P, const QmcdBlk&
 // identity  M11 = M0 + X Zc^-1 Y,  M12 = -X Zc^-1,  M21 = -Zc^-1 Y,  M22 = Zc^-1
 // with X = M0 Q_acc^T, Y = P_acc M0 (formed with Z0, in parallel, at the start).
 // In exact arithmetic this is the move-by-move bordering of qmcd_accept_update.
+// t = launch index of the block's first proposal, j0 = its electron.  Every CTA of the
+// cluster runs this on the same numbers, so decisions agree without communication.
+// Returns the mask of accepted moves (na of them): x.Rb holds the ratios, s.Js is extended.
+// ---------------------------------------------------------------------------
+template <bool MS>
+__device__ __forceinline__ unsigned qmcd_blk_chain(const QmcdArgs& A, const QmcdSmem& s, const QmcdBlk& x, const QmcdWalker& w,
+                                                   int RL, int t, int j0, int L, int m0, int& na_out) {
+    const QmcdDev& P = A.P;
+    const int tid = threadIdx.x;
+    const int N = P.N, K = P.K, Kp = qmcd_blk_Kp(K), ldM = qmcd_ldM(K);
+    // ---- X = M0 Q^T (Xm[i][t]) and Y = P M0 (Ym[t][b]) for every move of the block
+    if (MS) {
+        for (int idx = tid; idx < m0 * QMCD_TB; idx += QMCD_THREADS) {
+            const int i = idx >> 4, tl = idx & 15;
+            double xa = 0.0, ya = 0.0;
+            if (tl < L) {
+                const double* Gq = x.G + (size_t)tl * RL + Kp;      // Q[tl][:]
+                const double* Gp = x.G + (size_t)tl * RL;           // P[tl][:]
+                for (int b = 0; b < m0; ++b) {
+                    xa += s.Ms[(size_t)i * ldM + b] * Gq[b];
+                    ya += Gp[b] * s.Ms[(size_t)b * ldM + i];
+                }
+            }
+            x.Xm[i * QMCD_TB + tl] = xa;
+            x.Ym[tl * Kp + i] = ya;
+        }
+    } else {
+        qmcd_blk_xy_global(P, x, w, m0, L, RL);
+    }
+    __syncthreads();
+    // ---- Z0 = D - P X : one element per thread
+    double* Zc = x.Z;                                  // current / next buffer (ping-pong)
+    double* Zn = x.Z + QMCD_TB * QMCD_TB;
+    {
+        const int ti = tid >> 4, sj = tid & 15;
+        double z = 0.0;
+        if (ti < L && sj < L) {
+            z = x.G[(size_t)ti * RL + 2 * Kp + sj];
+            const double* Gp = x.G + (size_t)ti * RL;
+            for (int i = 0; i < m0; ++i) z -= Gp[i] * x.Xm[i * QMCD_TB + sj];
+        }
+        Zc[tid] = z;
+    }
+    __syncthreads();
+    unsigned accmask = 0;
+    int na = 0;
+    for (int tl = 0; tl < L; ++tl) {
+        const double R = Zc[tl * QMCD_TB + tl];
+        bool acc;
+        if (A.uniforms) { const double pa = fmin(1.0, R * R); acc = x.ub[tl] < pa; }
+        else acc = x.ub[tl] != 0.0;
+        if (acc && (R == 0.0 || !isfinite(R))) {
+            if (w.r == 0 && tid == 0) qmcd_set_status(P, QMCD_DEV_ESINGULAR, w.b, t + tl);
+            acc = false;
+        }
+        if (tid == 0) x.Rb[tl] = R;
+        if (acc) {
+            // sweep operator on index tl: thread (i, jj) owns Z[i][jj]
+            const int i = tid >> 4, jj = tid & 15;
+            const double rp = 1.0 / R;
+            const double zie = Zc[i * QMCD_TB + tl], zej = Zc[tl * QMCD_TB + jj], zij = Zc[tid];
+            double zn;
+            if (i == tl) zn = (jj == tl) ? rp : zej * rp;
+            else zn = (jj == tl) ? -zie * rp : zij - zie * (zej * rp);
+            Zn[tid] = zn;
+            __syncthreads();
+            double* tmp = Zc; Zc = Zn; Zn = tmp;
+            accmask |= 1u << tl;
+            na += 1;
+        }
+    }
+    // ---- M for the grown queue (block bordering); al(e) = block index of the e-th accepted move
+    if (na > 0) {
+        int* al_s = x.al;
+        if (tid < na) al_s[tid] = __fns(accmask, 0, tid + 1);
+        __syncthreads();
+        // U = X Zc^-1 restricted to accepted moves: U[i][f] = sum_e Xm[i][al_e] W1[e][f], W1 = Z[al_e][al_f]
+        for (int idx = tid; idx < m0 * na; idx += QMCD_THREADS) {
+            const int i = idx / na, f = idx - i * na;
+            double u = 0.0;
+            for (int e = 0; e < na; ++e) u += x.Xm[i * QMCD_TB + al_s[e]] * Zc[al_s[e] * QMCD_TB + al_s[f]];
+            x.Um[i * QMCD_TB + f] = u;
+        }
+        __syncthreads();
+        // M11 += U Y_acc ; M12 = -U ; M21 = -W1 Y_acc ; M22 = W1
+        const int mn = m0 + na;
+        auto newM = [&](int a, int b, double mold) -> double {
+            double v;
+            if (a < m0 && b < m0) {
+                v = mold;
+                for (int f = 0; f < na; ++f) v += x.Um[a * QMCD_TB + f] * x.Ym[al_s[f] * Kp + b];
+            } else if (a < m0) {
+                v = -x.Um[a * QMCD_TB + (b - m0)];
+            } else if (b < m0) {
+                v = 0.0;
+                for (int f = 0; f < na; ++f) v -= Zc[al_s[a - m0] * QMCD_TB + al_s[f]] * x.Ym[al_s[f] * Kp + b];
+            } else {
+                v = Zc[al_s[a - m0] * QMCD_TB + al_s[b - m0]];
+            }
+            return v;
+        };
+        if (MS) {
+            for (int idx = tid; idx < mn * mn; idx += QMCD_THREADS) {
+                const int a = idx / mn, b = idx - a * mn;
+                s.Ms[(size_t)a * ldM + b] = newM(a, b, (a < m0 && b < m0) ? s.Ms[(size_t)a * ldM + b] : 0.0);
+            }
+        } else if (w.r == 0) {
+            // M in global memory (row stride P.ldMg), written by the leader CTA only; four elements per thread in flight
+            const int ldg = P.ldMg;
+            for (int i0 = tid; i0 < mn * mn; i0 += 4 * QMCD_THREADS) {
+                double mo[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int idx = i0 + u * QMCD_THREADS;
+                    const int a = idx / mn, b = idx - a * mn;
+                    mo[u] = (idx < mn * mn && a < m0 && b < m0) ? __ldcg(w.M + (size_t)a * ldg + b) : 0.0;
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int idx = i0 + u * QMCD_THREADS;
+                    if (idx < mn * mn) { const int a = idx / mn, b = idx - a * mn; w.M[(size_t)a * ldg + b] = newM(a, b, mo[u]); }
+                }
+            }
+            __threadfence();
+        }
+        if (tid < na) s.Js[m0 + tid] = (j0 + al_s[tid]) % N;
+    }
+    na_out = na;
+    return accmask;
+}
+
+// ---------------------------------------------------------------------------
+// The sweep loop in blocks of 16 proposals, operands through LDG / cp.async (short column
+// slices, K > 64; the super-block loop of qmcd_superblock.cuh serves the other shapes).
+// Returns the queue length at the end.
 // ---------------------------------------------------------------------------
 // LS: the lock-step variant, a compile-time flag: a run-time test in this loop cost the
 // default scheme 12 % on c1 (measured A/B on one box), so each reading has its own kernel entry.
@@ -431,9 +438,9 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
                                   const QmcdWalker& w, int m) {
     const QmcdDev& P = A.P;
     const int tid = threadIdx.x;
-    const int N = P.N, K = P.K, Kp = qmcd_blk_Kp(K), RL = qmcd_blk_RL(K), ldM = qmcd_ldM(K);
+    const int N = P.N, K = P.K, RL = qmcd_blk_RL(K);
     const int len = w.khi - w.klo;
-    const QmcdBlk x = qmcd_blk_carve(s.rs, K, P.la_tma != 0);
+    const QmcdBlk x = qmcd_blk_carve(s.rs, K);
     // cycle accounting by one thread of the leader CTA (every phase boundary is a barrier)
     const bool prof = (w.r == 0 && tid == 0);
     long long cy_la = 0, cy_chain = 0, cy_app = 0, cy_fl = 0, c0 = prof ? clock64() : 0, c_start = c0;
@@ -444,7 +451,6 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
     while (t < A.n_moves) {
         const int j0 = (A.j_begin + t) % N;
         int L = min(min(QMCD_TB, LS ? min(K - pw, K - m) : K - m), A.n_moves - t);
-        if (P.la_tma) L = min(L, N - j0);              // the TMA ring takes the block's rows of B0 as one box: no wrap-around
         // an electron already queued may not be proposed inside a block (G7):
         // cut the block before it, or flush first when it is the block's first move
         {
@@ -481,170 +487,36 @@ __device__ int qmcd_sweep_blocked(const QmcdArgs& A, const QmcdSmem& s, cg::clus
                 qmcd_prefetch_l2(w.B + (size_t)((A.j_begin + tn) % N) * N + w.klo + k);
             }
         }
-        if (P.la_tma) {
-            unsigned itc = (unsigned)s.iflag[12];
-            switch (qmcd_tma_NB(K)) {
-                case 1: qmcd_blk_strips_tma<1>(A, s, x, cl, w, t, L, m, itc); break;
-                case 2: qmcd_blk_strips_tma<2>(A, s, x, cl, w, t, L, m, itc); break;
-                case 4: qmcd_blk_strips_tma<4>(A, s, x, cl, w, t, L, m, itc); break;
-                default: qmcd_blk_strips_tma<8>(A, s, x, cl, w, t, L, m, itc); break;
-            }
-            if (tid == 0) s.iflag[12] = (int)itc;      // (read again only after the barriers below)
-        } else {
-            qmcd_blk_strips(A, s, x, cl, w, t, L, m);
-        }
+        qmcd_blk_strips(A, s, x, cl, w, t, L, m);
         QMCD_TICK(cy_la);
 
         const int m0 = m;
-        // ---- X = M0 Q^T (Xm[i][t]) and Y = P M0 (Ym[t][b]) for every move of the block
-        if (MS) {
-            for (int idx = tid; idx < m0 * QMCD_TB; idx += QMCD_THREADS) {
-                const int i = idx >> 4, tl = idx & 15;
-                double xa = 0.0, ya = 0.0;
-                if (tl < L) {
-                    const double* Gq = x.G + (size_t)tl * RL + Kp;      // Q[tl][:]
-                    const double* Gp = x.G + (size_t)tl * RL;           // P[tl][:]
-                    for (int b = 0; b < m0; ++b) {
-                        xa += s.Ms[(size_t)i * ldM + b] * Gq[b];
-                        ya += Gp[b] * s.Ms[(size_t)b * ldM + i];
-                    }
-                }
-                x.Xm[i * QMCD_TB + tl] = xa;
-                x.Ym[tl * Kp + i] = ya;
-            }
-        } else {
-            qmcd_blk_xy_global(P, x, w, m0, L);
-        }
-        __syncthreads();
-        // ---- Z0 = D - P X : one element per thread
-        double* Zc = x.Z;                                  // current / next buffer (ping-pong)
-        double* Zn = x.Z + QMCD_TB * QMCD_TB;
-        {
-            const int ti = tid >> 4, sj = tid & 15;
-            double z = 0.0;
-            if (ti < L && sj < L) {
-                z = x.G[(size_t)ti * RL + 2 * Kp + sj];
-                const double* Gp = x.G + (size_t)ti * RL;
-                for (int i = 0; i < m0; ++i) z -= Gp[i] * x.Xm[i * QMCD_TB + sj];
-            }
-            Zc[tid] = z;
-        }
-        __syncthreads();
-        unsigned accmask = 0;
         int na = 0;
-        for (int tl = 0; tl < L; ++tl) {
-            const double R = Zc[tl * QMCD_TB + tl];
-            bool acc;
-            if (A.uniforms) { const double pa = fmin(1.0, R * R); acc = x.ub[tl] < pa; }
-            else acc = x.ub[tl] != 0.0;
-            if (acc && (R == 0.0 || !isfinite(R))) {
-                if (w.r == 0 && tid == 0) qmcd_set_status(P, QMCD_DEV_ESINGULAR, w.b, t + tl);
-                acc = false;
-            }
-            if (tid == 0) x.Rb[tl] = R;
-            if (acc) {
-                // sweep operator on index tl: thread (i, jj) owns Z[i][jj]
-                const int i = tid >> 4, jj = tid & 15;
-                const double rp = 1.0 / R;
-                const double zie = Zc[i * QMCD_TB + tl], zej = Zc[tl * QMCD_TB + jj], zij = Zc[tid];
-                double zn;
-                if (i == tl) zn = (jj == tl) ? rp : zej * rp;
-                else zn = (jj == tl) ? -zie * rp : zij - zie * (zej * rp);
-                Zn[tid] = zn;
-                __syncthreads();
-                double* tmp = Zc; Zc = Zn; Zn = tmp;
-                accmask |= 1u << tl;
-                na += 1;
-            }
-        }
-        // ---- M for the grown queue (block bordering); al(e) = block index of the e-th accepted move
-        if (na > 0) {
-            int* al_s = x.al;
-            if (tid < na) al_s[tid] = __fns(accmask, 0, tid + 1);
-            __syncthreads();
-            // U = X Zc^-1 restricted to accepted moves: U[i][f] = sum_e Xm[i][al_e] W1[e][f], W1 = Z[al_e][al_f]
-            for (int idx = tid; idx < m0 * na; idx += QMCD_THREADS) {
-                const int i = idx / na, f = idx - i * na;
-                double u = 0.0;
-                for (int e = 0; e < na; ++e) u += x.Xm[i * QMCD_TB + al_s[e]] * Zc[al_s[e] * QMCD_TB + al_s[f]];
-                x.Um[i * QMCD_TB + f] = u;
-            }
-            __syncthreads();
-            // M11 += U Y_acc ; M12 = -U ; M21 = -W1 Y_acc ; M22 = W1
-            const int mn = m0 + na;
-            auto newM = [&](int a, int b, double mold) -> double {
-                double v;
-                if (a < m0 && b < m0) {
-                    v = mold;
-                    for (int f = 0; f < na; ++f) v += x.Um[a * QMCD_TB + f] * x.Ym[al_s[f] * Kp + b];
-                } else if (a < m0) {
-                    v = -x.Um[a * QMCD_TB + (b - m0)];
-                } else if (b < m0) {
-                    v = 0.0;
-                    for (int f = 0; f < na; ++f) v -= Zc[al_s[a - m0] * QMCD_TB + al_s[f]] * x.Ym[al_s[f] * Kp + b];
-                } else {
-                    v = Zc[al_s[a - m0] * QMCD_TB + al_s[b - m0]];
-                }
-                return v;
-            };
-            if (MS) {
-                for (int idx = tid; idx < mn * mn; idx += QMCD_THREADS) {
-                    const int a = idx / mn, b = idx - a * mn;
-                    s.Ms[(size_t)a * ldM + b] = newM(a, b, (a < m0 && b < m0) ? s.Ms[(size_t)a * ldM + b] : 0.0);
-                }
-            } else if (w.r == 0) {
-                // M in global memory (row stride P.ldMg), written by the leader CTA only; four elements per thread in flight
-                const int ldg = P.ldMg;
-                for (int i0 = tid; i0 < mn * mn; i0 += 4 * QMCD_THREADS) {
-                    double mo[4];
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const int idx = i0 + u * QMCD_THREADS;
-                        const int a = idx / mn, b = idx - a * mn;
-                        mo[u] = (idx < mn * mn && a < m0 && b < m0) ? __ldcg(w.M + (size_t)a * ldg + b) : 0.0;
-                    }
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const int idx = i0 + u * QMCD_THREADS;
-                        if (idx < mn * mn) { const int a = idx / mn, b = idx - a * mn; w.M[(size_t)a * ldg + b] = newM(a, b, mo[u]); }
-                    }
-                }
-                __threadfence();
-            }
-            if (tid < na) s.Js[m0 + tid] = (j0 + al_s[tid]) % N;
-        }
+        const unsigned accmask = qmcd_blk_chain<MS>(A, s, x, w, RL, t, j0, L, m0, na);
         QMCD_TICK(cy_chain);
         // ---- append the block's accepted moves to the queue: C[slot] = v, W[slot] = B0[j,:]
         {
-            if (P.la_tma) {
-                if (tid == 0 && na > 0) {
-                    unsigned ph = (unsigned)s.iflag[13];
-                    qmcd_blk_append_bulk(A, s, x, w, t, j0, m0, accmask, na, ph);
-                    s.iflag[13] = (int)ph;
-                }
-            } else {
-                // four 16-byte vectors of each source row in flight per thread (the copy is a latency chain otherwise)
-                const int vpr = len >> 1, total = na * vpr;
-                for (int i0 = tid; i0 < total; i0 += 4 * QMCD_THREADS) {
-                    double2 vv[4], bb[4];
-                    size_t off[4];
-    #pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const int idx = i0 + u * QMCD_THREADS;
-                        if (idx < total) {
-                            const int e = idx / vpr, k = (idx - e * vpr) * 2;
-                            const int al = __fns(accmask, 0, e + 1);
-                            vv[u] = qmcd_ldcg128(A.v + ((size_t)(t + al) * P.batch + w.b) * N + w.klo + k);
-                            bb[u] = qmcd_ldcg128(w.B + (size_t)((j0 + al) % N) * N + w.klo + k);
-                            off[u] = (size_t)(m0 + e) * N + w.klo + k;
-                        }
+            // four 16-byte vectors of each source row in flight per thread (the copy is a latency chain otherwise)
+            const int vpr = len >> 1, total = na * vpr;
+            for (int i0 = tid; i0 < total; i0 += 4 * QMCD_THREADS) {
+                double2 vv[4], bb[4];
+                size_t off[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int idx = i0 + u * QMCD_THREADS;
+                    if (idx < total) {
+                        const int e = idx / vpr, k = (idx - e * vpr) * 2;
+                        const int al = __fns(accmask, 0, e + 1);
+                        vv[u] = qmcd_ldcg128(A.v + ((size_t)(t + al) * P.batch + w.b) * N + w.klo + k);
+                        bb[u] = qmcd_ldcg128(w.B + (size_t)((j0 + al) % N) * N + w.klo + k);
+                        off[u] = (size_t)(m0 + e) * N + w.klo + k;
                     }
-    #pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        if (i0 + u * QMCD_THREADS < total) {
-                            qmcd_stg128(w.C + off[u], vv[u].x, vv[u].y);
-                            qmcd_stg128(w.W + off[u], bb[u].x, bb[u].y);
-                        }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    if (i0 + u * QMCD_THREADS < total) {
+                        qmcd_stg128(w.C + off[u], vv[u].x, vv[u].y);
+                        qmcd_stg128(w.W + off[u], bb[u].x, bb[u].y);
                     }
                 }
             }

@@ -81,6 +81,18 @@ __device__ __forceinline__ void qmcd_stage_half(double* __restrict__ dst, const 
 }
 
 __device__ __forceinline__ double2 qmcd_lds128(const double* p) { return *reinterpret_cast<const double2*>(p); }
+// the same from a 32-bit shared-memory address: LDS.128 whatever the compiler knows about the pointer's origin (a generic
+// pointer that reaches a __noinline__ function is read with LD.E.128 plus descriptor moves)
+__device__ __forceinline__ double2 qmcd_lds128s(unsigned a) {
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ double qmcd_lds64s(unsigned a) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a) : "memory");
+    return v;
+}
 // coherent 16-byte global load / store of B: the same kernel rewrites B, and a tile is taken by a
 // different CTA from one flush to the next, so the loads go to L2 (.cg), never through L1
 __device__ __forceinline__ double2 qmcd_ldg128(const double* p) {

@@ -24,9 +24,10 @@
 #include <cuda.h>
 #include "qmcd_flush_mma.cuh"
 
-// 4-D views, see qmcd_api.cu.  B, C, W, M: the flush (this file).  B16, V, Wk (+ C): the look-ahead ring of
-// qmcd_block.cuh -- B with 16-row boxes, the proposals of the current qmcd_sweep launch, W in the k-major view.
-struct QmcdTmaps { CUtensorMap B, C, W, M, B16, V, Wk, B64, Y; };   // B64: 64-row boxes of B; Y = M W (K > 64), viewed like W
+// 4-D views, see qmcd_api.cu.  B, B64, C, W, M, Y: the flush (this file; B64: 64-row boxes of B; Y = M W (K > 64), viewed
+// like W).  Bs, Vs, C32, W32: the look-ahead ring of qmcd_superblock.cuh -- boxes of 2 k-groups (k-major view): 16 / 32 / 64
+// rows of B, as many proposals of the current qmcd_sweep launch, 32 rows of C and of W.
+struct QmcdTmaps { CUtensorMap B, C, W, M, B64, Y, C32, W32, Bs[3], Vs[3]; };
 
 #define QMCD_TMA_NS 4
 #define QMCD_TMA_STAGE_BYTES 49152
@@ -66,6 +67,7 @@ __device__ __forceinline__ void qmcd_bulk_store(void* dst, unsigned src, unsigne
 }
 __device__ __forceinline__ void qmcd_bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void qmcd_bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void qmcd_bulk_wait_read1() { asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory"); }
 __device__ __forceinline__ void qmcd_bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 // L2 eviction policies: the flush streams each tile of B once per pass (evict first: do not push the queues
 // out of L2); the queue rows C, W and M are re-read by every tile and every look-ahead block (evict last)
@@ -82,11 +84,9 @@ __device__ __forceinline__ void qmcd_tma_load4_hint(unsigned dst, const CUtensor
 }
 __device__ __forceinline__ void qmcd_fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
-// look-ahead ring (qmcd_block.cuh): 3 stages; full[3] at +576, empty[3] at +600, the append's barrier at +624
+// look-ahead ring (qmcd_superblock.cuh): 3 stages; full[3] at +576, empty[3] at +600 (the append's barriers: +640 ... +768)
 #define QMCD_LA_NS 3
 #define QMCD_LA_BAR_OFF 576
-#define QMCD_LA_APP_BAR_OFF 624
-__host__ __device__ inline size_t qmcd_la_stage_bytes(int K) { return 8192 + 4096 * (size_t)qmcd_tma_NB(K); }
 __device__ __forceinline__ void qmcd_la_init_barriers(unsigned char* smem) {
     const unsigned bar0 = qmcd_su32(smem + QMCD_LA_BAR_OFF);
 #pragma unroll
@@ -94,7 +94,6 @@ __device__ __forceinline__ void qmcd_la_init_barriers(unsigned char* smem) {
         qmcd_mbar_init(bar0 + 8 * s, 1);
         qmcd_mbar_init(bar0 + 8 * QMCD_LA_NS + 8 * s, QMCD_WARPS);
     }
-    qmcd_mbar_init(qmcd_su32(smem + QMCD_LA_APP_BAR_OFF), 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 }
 
@@ -169,22 +168,22 @@ __device__ __noinline__ void qmcd_flush_tile_tma(const QmcdDev& P, const QmcdTma
         const unsigned char* stg = st0 + s * QMCD_TMA_STAGE_BYTES;
         qmcd_mbar_wait(bar0 + 8 * s, u & 1);
         if (wid == (j & 7) && lane == 0 && j + NS - 1 < total) issue(j + NS - 1);
-        const double* As = reinterpret_cast<const double*>(stg) + (wrow + g) * 8 + 2 * c;
-        const double* Cs = reinterpret_cast<const double*>(stg + OFF2) + g * 8 + 2 * c;
+        const unsigned As = qmcd_su32(stg) + 8u * ((wrow + g) * 8 + 2 * c);        // byte addresses in shared memory
+        const unsigned Cs = qmcd_su32(stg) + OFF2 + 8u * (g * 8 + 2 * c);
         if (DB) {
             double2 av[2][A_T], bv[2][NB];
 #pragma unroll
-            for (int a = 0; a < A_T; ++a) av[0][a] = qmcd_lds128(As + a * 64);
+            for (int a = 0; a < A_T; ++a) av[0][a] = qmcd_lds128s(As + a * 512);
 #pragma unroll
-            for (int bt = 0; bt < NB; ++bt) bv[0][bt] = qmcd_lds128(Cs + bt * 64);
+            for (int bt = 0; bt < NB; ++bt) bv[0][bt] = qmcd_lds128s(Cs + bt * 512);
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const int cur = q & 1, nxt = cur ^ 1;
                 if (q < 3) {
 #pragma unroll
-                    for (int a = 0; a < A_T; ++a) av[nxt][a] = qmcd_lds128(As + (q + 1) * (ROWS * 8) + a * 64);
+                    for (int a = 0; a < A_T; ++a) av[nxt][a] = qmcd_lds128s(As + (q + 1) * (ROWS * 64) + a * 512);
 #pragma unroll
-                    for (int bt = 0; bt < NB; ++bt) bv[nxt][bt] = qmcd_lds128(Cs + (q + 1) * (64 * NB) + bt * 64);
+                    for (int bt = 0; bt < NB; ++bt) bv[nxt][bt] = qmcd_lds128s(Cs + (q + 1) * (512 * NB) + bt * 512);
                 }
 #pragma unroll
                 for (int bt = 0; bt < NB; ++bt)
@@ -200,12 +199,12 @@ __device__ __noinline__ void qmcd_flush_tile_tma(const QmcdDev& P, const QmcdTma
             for (int q = 0; q < 4; ++q) {
                 double2 av[A_T];
 #pragma unroll
-                for (int a = 0; a < A_T; ++a) av[a] = qmcd_lds128(As + q * (ROWS * 8) + a * 64);
+                for (int a = 0; a < A_T; ++a) av[a] = qmcd_lds128s(As + q * (ROWS * 64) + a * 512);
 #pragma unroll
                 for (int h = 0; h < NB; h += 8) {          // 8 n-tiles at a time: 8 fragment registers pairs live
                     double2 bv[8];
 #pragma unroll
-                    for (int bt = 0; bt < 8; ++bt) bv[bt] = qmcd_lds128(Cs + q * (64 * NB) + (h + bt) * 64);
+                    for (int bt = 0; bt < 8; ++bt) bv[bt] = qmcd_lds128s(Cs + q * (512 * NB) + (h + bt) * 512);
 #pragma unroll
                     for (int bt = 0; bt < 8; ++bt)
 #pragma unroll
@@ -247,16 +246,16 @@ __device__ __noinline__ void qmcd_flush_tile_tma(const QmcdDev& P, const QmcdTma
 #pragma unroll
             for (int t = 0; t < NB; ++t) { T2[a][t][0] = 0.0; T2[a][t][1] = 0.0; }
         // M[k][n] at group (n / 16): row k, 16-byte chunk ((n % 16) / 2) ^ (k % 8), half n % 2;  k = 8q + 2c + s, n = 8t + g
-        const unsigned char* Ms = stg + (2 * c) * 128 + (g & 1) * 8;
+        const unsigned Ms = qmcd_su32(stg) + (2 * c) * 128 + (g & 1) * 8;
         const int ch0 = (g >> 1) ^ (2 * c), ch1 = (g >> 1) ^ (2 * c + 1);            // chunk of n-tile parity 0; parity 1: ^ 4
 #pragma unroll
         for (int q = 0; q < NB; ++q) {
             double b0[NB], b1[NB];
 #pragma unroll
             for (int t = 0; t < NB; ++t) {
-                const unsigned char* pm = Ms + (t >> 1) * 8192 + q * 1024;
-                b0[t] = *reinterpret_cast<const double*>(pm + ((ch0 ^ ((t & 1) << 2)) << 4));
-                b1[t] = *reinterpret_cast<const double*>(pm + 128 + ((ch1 ^ ((t & 1) << 2)) << 4));
+                const unsigned pm = Ms + (t >> 1) * 8192 + q * 1024;
+                b0[t] = qmcd_lds64s(pm + ((ch0 ^ ((t & 1) << 2)) << 4));
+                b1[t] = qmcd_lds64s(pm + 128 + ((ch1 ^ ((t & 1) << 2)) << 4));
             }
 #pragma unroll
             for (int t = 0; t < NB; ++t)
@@ -284,22 +283,22 @@ __device__ __noinline__ void qmcd_flush_tile_tma(const QmcdDev& P, const QmcdTma
         const int n0 = 32 * (j - nn0);
         qmcd_mbar_wait(bar0 + 8 * s, u & 1);
         if (wid == (j & 7) && lane == 0 && j + NS - 1 < total) issue(j + NS - 1);
-        const double* Ds = reinterpret_cast<const double*>(stg);                     // [4 groups of 8 columns][ROWS][8]
-        const unsigned char* Ws = stg + OFF2 + (2 * c) * 128;                         // [2 groups of 16 columns][8 NB rows][128 B]
+        const unsigned Ds = qmcd_su32(stg);                                           // [4 groups of 8 columns][ROWS][8]
+        const unsigned Ws = Ds + OFF2 + (2 * c) * 128;                                // [2 groups of 16 columns][8 NB rows][128 B]
         double an[A_T][2][2][2];                                                     // [a][G][t][e]
 #pragma unroll
         for (int a = 0; a < A_T; ++a)
 #pragma unroll
             for (int G = 0; G < 2; ++G) {              // this lane's columns 16 G + 4 c .. + 3 of row wrow + 8 a + g
-                const double* p = Ds + ((2 * G + (c >> 1)) * ROWS + wrow + a * 8 + g) * 8 + 4 * (c & 1);
-                const double2 v0 = qmcd_lds128(p), v1 = qmcd_lds128(p + 2);
+                const unsigned p = Ds + 8u * (((2 * G + (c >> 1)) * ROWS + wrow + a * 8 + g) * 8 + 4 * (c & 1));
+                const double2 v0 = qmcd_lds128s(p), v1 = qmcd_lds128s(p + 16);
                 an[a][G][0][0] = v0.x; an[a][G][1][0] = v0.y; an[a][G][0][1] = v1.x; an[a][G][1][1] = v1.y;
             }
         double2 x0[2][2], x1[2][2];                                                  // [buffer][G]
 #pragma unroll
         for (int G = 0; G < 2; ++G) {
-            x0[0][G] = *reinterpret_cast<const double2*>(Ws + G * (1024 * NB) + sw0);
-            x1[0][G] = *reinterpret_cast<const double2*>(Ws + G * (1024 * NB) + 128 + sw1);
+            x0[0][G] = qmcd_lds128s(Ws + G * (1024 * NB) + sw0);
+            x1[0][G] = qmcd_lds128s(Ws + G * (1024 * NB) + 128 + sw1);
         }
 #pragma unroll
         for (int q = 0; q < NB; ++q) {
@@ -307,8 +306,8 @@ __device__ __noinline__ void qmcd_flush_tile_tma(const QmcdDev& P, const QmcdTma
             if (q + 1 < NB) {
 #pragma unroll
                 for (int G = 0; G < 2; ++G) {
-                    x0[nxt][G] = *reinterpret_cast<const double2*>(Ws + G * (1024 * NB) + (q + 1) * 1024 + sw0);
-                    x1[nxt][G] = *reinterpret_cast<const double2*>(Ws + G * (1024 * NB) + (q + 1) * 1024 + 128 + sw1);
+                    x0[nxt][G] = qmcd_lds128s(Ws + G * (1024 * NB) + (q + 1) * 1024 + sw0);
+                    x1[nxt][G] = qmcd_lds128s(Ws + G * (1024 * NB) + (q + 1) * 1024 + 128 + sw1);
                 }
             }
 #pragma unroll

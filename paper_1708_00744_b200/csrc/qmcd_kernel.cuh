@@ -201,6 +201,7 @@ __device__ void qmcd_pool_loop(const QmcdDev& P, const QmcdSmem& s) {
 }
 
 #include "qmcd_block.cuh"
+#include "qmcd_superblock.cuh"
 
 // Accept path shared by ACCEPT and SWEEP.  Called by ALL CTAs with the same
 // (j, m, R, inq) and cf / rf valid in every CTA.  Returns the new m.
@@ -380,9 +381,9 @@ __device__ __forceinline__ void qmcd_kernel_body(const QmcdArgs& A, const QmcdTm
     QmcdSmem s = qmcd_carve(qmcd_smem_raw, P.N, P.K, S, P.m_in_smem != 0);
     s.tm = &TM;
     if (threadIdx.x == 0) {
-        s.iflag[8] = 0; s.iflag[10] = 0; s.iflag[12] = 0; s.iflag[13] = 0; s.iflag[15] = 0;
+        s.iflag[8] = 0; s.iflag[10] = 0; s.iflag[12] = 0; s.iflag[13] = 0; s.iflag[14] = 0; s.iflag[15] = 0;
         if (P.use_tma) qmcd_tma_init_barriers(qmcd_smem_raw);
-        if (P.la_tma) qmcd_la_init_barriers(qmcd_smem_raw);
+        if (P.la_tma) { qmcd_la_init_barriers(qmcd_smem_raw); qmcd_sb_app_init(qmcd_smem_raw); }
     }
     __syncthreads();
     if (b >= P.batch) { qmcd_pool_loop(P, s); return; }
@@ -397,7 +398,7 @@ __device__ __forceinline__ void qmcd_kernel_body(const QmcdArgs& A, const QmcdTm
     } else if (BLOCKED) {
         int m = __ldcg(P.m + b);
         qmcd_load_state<true>(P, s, w, m);
-        m = qmcd_sweep_blocked<BLOCKED == 2, true>(A, s, cl, w, m);
+        m = P.la_tma ? qmcd_sweep_sb<BLOCKED == 2>(A, s, cl, w, m) : qmcd_sweep_blocked<BLOCKED == 2, true>(A, s, cl, w, m);
         qmcd_writeback_M<true>(P, s, w, m);
         if (r == 0 && threadIdx.x == 0) { P.sj[b] = -1; P.m[b] = m; }
     } else {
