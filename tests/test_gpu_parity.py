@@ -256,8 +256,10 @@ def test_blocked_lookahead_matches_oracle_and_per_move(qmcd, N, K, batch, cluste
     wl.n_moves = n_moves
     mask = wl.bernoulli_mask(p)
     Bo = wl.Ainv.copy(); Ro, acco, _ = oracle.run(2, Bo, K, wl.proposals, j_begin=j_begin, mask=mask)
-    g = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, j_begin=j_begin)
-    assert g["status"] == 0 and g["S"] == cluster and g["blocked"]
+    # la_tma = 0: the 16-proposal blocks of qmcd_block.cuh (LDG / cp.async strips) -- the path of K > 64 and of shapes the
+    # super-block ring does not take; the default (super-blocks where they fit) is checked below and in the next test
+    g = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, j_begin=j_begin, la_tma=0)
+    assert g["status"] == 0 and g["S"] == cluster and g["blocked"] and g["la_tma"] == 0
     assert np.array_equal(g["acc"], acco)
     assert _rel(g["R"], Ro) <= RTOL_RATIO
     assert np.max(np.abs(g["B"] - Bo)) <= 1e-10
@@ -267,14 +269,59 @@ def test_blocked_lookahead_matches_oracle_and_per_move(qmcd, N, K, batch, cluste
     assert not pm["blocked"]
     assert np.max(np.abs(g["R"] - pm["R"])) <= 1e-11
     assert np.max(np.abs(g["B"] - pm["B"])) <= 1e-11
-    # the same blocks with the operands streamed through the TMA ring (forced on: by default only long slices use
-    # it) -- wrap-around cuts the block, a repeated electron cuts it or flushes first; K <= 64, slices of 32-column chunks
-    if K <= 64 and N >= 128 and N % 64 == 0 and (N // cluster) % 32 == 0:
-        gt = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, j_begin=j_begin, la_tma=2)
-        assert gt["la_tma"] == 1 and gt["blocked"] and gt["status"] == 0
-        assert np.array_equal(gt["acc"], acco)
-        assert _rel(gt["R"], Ro) <= RTOL_RATIO
-        assert np.max(np.abs(gt["B"] - Bo)) <= 1e-10
+    # the library's default for this shape: super-blocks through the TMA ring when K <= 64 and the slices are whole
+    # 16-column chunks -- wrap-around cuts the super-block, a repeated electron cuts it or flushes first
+    gt = gpu_sweep(qmcd, wl, K, mask=mask, cluster=cluster, j_begin=j_begin)
+    assert gt["la_tma"] == (1 if (K <= 64 and N >= 128 and N % 64 == 0 and (N // cluster) % 16 == 0) else 0)
+    assert gt["blocked"] and gt["status"] == 0
+    assert np.array_equal(gt["acc"], acco)
+    assert _rel(gt["R"], Ro) <= RTOL_RATIO
+    assert np.max(np.abs(gt["B"] - Bo)) <= 1e-10
+
+
+@pytest.mark.parametrize("N,K,batch,cluster,mode,j_begin,lockstep", [
+    (256, 64, 2, 1, "bern0.99", 0, 0),     # one 64-proposal super-block per window, tiles of D only
+    (256, 64, 2, 2, "bern0.5", 200, 0),    # rate-adaptive length (64 proposals at queue length 32), wrap-around, cluster-wide sum
+    (512, 64, 2, 4, "bern0.3", 0, 0),      # over-long super-blocks: the queue fills inside one and the rest is looked at again
+    (128, 64, 2, 1, "bern0.2", 0, 0),      # K near N with many rejections: queued electrons come round again (cut / flush first)
+    (256, 48, 3, 2, "bern0.7", 5, 0),      # K = 48: shapes 64 -> 32 -> 16 as the queue fills
+    (192, 20, 2, 1, "bern0.9", 0, 0),      # K not a multiple of 8, N = 3 x 64
+    (256, 3, 2, 1, "bern1.0", 0, 0),       # K smaller than a block
+    (256, 64, 2, 8, "metropolis", 0, 0),   # 8 CTAs per walker (32-column slices), Metropolis decisions on the ratios
+    (1024, 64, 2, 2, "bern0.8", 1000, 0),  # long slices: queue append in several pieces per warp
+    (256, 64, 2, 1, "bern0.5", 0, 1),      # lock-step windows (oracle path 3)
+    (256, 40, 2, 2, "bern0.1", 3, 1),      # lock-step with few acceptances
+])
+def test_superblock_lookahead_matches_oracle(qmcd, N, K, batch, cluster, mode, j_begin, lockstep):
+    """qmcd_sweep's super-block look-ahead (qmcd_superblock.cuh: P | Q | D of up to 64 proposals from one pass over the
+    operands, queue entries accepted inside the super-block read out of D) against the oracle's delayed path (path 2;
+    lock-step: the literal path 3), every ratio, decision and the final inverse; launches cut at odd places."""
+    wl = inputs.make_workload(batch, N, n_moves=3 * N, seed=31)
+    n_moves = 2 * N + 37
+    t = np.arange(n_moves)
+    pick = (t % N + j_begin) % N + N * (t // N)
+    wl.proposals = np.ascontiguousarray(wl.proposals[pick]); wl.uniforms = np.ascontiguousarray(wl.uniforms[pick])
+    wl.n_moves = n_moves
+    mask = wl.bernoulli_mask(float(mode[4:])) if mode.startswith("bern") else None
+    u = wl.uniforms if mode == "metropolis" else None
+    Bo = wl.Ainv.copy()
+    if lockstep:
+        Ao = wl.A.copy()
+        Ro, acco, _, _ = oracle.run_lockstep(Ao, Bo, K, wl.proposals, j_begin=j_begin, mask=mask, uniforms=u)
+    else:
+        Ro, acco, _ = oracle.run(2, Bo, K, wl.proposals, j_begin=j_begin, mask=mask, uniforms=u)
+    for split in (None, [7, 100, N + 1]):
+        g = gpu_sweep(qmcd, wl, K, mask=mask, uniforms=u, cluster=cluster, j_begin=j_begin, lockstep=lockstep or None, split=split)
+        assert g["status"] == 0 and g["S"] == cluster and g["blocked"] and g["la_tma"] == 1
+        if u is not None:
+            near_tie = np.abs(u - np.minimum(1.0, Ro * Ro)) < 1e-9            # reading G20
+            assert np.array_equal(g["acc"][~near_tie], acco[~near_tie])
+        else:
+            assert np.array_equal(g["acc"], acco)
+        assert _rel(g["R"], Ro) <= RTOL_RATIO
+        assert np.max(np.abs(g["B"] - Bo)) <= 1e-10 * max(1.0, np.abs(Bo).max())
+        assert np.array_equal(g["counters"][:, 0], acco.sum(axis=0))
+        assert np.all(g["pending"] == 0)
 
 
 @pytest.mark.parametrize("K", [1, 16, 32])
