@@ -200,9 +200,10 @@ int qmcd_invert_static(qmcd_handle h, const double* A_dev, double* Ainv_dev, int
  *                   cannot replay cooperative cluster launches; safe on an otherwise idle device: one CTA per SM).
  *   "tma"           1 (default): flush tiles for K <= 64, N >= 128, N % 64 == 0 through the TMA-fed kernel
  *                   (128-row tiles); 0 = the cp.async DMMA kernels.  "tile_rows" (64 / 128) applies to the latter.
- *   "la_tma"        qmcd_sweep's blocked look-ahead streams its operands through a TMA ring: 1 (default) when a CTA's
- *                   column slice has >= 1024 columns, 2 whenever the shape allows (K <= 64, slices of whole 32-column
- *                   chunks), 0 never.
+ *   "la_tma"        1 (default; 2 means the same): qmcd_sweep looks ahead in SUPER-BLOCKS of up to 64 proposals whose
+ *                   operands stream through a TMA ring once (K <= 128, K even beyond 64, N >= 128, N % 64 == 0, column
+ *                   slices of whole 16- / 8-column chunks); 0 = blocks of 16 proposals with LDG / cp.async strips (the
+ *                   path of every other shape).
  *   "ratio_kernel"  1 (default): qmcd_ratio runs the dedicated bandwidth kernel; 0 = the cluster kernel's look-ahead
  *                   (the arithmetic of the per-move sweep, bit for bit).
  *   "flush_path"    0 auto, 1 CUDA-core, 2 DMMA.

@@ -123,24 +123,25 @@ static bool encode_view(CUtensorMap* tm, double* base, int rows, int N, size_t b
     return encode_4d(tm, base, gd, gs, bd, swizzle);
 }
 // The proposals of one qmcd_sweep launch, [n_moves][batch][N], seen as {8, n_moves, N / 8, batch}: row t of walker b
-static bool encode_proposals(CUtensorMap* tm, const double* base, int n_moves, int N, int batch, int box_rows) {
+static bool encode_proposals(CUtensorMap* tm, const double* base, int n_moves, int N, int batch, int box_rows, int groups) {
     const cuuint64_t gd[4] = {8, (cuuint64_t)n_moves, (cuuint64_t)(N / 8), (cuuint64_t)batch};
     const cuuint64_t gs[3] = {(cuuint64_t)batch * N * 8, 64, (cuuint64_t)N * 8};
-    const cuuint32_t bd[4] = {8, (cuuint32_t)box_rows, 2, 1};
+    const cuuint32_t bd[4] = {8, (cuuint32_t)box_rows, (cuuint32_t)groups, 1};
     return encode_4d(tm, base, gd, gs, bd, false);
 }
 static bool tma_shape_ok(int N, int K) { return K <= 128 && N % 64 == 0 && N >= 128; }
-static bool la_shape_ok(int N, int K) { return K <= 64 && N % 64 == 0 && N >= 128; }
+static bool la_shape_ok(int N, int K) { return K <= QMCD_SB_KMAX && N % 64 == 0 && N >= 128; }
 static void encode_queue_tmaps(qmcd_ctx* h) {
     h->tmaps_ok = false;
     if (!tma_shape_ok(h->N, h->K)) return;
     const int N = h->N, K = h->K, rows = 8 * qmcd_tma_NB(K);
-    h->tmaps_ok = encode_view(&h->tmaps.C, h->P.C, K, N, (size_t)K * N, h->batch, 8, rows, 4, false);
+    const int nq = qmcd_sb_nq(K);
+    h->tmaps_ok = encode_view(&h->tmaps.C, h->P.C, K, N, (size_t)K * N, h->batch, 8, rows, 4, false) &&
+                  encode_view(&h->tmaps.W32, h->P.W, K, N, (size_t)K * N, h->batch, 8, 32, nq, false) &&
+                  encode_view(&h->tmaps.C32, h->P.C, K, N, (size_t)K * N, h->batch, 8, 32, nq, false);
     if (K <= 64)
         h->tmaps_ok = h->tmaps_ok && encode_view(&h->tmaps.W, h->P.W, K, N, (size_t)K * N, h->batch, 16, rows, 2, true) &&
-                      encode_view(&h->tmaps.M, h->P.M, 64, 64, (size_t)64 * 64, h->batch, 16, 64, 4, true) &&
-                      encode_view(&h->tmaps.W32, h->P.W, K, N, (size_t)K * N, h->batch, 8, 32, 2, false) &&
-                      encode_view(&h->tmaps.C32, h->P.C, K, N, (size_t)K * N, h->batch, 8, 32, 2, false);
+                      encode_view(&h->tmaps.M, h->P.M, 64, 64, (size_t)64 * 64, h->batch, 16, 64, 4, true);
     else                                       // 64 < K <= 128: the tile multiplies by Y = M W (formed by the job's first phase)
         h->tmaps_ok = h->tmaps_ok && encode_view(&h->tmaps.Y, h->P.Y, K, N, (size_t)K * N, h->batch, 16, rows, 2, true);
 }
@@ -150,31 +151,31 @@ static void refresh_use_tma(qmcd_ctx* h) {
     // 128-row tiles when a job then still has >= 8 of them, else 64-row tiles (more workers per job: a short flush is
     // latency, not throughput); K > 64 runs 64-row tiles (the registers hold T for 8 rows x 128 columns per warp)
     if (h->P.use_tma) h->P.tile_rows = (h->K <= 64 && h->N >= 1024 && h->tile_opt != 64) || (h->K <= 64 && h->tile_opt == 128) ? 128 : 64;
-    h->P.la_tma = (h->la_opt && h->la_fit && h->tmaps_ok && h->P.B != nullptr && h->P.blk_ok && h->P.m_in_smem) ? 1 : 0;
+    h->P.la_tma = (h->la_opt && h->la_fit && h->tmaps_ok && h->P.B != nullptr && h->P.blk_ok) ? 1 : 0;
 }
 
 static int configure_kernel(qmcd_ctx* h, int S) {
     const size_t cap = 227 * 1024;
+    const int N = h->N, K = h->K;
     // blocked look-ahead: 16-byte vector access to every slice, <= 40 output tiles
-    const bool blk_shape = h->N >= QMCD_TB && (h->N % (8 * S) == 0) && (2 * ((h->K + 7) / 8) + 2 <= 8 * QMCD_BLK_MAXU);
-    // the TMA look-ahead ring (super-blocks, qmcd_superblock.cuh): K <= 64 tensor maps, column slices of whole 16-column chunks
-    // (measured against the LDG / cp.async strips of qmcd_block.cuh: c1 +11 %, c2 +21 %, c3 +8 %, c4 +13 %)
-    bool la = blk_shape && h->la_opt && la_shape_ok(h->N, h->K) && (h->N / S) % QMCD_SB_CW == 0 && h->N % S == 0;
-    size_t blk = blk_shape ? (la ? qmcd_sb_smem_bytes(h->K) : qmcd_blk_smem_bytes(h->K)) : 0;
-    size_t base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, blk);
-    if (la && base > cap) { la = false; blk = qmcd_blk_smem_bytes(h->K); base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, blk); }
-    h->la_fit = la;
-    h->P.m_in_smem = 1; h->P.blk_ok = blk_shape ? 1 : 0;
-    if (base > cap) {
-        // M does not fit beside the blocked look-ahead's area: keep the blocked look-ahead and leave M in global memory
-        // (staged 16 rows at a time, qmcd_blk_xy_global) when K is even and small enough for its register tile
-        h->la_fit = false;
-        const size_t nb = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, false, qmcd_blk_smem_bytes(h->K));
-        if (blk_shape && h->K % 2 == 0 && h->K <= 16 * QMCD_BLK_YU && nb <= cap) { base = nb; h->P.m_in_smem = 0; h->P.blk_ok = 1; }
-        else {
-            base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, true, 0); h->P.blk_ok = 0;
-            if (base > cap) { base = QMCD_SMEM_HEADER + qmcd_smem_base_bytes(h->N, h->K, S, false, 0); h->P.m_in_smem = 0; }
-        }
+    const bool blk_shape = N >= QMCD_TB && (N % (8 * S) == 0) && (2 * ((K + 7) / 8) + 2 <= 8 * QMCD_BLK_MAXU);
+    // M in global memory (staged 16 rows at a time, qmcd_blk_xy_global): K even (16-byte rows), small enough for its register tile
+    const bool gm_ok = blk_shape && K % 2 == 0 && K <= 16 * QMCD_BLK_YU;
+    // super-blocks through the TMA ring (qmcd_superblock.cuh): K <= 128 tensor maps, column slices of whole chunks
+    // (measured against the 16-proposal blocks with LDG / cp.async strips: c1 +11 %, c2 +21 %, c3 +8 %, c4 +13 % at K <= 64)
+    const bool la_shape = blk_shape && h->la_opt && la_shape_ok(N, K) && N % S == 0 && (N / S) % (8 * qmcd_sb_nq(K)) == 0;
+    auto need = [&](bool with_M, size_t blk) { return (size_t)QMCD_SMEM_HEADER + qmcd_smem_base_bytes(N, K, S, with_M, blk); };
+    const size_t sbb = qmcd_sb_smem_bytes(K), blkb = qmcd_blk_smem_bytes(K);
+    size_t base;
+    h->la_fit = false; h->P.m_in_smem = 1; h->P.blk_ok = blk_shape ? 1 : 0;
+    if (la_shape && K <= 64 && need(true, sbb) <= cap) { base = need(true, sbb); h->la_fit = true; }                  // super-blocks, M in shared memory
+    else if (la_shape && K > 64 && gm_ok && need(false, sbb) <= cap) { base = need(false, sbb); h->la_fit = true; h->P.m_in_smem = 0; }   // ..., M in global memory
+    else if (blk_shape && need(true, blkb) <= cap) base = need(true, blkb);                                         // 16-proposal blocks
+    else if (gm_ok && need(false, blkb) <= cap) { base = need(false, blkb); h->P.m_in_smem = 0; }                     // ..., M in global memory
+    else {                                                                                                          // per-move look-ahead
+        h->P.blk_ok = 0;
+        base = need(true, 0);
+        if (base > cap) { base = need(false, 0); h->P.m_in_smem = 0; }
     }
     const size_t mma = QMCD_SMEM_HEADER + qmcd_flush_mma_smem_bytes(h->N, h->K);
     if (base > cap) { snprintf(g_last_error, sizeof(g_last_error), "shared memory need %zu > 227 KB", base); return QMCD_EINVAL; }
@@ -379,9 +380,9 @@ extern "C" int qmcd_set_inverse(qmcd_handle h, double* Ainv_dev) {
     h->P.B = Ainv_dev;
     if (h->tmaps_ok && !(encode_view(&h->tmaps.B, Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 128, 4, false) &&
                          encode_view(&h->tmaps.B64, Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 64, 4, false) &&
-                         encode_view(&h->tmaps.Bs[0], Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 16, 2, false) &&
-                         encode_view(&h->tmaps.Bs[1], Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 32, 2, false) &&
-                         encode_view(&h->tmaps.Bs[2], Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 64, 2, false)))
+                         encode_view(&h->tmaps.Bs[0], Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 16, qmcd_sb_nq(h->K), false) &&
+                         encode_view(&h->tmaps.Bs[1], Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 32, qmcd_sb_nq(h->K), false) &&
+                         encode_view(&h->tmaps.Bs[2], Ainv_dev, h->N, h->N, (size_t)h->N * h->N, h->batch, 8, 64, qmcd_sb_nq(h->K), false)))
         h->tmaps_ok = false;
     refresh_use_tma(h);
     CK(h, cudaMemsetAsync(h->P.m, 0, (size_t)h->batch * 4, h->stream));
@@ -542,9 +543,9 @@ extern "C" int qmcd_sweep(qmcd_handle h, int j_begin, int n_moves,
     QmcdArgs a = base_args(h, QMCD_MODE_SWEEP);
     a.j_begin = j_begin; a.n_moves = n_moves; a.v = proposals_dev;
     a.mask = mask_dev; a.uniforms = uniforms_dev; a.R_out = R_out_dev; a.acc_out = acc_out_dev;
-    if (h->P.la_tma && !(encode_proposals(&h->tmaps.Vs[0], proposals_dev, n_moves, h->N, h->batch, 16) &&
-                         encode_proposals(&h->tmaps.Vs[1], proposals_dev, n_moves, h->N, h->batch, 32) &&
-                         encode_proposals(&h->tmaps.Vs[2], proposals_dev, n_moves, h->N, h->batch, 64))) { h->la_opt = 0; refresh_use_tma(h); a.P = h->P; }
+    if (h->P.la_tma && !(encode_proposals(&h->tmaps.Vs[0], proposals_dev, n_moves, h->N, h->batch, 16, qmcd_sb_nq(h->K)) &&
+                         encode_proposals(&h->tmaps.Vs[1], proposals_dev, n_moves, h->N, h->batch, 32, qmcd_sb_nq(h->K)) &&
+                         encode_proposals(&h->tmaps.Vs[2], proposals_dev, n_moves, h->N, h->batch, 64, qmcd_sb_nq(h->K)))) { h->la_opt = 0; refresh_use_tma(h); a.P = h->P; }
     // (the blocked look-ahead with M in global memory has no lock-step variant: that combination runs per move)
     a.blocked = (h->lookahead != 1 && !h->P.slot_replace && h->P.blk_ok && (h->P.m_in_smem || !h->P.lockstep) &&
                  (((uintptr_t)proposals_dev & 15) == 0)) ? 1 : 0;

@@ -393,12 +393,12 @@ __device__ __forceinline__ void qmcd_kernel_body(const QmcdArgs& A, const QmcdTm
     if (BLOCKED == 3) {                              // blocked sweep with M in global memory (K too large for shared memory)
         int m = __ldcg(P.m + b);
         qmcd_load_state<false>(P, s, w, m);
-        m = qmcd_sweep_blocked<false, false>(A, s, cl, w, m);
+        m = P.la_tma ? qmcd_sweep_sb<false, false>(A, s, cl, w, m) : qmcd_sweep_blocked<false, false>(A, s, cl, w, m);
         if (r == 0 && threadIdx.x == 0) { P.sj[b] = -1; P.m[b] = m; }
     } else if (BLOCKED) {
         int m = __ldcg(P.m + b);
         qmcd_load_state<true>(P, s, w, m);
-        m = P.la_tma ? qmcd_sweep_sb<BLOCKED == 2>(A, s, cl, w, m) : qmcd_sweep_blocked<BLOCKED == 2, true>(A, s, cl, w, m);
+        m = P.la_tma ? qmcd_sweep_sb<BLOCKED == 2, true>(A, s, cl, w, m) : qmcd_sweep_blocked<BLOCKED == 2, true>(A, s, cl, w, m);
         qmcd_writeback_M<true>(P, s, w, m);
         if (r == 0 && threadIdx.x == 0) { P.sj[b] = -1; P.m[b] = m; }
     } else {

@@ -25,28 +25,31 @@
 
 #define QMCD_SB_MAXU 8          // output tiles (16 x 8) per warp
 #define QMCD_SB_NS 3            // ring stages (== QMCD_LA_NS: the mbarriers of qmcd_la_init_barriers)
-#define QMCD_SB_CW 16           // columns per stage
 #define QMCD_SB_MAXR 16         // elements per thread in the cluster-wide sum
+#define QMCD_SB_KMAX 128        // largest delay served (beyond it SBG, G, X, Y, U no longer fit beside the ring)
+// k-groups of 8 columns per ring stage: 2 for K <= 64 (M in shared memory), 1 beyond (M in global memory; the stages
+// hold up to 2 x 128 queue rows)
+__host__ __device__ inline int qmcd_sb_nq(int K) { return K <= 64 ? 2 : 1; }
 
 // largest queue length (rounded up to 8) a super-block of `shape` proposals may start at: 2 ceil(m0/8) + shape/8
 // output-tile columns over 8 / (shape/16) warps per row block must stay <= QMCD_SB_MAXU per warp (shape 64: 32; 32: 112,
 // kept at 56 for the size of a ring stage; 16: 248)
-__host__ __device__ inline int qmcd_sb_m0p_max(int shape) { return shape == 64 ? 32 : shape == 32 ? 56 : 248; }
+__host__ __device__ inline int qmcd_sb_m0p_max(int shape, int K) { return shape == 64 ? 32 : shape == 32 ? (K <= 64 ? 56 : 96) : 248; }
 __host__ __device__ inline size_t qmcd_sb_stage_bytes(int K) {
     const int Kp = qmcd_blk_Kp(K);
     int rows = 0;
     for (int shape = 16; shape <= 64; shape *= 2) {
-        const int mp = Kp < qmcd_sb_m0p_max(shape) ? Kp : qmcd_sb_m0p_max(shape);
+        const int mp = Kp < qmcd_sb_m0p_max(shape, K) ? Kp : qmcd_sb_m0p_max(shape, K);
         const int mb = (mp + 31) & ~31;            // C and W come in boxes of 32 rows
         if (2 * shape + 2 * mb > rows) rows = 2 * shape + 2 * mb;
     }
-    return (size_t)rows * (QMCD_SB_CW * 8);
+    return (size_t)rows * (qmcd_sb_nq(K) * 64);
 }
 __host__ __device__ inline size_t qmcd_sb_g_doubles(int K) {
     const int Kp = qmcd_blk_Kp(K);
     size_t n = 0;
     for (int shape = 16; shape <= 64; shape *= 2) {
-        const int mp = Kp < qmcd_sb_m0p_max(shape) ? Kp : qmcd_sb_m0p_max(shape);
+        const int mp = Kp < qmcd_sb_m0p_max(shape, K) ? Kp : qmcd_sb_m0p_max(shape, K);
         const size_t v = (size_t)shape * (2 * mp + shape);
         if (v > n) n = v;
     }
@@ -95,19 +98,20 @@ __device__ inline QmcdSb qmcd_sb_carve(double* base, int K) {
 // Rows of B0 past N and proposals past the launch are zero-filled by TMA; entries of rows / columns >= nb are never read.
 // `itc` = chunks this CTA has pushed through the ring.
 // ---------------------------------------------------------------------------
-template <int NU>     // output tiles per warp (tiles past the last one repeat the first and are dropped: the loop has no branch)
+template <int NU, int NQ>     // NU output tiles per warp (tiles past the last one repeat the first and are dropped: the loop
+                              // has no branch), NQ k-groups of 8 columns per stage
 __device__ __noinline__ void qmcd_sb_strips(const QmcdArgs& A, const QmcdSmem& s, const QmcdSb& sb, cg::cluster_group& cl,
                                             const QmcdWalker& w, int t0, int j0, int shape, int m0, unsigned& itc) {
     constexpr int NS = QMCD_SB_NS;
     const QmcdDev& P = A.P;
     const QmcdTmaps& TM = *s.tm;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, g = lane >> 2, c = lane & 3;
-    const int len = w.khi - w.klo, nch = len / QMCD_SB_CW;
+    const int len = w.khi - w.klo, nch = len / (8 * NQ);
     const int nP = (m0 + 7) >> 3, nrb = shape >> 4, wpr = 8 / nrb;
     const int nQB = (nP + 3) >> 2;                              // 32-row boxes of C and of W (rows past m0: stale, finite, unused)
     const int ncu = 2 * nP + (shape >> 3), ld = 8 * ncu;
     const unsigned STAGE = (unsigned)qmcd_sb_stage_bytes(P.K);
-    const unsigned stage_tx = 256u * shape + 8192u * nQB;
+    const unsigned stage_tx = (unsigned)NQ * (128u * shape + 4096u * nQB);
     const int si = shape == 64 ? 2 : shape == 32 ? 1 : 0;
     unsigned char* smem = reinterpret_cast<unsigned char*>(s.red);
     const unsigned bar0 = qmcd_su32(smem + QMCD_LA_BAR_OFF);
@@ -119,19 +123,19 @@ __device__ __noinline__ void qmcd_sb_strips(const QmcdArgs& A, const QmcdSmem& s
         if (u > 0) qmcd_mbar_wait(bar0 + 8 * NS + 8 * st, (u - 1) & 1);
         unsigned dst = ring0 + st * STAGE;
         const unsigned fb = bar0 + 8 * st;
-        const int kg = (w.klo >> 3) + 2 * kc;
+        const int kg = (w.klo >> 3) + NQ * kc;
         qmcd_mbar_expect_tx(fb, stage_tx);
-        qmcd_tma_load4(dst, &TM.Bs[si], 0, j0, kg, w.b, fb); dst += 128u * shape;
-        qmcd_tma_load4(dst, &TM.Vs[si], 0, t0, kg, w.b, fb); dst += 128u * shape;
-        for (int u32 = 0; u32 < nQB; ++u32) { qmcd_tma_load4_hint(dst, &TM.C32, 0, 32 * u32, kg, w.b, fb, pol_keep); dst += 4096; }
-        for (int u32 = 0; u32 < nQB; ++u32) { qmcd_tma_load4_hint(dst, &TM.W32, 0, 32 * u32, kg, w.b, fb, pol_keep); dst += 4096; }
+        qmcd_tma_load4(dst, &TM.Bs[si], 0, j0, kg, w.b, fb); dst += 64u * NQ * shape;
+        qmcd_tma_load4(dst, &TM.Vs[si], 0, t0, kg, w.b, fb); dst += 64u * NQ * shape;
+        for (int u32 = 0; u32 < nQB; ++u32) { qmcd_tma_load4_hint(dst, &TM.C32, 0, 32 * u32, kg, w.b, fb, pol_keep); dst += 2048 * NQ; }
+        for (int u32 = 0; u32 < nQB; ++u32) { qmcd_tma_load4_hint(dst, &TM.W32, 0, 32 * u32, kg, w.b, fb, pol_keep); dst += 2048 * NQ; }
     };
     if (tid == 0) {
         for (int kc = 0; kc < NS - 1 && kc < nch; ++kc) issue(kc);
     }
-    // this warp: row block rb, output-tile columns cu = wi + wpr i.  Stage layout in doubles: B0 rows [2][shape][8] at 0,
-    // V rows at 16 shape, C boxes [2][32][8] at 32 shape, W boxes after them.  Right operand of tile column cu: BYTE offset
-    // at k-group 0 (roff) and k-group stride (rqs); left operand: B0 rows (P, D) or V rows (Q: qs)
+    // this warp: row block rb, output-tile columns cu = wi + wpr i.  Stage layout in doubles: B0 rows [NQ][shape][8] at 0,
+    // V rows at 8 NQ shape, C boxes [NQ][32][8] at 16 NQ shape, W boxes after them.  Right operand of tile column cu: BYTE
+    // offset at k-group 0 (roff) and k-group stride (rqs); left operand: B0 rows (P, D) or V rows (Q: qs)
     const int rb = wid / wpr, wi = wid - rb * wpr;
     unsigned roff[NU], rqs[NU];
     bool qs[NU];
@@ -139,9 +143,9 @@ __device__ __noinline__ void qmcd_sb_strips(const QmcdArgs& A, const QmcdSmem& s
     for (int i = 0; i < NU; ++i) {
         int cu = wi + wpr * i;
         if (cu >= ncu) cu = wi;                                 // a tile this warp does not have: recompute its first one
-        if (cu < nP) { roff[i] = 32 * shape + 512 * (cu >> 2) + ((cu & 3) * 8 + g) * 8 + 2 * c; rqs[i] = 256 * 8; qs[i] = false; }
-        else if (cu < 2 * nP) { const int u8 = cu - nP; roff[i] = 32 * shape + 512 * nQB + 512 * (u8 >> 2) + ((u8 & 3) * 8 + g) * 8 + 2 * c; rqs[i] = 256 * 8; qs[i] = true; }
-        else { const int d = cu - 2 * nP; roff[i] = 16 * shape + (d * 8 + g) * 8 + 2 * c; rqs[i] = 8 * shape * 8; qs[i] = false; }
+        if (cu < nP) { roff[i] = 16 * NQ * shape + 256 * NQ * (cu >> 2) + ((cu & 3) * 8 + g) * 8 + 2 * c; rqs[i] = 256 * 8; qs[i] = false; }
+        else if (cu < 2 * nP) { const int u8 = cu - nP; roff[i] = 16 * NQ * shape + 256 * NQ * nQB + 256 * NQ * (u8 >> 2) + ((u8 & 3) * 8 + g) * 8 + 2 * c; rqs[i] = 256 * 8; qs[i] = true; }
+        else { const int d = cu - 2 * nP; roff[i] = 8 * NQ * shape + (d * 8 + g) * 8 + 2 * c; rqs[i] = 8 * shape * 8; qs[i] = false; }
         roff[i] *= 8;
     }
     double acc[NU][2][2];
@@ -153,9 +157,9 @@ __device__ __noinline__ void qmcd_sb_strips(const QmcdArgs& A, const QmcdSmem& s
         const unsigned stg = ring0 + st * STAGE;
         qmcd_mbar_wait(bar0 + 8 * st, u & 1);
         if (wid == (kc & 7) && lane == 0 && kc + NS - 1 < nch) issue(kc + NS - 1);
-        const unsigned Lb = stg + loffB, Lv = Lb + 128u * shape;        // rows 8..15 of the block at + 512 bytes
+        const unsigned Lb = stg + loffB, Lv = Lb + 64u * NQ * shape;    // rows 8..15 of the block at + 512 bytes
 #pragma unroll
-        for (int q = 0; q < 2; ++q) {
+        for (int q = 0; q < NQ; ++q) {
             const double2 lb0 = qmcd_lds128s(Lb + q * qst), lb1 = qmcd_lds128s(Lb + q * qst + 512);
             const double2 lv0 = qmcd_lds128s(Lv + q * qst), lv1 = qmcd_lds128s(Lv + q * qst + 512);
             double2 bv[NU];
@@ -278,8 +282,9 @@ __device__ __noinline__ void qmcd_sb_append(const QmcdArgs& A, const QmcdSmem& s
 // The sweep loop in super-blocks (M in shared memory, replicated in every CTA of the cluster).  Returns the queue
 // length at the end.  LS: the lock-step variant, a compile-time flag as in qmcd_sweep_blocked.
 // ---------------------------------------------------------------------------
-template <bool LS>
+template <bool LS, bool MS>
 __device__ int qmcd_sweep_sb(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_group& cl, const QmcdWalker& w, int m) {
+    constexpr int NQ = MS ? 2 : 1;                 // the host pairs M in shared memory with K <= 64 (qmcd_sb_nq)
     const QmcdDev& P = A.P;
     const int tid = threadIdx.x;
     const int N = P.N, K = P.K, Kp = qmcd_blk_Kp(K), RL = qmcd_sb_RL(K);
@@ -318,7 +323,7 @@ __device__ int qmcd_sweep_sb(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_g
                 __syncthreads();
                 if (nb == 0) {
                     QMCD_TICK(cy_la);
-                    qmcd_flush_phase<true>(P, s, cl, w, m);
+                    qmcd_flush_phase<MS>(P, s, cl, w, m);
                     QMCD_TICK(cy_fl);
                     m = 0; pw = 0;
                     continue;
@@ -327,16 +332,16 @@ __device__ int qmcd_sweep_sb(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_g
         }
         const int m0sb = m, nP = (m + 7) >> 3;
         int shape = nb > 32 ? 64 : nb > 16 ? 32 : 16;
-        while (shape > 16 && 8 * nP > qmcd_sb_m0p_max(shape)) shape >>= 1;
+        while (shape > 16 && 8 * nP > qmcd_sb_m0p_max(shape, K)) shape >>= 1;
         nb = min(nb, shape);
         const int ld = 8 * (2 * nP + (shape >> 3));
         {
             unsigned itc = (unsigned)s.iflag[12];
             const int nu = (2 * nP + (shape >> 3) + (128 / shape) - 1) / (128 / shape);     // output tiles per warp
-            if (nu <= 2) qmcd_sb_strips<2>(A, s, sb, cl, w, t, j0, shape, m, itc);
-            else if (nu <= 4) qmcd_sb_strips<4>(A, s, sb, cl, w, t, j0, shape, m, itc);
-            else if (nu <= 6) qmcd_sb_strips<6>(A, s, sb, cl, w, t, j0, shape, m, itc);
-            else qmcd_sb_strips<QMCD_SB_MAXU>(A, s, sb, cl, w, t, j0, shape, m, itc);
+            if (nu <= 2) qmcd_sb_strips<2, NQ>(A, s, sb, cl, w, t, j0, shape, m, itc);
+            else if (nu <= 4) qmcd_sb_strips<4, NQ>(A, s, sb, cl, w, t, j0, shape, m, itc);
+            else if (nu <= 6) qmcd_sb_strips<6, NQ>(A, s, sb, cl, w, t, j0, shape, m, itc);
+            else qmcd_sb_strips<QMCD_SB_MAXU, NQ>(A, s, sb, cl, w, t, j0, shape, m, itc);
             if (tid == 0) s.iflag[12] = (int)itc;      // (read again only after the barriers below)
         }
         QMCD_TICK(cy_la);
@@ -366,9 +371,10 @@ __device__ int qmcd_sweep_sb(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_g
             }
             __syncthreads();
             int na = 0;
-            const unsigned accmask = qmcd_blk_chain<true>(A, s, x, w, RL, t + o, j0 + o, L, m, na);
+            const unsigned accmask = qmcd_blk_chain<MS>(A, s, x, w, RL, t + o, j0 + o, L, m, na);
             if (tid < na) sb.alsb[na_sb + tid] = o + x.al[tid];
-            __syncthreads();                       // Rb of the last move, alsb
+            // M in global memory is written by the leader CTA alone: the others read it again in the next block
+            if (!MS && P.S > 1) cl.sync(); else __syncthreads();   // (and: Rb of the last move, alsb)
             if (w.r == 0 && tid < L) {
                 const size_t tb = (size_t)(t + o + tid) * P.batch + w.b;
                 if (A.R_out) A.R_out[tb] = x.Rb[tid];
@@ -392,10 +398,10 @@ __device__ int qmcd_sweep_sb(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_g
         // flush when the queue is full -- or nearly full: a few moves early is neutral
         if (LS) {
             if (pw >= K) {                             // every walker closes its window here, rank m <= K
-                if (m > 0) { qmcd_flush_phase<true>(P, s, cl, w, m); m = 0; QMCD_TICK(cy_fl); }
+                if (m > 0) { qmcd_flush_phase<MS>(P, s, cl, w, m); m = 0; QMCD_TICK(cy_fl); }
                 pw = 0;
             }
-        } else if (K - m < thresh) { qmcd_flush_phase<true>(P, s, cl, w, m); m = 0; QMCD_TICK(cy_fl); }
+        } else if (K - m < thresh) { qmcd_flush_phase<MS>(P, s, cl, w, m); m = 0; QMCD_TICK(cy_fl); }
     }
     if (LS && w.r == 0 && tid == 0) P.counters[(size_t)w.b * 8 + 7] = pw;
     if (prof) {
