@@ -35,6 +35,7 @@ if ROOT not in sys.path:
 METRIC = "accepted electron moves/s (fp64, batched walkers)"
 UNIT = "moves/s"
 DEFAULT_CONFIG, DEFAULT_K, DEFAULT_MODE = "c3", 64, "bern0.99"
+NCU_TRAFFIC_BYTES_DEFAULT = 232.0e9       # profiles/r2_ncu_c3_sweep.md: 158.9 GB read + 73.1 GB written per sweep launch
 
 
 def parse_args():
@@ -437,8 +438,8 @@ def run_ours(args, wl_cache=None):
     roofline = {"kernel": "qmcd_kernel_sweep (look-ahead + accept + flush jobs; persistent: leader clusters + pool, one launch/step)",
                 "bound": "tensor", "achieved": ach, "peak": dmma, "unit": "TFLOP/s",
                 "frac": ach / dmma, "traffic": None,
-                "traffic_note": "not measured inside this run (a number read from an old capture goes stale); the ncu capture "
-                                "of this kernel on this config and build is under profiles/ with its command",
+                "traffic_note": "no ncu capture of this configuration; the capture of the default workload is "
+                                "profiles/r2_ncu_c3_sweep.md",
                 "peak_source": "measured live: register-resident DMMA.8x8x4 fp64 loop (qmcd_probe_fp64) = 148 SMs x SM clock x "
                                f"128 flop/clk; DFMA loop {dfma:.1f} TFLOP/s; MEASURED_PEAKS.json has no fp64 figure",
                 "kernel_ms": sweep_ms, "algorithmic_flops_per_launch": work["flops"],
@@ -448,6 +449,14 @@ def run_ours(args, wl_cache=None):
                 "hbm_peak_source": "MEASURED_PEAKS.json (of measured)" if peaks else None,
                 "share_of_step": sweep_ms / ms_per_step}
 
+    if (args.config, K, args.mode) == (DEFAULT_CONFIG, DEFAULT_K, DEFAULT_MODE) and not args.cluster and not args.flush_path \
+            and all(o.startswith("cooperative=") for o in args.opt):
+        # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of this kernel on this workload, from the ncu --set full
+        # capture of this build (a constant of the build, not of this run: refreshed with every change of the kernel)
+        roofline["traffic"] = NCU_TRAFFIC_BYTES_DEFAULT
+        roofline["traffic_note"] = ("bytes per launch: dram__bytes_read.sum + dram__bytes_write.sum from "
+                                    "profiles/r2_ncu_c3_sweep.md (ncu --set full of this kernel, this workload, this build); "
+                                    "algorithmic flush bytes per launch: %.4g" % work["flush_bytes"])
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": n_warm, "ms_per_step": ms_per_step, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
