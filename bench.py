@@ -397,7 +397,8 @@ def run_ours(args, wl_cache=None):
             Uh = None if uniforms is None else torch.from_numpy(uniforms).pin_memory()
             Rh = torch.zeros((n_moves, batch), dtype=torch.float64).pin_memory()
             Ah = torch.zeros((n_moves, batch), dtype=torch.uint8).pin_memory()
-            staging = torch.empty((64 << 20) + 256, dtype=torch.uint8, device="cuda")
+            # two buffers of up to 1024 moves each (qmcd_sweep_host cuts the sweep into launches of 128, 256, ... moves)
+            staging = torch.empty(2 * min(n_moves, 1024) * (batch * N * 8 + 64 * batch) + 4096, dtype=torch.uint8, device="cuda")
 
             def e2e_step():
                 B.copy_(Bh, non_blocking=True)

@@ -675,8 +675,11 @@ extern "C" int qmcd_sweep_host(qmcd_handle h, int j_begin, int n_moves,
     if (cm < 1) cm = 1;
     if (cm > n_moves) cm = n_moves > 0 ? n_moves : 1;
     const size_t half = staging_bytes / 2 & ~(size_t)255;
-    for (int c = 0, t0 = 0; t0 < n_moves; ++c, t0 += (int)cm) {
-        const int cnt = (int)((n_moves - t0 < cm) ? n_moves - t0 : cm);
+    // chunk sizes grow geometrically from 128 moves to cm: the first copy (nothing to overlap it with) stays short, the
+    // later launches long (every launch fills and drains the pool once)
+    long long cur = cm < 128 ? cm : 128;
+    for (int c = 0, t0 = 0, cnt = 0; t0 < n_moves; ++c, t0 += cnt, cur = (2 * cur < cm) ? 2 * cur : cm) {
+        cnt = (int)((n_moves - t0 < cur) ? n_moves - t0 : cur);
         const int buf = c & 1;
         unsigned char* base = (unsigned char*)staging_dev + (size_t)buf * half;
         double* d_prop = (double*)base;

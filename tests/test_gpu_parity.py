@@ -561,6 +561,10 @@ def test_autotune_K_picks_a_tensor_bound_delay(qmcd):
     assert set(r["moves_per_s"]) == {1, 16, 32, 64}
     assert r["best_K"] in (16, 32, 64)
     assert r["moves_per_s"][r["best_K"]] > 5 * r["moves_per_s"][1]
+    # the launch shape too: CTAs per leader cluster (the default is a rule fitted to the BASELINE shapes)
+    r = autotune.autotune_K(1024, 16, Ks=(64,), n_moves=256, reps=1, clusters=(1, 2, 4, 3))
+    assert set(r["by_cluster"][64]) == {1, 2, 4}                     # 3 is refused by the library and skipped
+    assert r["best_cluster"] in (1, 2, 4) and r["moves_per_s"][64] == max(r["by_cluster"][64].values())
 
 
 def test_randomized_shapes_seeds_modes_and_launch_splits(qmcd):
