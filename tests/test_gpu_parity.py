@@ -328,6 +328,41 @@ def test_superblock_lookahead_matches_oracle(qmcd, N, K, batch, cluster, mode, j
         assert np.all(g["pending"] == 0)
 
 
+@pytest.mark.parametrize("N,K,batch,cluster,p", [
+    (128, 1, 3, 1, 0.9),       # K = 1: the classic Sherman-Morrison update (Eqs. 1-2)
+    (192, 1, 2, 2, 1.0),       # N a multiple of 64 but not of 128
+    (1024, 1, 2, 1, 0.5),      # 8 tiles per flush through the pool
+    (2048, 2, 2, 1, 0.8),      # K = 2: ranks 1 and 2
+    (4096, 2, 1, 2, 0.99),
+    (256, 2, 40, 1, 0.7),      # 40 walkers, 64-row tiles
+])
+def test_rank1_and_rank2_flush_matches_oracle(qmcd, N, K, batch, cluster, p):
+    """K <= 2 (in particular K = 1, the classic Sherman-Morrison baseline of Eqs. 1-2): rank-1 / rank-2 flush jobs through
+    the tile kernels and the pool against the oracle's rank-1 path (path 1), launches cut in two."""
+    import torch
+    n_moves = min(N, 300) + 7
+    wl = inputs.make_workload(batch, N, n_moves=n_moves, seed=77)
+    mask = wl.bernoulli_mask(p)
+    B1 = wl.Ainv.copy(); R1, acc1, _ = oracle.run(1, B1, 1, wl.proposals, mask=mask)      # K-independent (PAPER.md:95)
+    q = qmcd.Qmcd(N, K, batch)
+    q.set_option("cluster", cluster)
+    B = _dev(wl.Ainv)
+    q.set_inverse(B)
+    R = torch.zeros((n_moves, batch), dtype=torch.float64, device="cuda")
+    acc = torch.zeros((n_moves, batch), dtype=torch.uint8, device="cuda")
+    q.sweep(0, _dev(wl.proposals[:100]), mask=_dev(mask[:100]), R_out=R[:100], acc_out=acc[:100])
+    q.sweep(100 % N, _dev(wl.proposals[100:]), mask=_dev(mask[100:]), R_out=R[100:], acc_out=acc[100:])
+    q.flush()
+    st, _ = q.status()
+    cnt = q.counters().cpu().numpy()
+    q.close()
+    assert st == 0
+    assert np.array_equal(acc.cpu().numpy(), acc1)
+    assert _rel(R.cpu().numpy(), R1) <= RTOL_RATIO
+    assert np.max(np.abs(B.cpu().numpy() - B1)) <= 1e-10 * max(1.0, np.abs(B1).max())
+    assert np.array_equal(cnt[:, 0], acc1.sum(axis=0))
+
+
 @pytest.mark.parametrize("K", [1, 16, 32])
 def test_c1_full_size_vs_rank1_oracle(qmcd, K):
     """BASELINE.json configs[1] at full size, in bench.py's launch configuration (qmcd_sweep):
