@@ -11,6 +11,7 @@
 #include "../../include/qmcd.h"
 #include "qmcd_kernel.cuh"
 #include "qmcd_invert.cuh"
+#include "qmcd_invert_blocked.cuh"
 #include "qmcd_ratio.cuh"
 
 enum { QMCD_IDLE = 0, QMCD_PROPOSED = 1 };
@@ -34,6 +35,7 @@ struct qmcd_ctx {
     bool tmaps_ok;            // C, W, M, Wk encoded (and B, B16 once an inverse is adopted)
     double* rpart; unsigned* rcnt;   // qmcd_ratio kernel scratch
     int ratio_opt;            // option "ratio_kernel": 1 = qmcd_ratio through the dedicated kernel (qmcd_ratio.cuh)
+    int invb_opt;             // option "invert_blocked": 1 = qmcd_invert runs the blocked Gauss-Jordan kernel when the batch is co-resident
     int la_opt;               // option "la_tma": 1 = TMA-ring look-ahead in qmcd_sweep when the shape allows
     bool la_fit;              // the kernel's shared memory was sized with the look-ahead ring
     size_t ctl_off, ctl_bytes;    // job words inside the workspace (zeroed before every pooled launch)
@@ -327,7 +329,7 @@ extern "C" int qmcd_create(qmcd_handle* out, int N, int K, int batch,
     P.fin = (unsigned*)(ws + L.fin); P.ctrl = (unsigned*)(ws + L.ctrl);
     P.chain_regs = 1; P.pool = 0;
     P.flush_path = 0; P.use_tma = 0; P.ldMg = qmcd_ldMg_host(K);
-    h->tma_opt = 1; h->la_opt = 1; h->la_fit = false; h->ratio_opt = 1;
+    h->tma_opt = 1; h->la_opt = 1; h->la_fit = false; h->ratio_opt = 1; h->invb_opt = 1;
     h->rpart = (double*)(ws + L.rpart); h->rcnt = (unsigned*)(ws + L.rcnt);
     encode_queue_tmaps(h);
     P.tile_rows = (K <= 64 && N >= 2048) ? 128 : 64;
@@ -555,10 +557,55 @@ extern "C" int qmcd_sweep(qmcd_handle h, int j_begin, int n_moves,
 // ---- batched on-device inversion (qmcd_invert.cuh)
 static size_t inv_smem_bytes(int N) { return (size_t)N * 16; }
 
+// CTAs per walker of the blocked kernel are bounded so that its candidate records stay small: batch * C <= 512
+static int invb_cmax(int batch) { int c = 512 / batch; if (c < 1) c = 1; if (c > QMCD_INV_CMAX) c = QMCD_INV_CMAX; return c; }
 extern "C" size_t qmcd_invert_scratch_bytes(int N, int batch) {
     if (N < 1 || batch < 1 || inv_smem_bytes(N) > 227 * 1024) return 0;
     return al256((size_t)batch * N * 4) + al256((size_t)batch * QMCD_INV_CMAX * 8) +
-           al256((size_t)batch * QMCD_INV_CMAX * 4) + al256((size_t)batch * 4);
+           al256((size_t)batch * QMCD_INV_CMAX * 4) + al256((size_t)batch * 4) +
+           al256((size_t)batch * 2 * invb_cmax(batch) * QMCD_INVB_REC * 8) +          // blocked kernel: candidate records,
+           al256((size_t)batch * 2 * 2 * QMCD_INVB_KB * 8) +                         // slot k's data,
+           al256((size_t)batch * QMCD_INVB_KB * QMCD_INVB_KB * 8);                   // L | d | later multipliers
+}
+
+// The blocked Gauss-Jordan kernel (qmcd_invert_blocked.cuh): panel width KB <= 16, C CTAs per walker and the chunk width
+// chosen so that the whole batch is co-resident (one cooperative launch) with the widest panel that fits shared memory.
+// Returns QMCD_OK with *done = 1 when it ran; *done = 0 = not applicable (the caller runs the unblocked kernel).
+static int launch_invert_blocked(qmcd_ctx* h, const double* A_dev, double* Ainv_dev, unsigned char* sc, int* info, int* done) {
+    *done = 0;
+    const int N = h->N, batch = h->batch;
+    const size_t cap = 227 * 1024 - 1024;                // (the kernel also has a few hundred bytes of static shared memory)
+    int dev = 0, sms = 0;
+    CK(h, cudaGetDevice(&dev));
+    CK(h, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CK(h, cudaFuncSetAttribute(qmcd_invert_blocked_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cap));
+    const int threads = QMCD_INV_THREADS;
+    int CH = 512; while (CH / 2 >= N && CH > 32) CH /= 2;
+    int bestC = 0, bestKB = 0; size_t best_smem = 0;
+    for (int KB = QMCD_INVB_KB; KB >= 2 && !bestC; KB /= 2) {
+        for (int C = invb_cmax(batch); C >= 1; --C) {
+            if (C > 1 && (N + C - 1) / C < 8) continue;                  // at least 8 slots per CTA
+            const size_t smem = qmcd_invb_smem_bytes(N, C, KB, CH);
+            if (smem > cap) break;                                       // fewer CTAs per walker need more still
+            int per_sm = 0;
+            CK(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, qmcd_invert_blocked_kernel, threads, smem));
+            if ((long long)C * batch <= (long long)sms * per_sm) { bestC = C; bestKB = KB; best_smem = smem; break; }
+        }
+    }
+    if (!bestC) return QMCD_OK;                                          // the batch is not co-resident at any width: unblocked kernel
+    QmcdInvBArgs a;
+    a.N = N; a.batch = batch; a.C = bestC; a.KB = bestKB; a.CH = CH;
+    a.A = A_dev; a.X = Ainv_dev; a.info = info;
+    a.piv = (int*)sc; sc += al256((size_t)batch * N * 4);
+    sc += al256((size_t)batch * QMCD_INV_CMAX * 8) + al256((size_t)batch * QMCD_INV_CMAX * 4) + al256((size_t)batch * 4);
+    a.cand = (double*)sc; sc += al256((size_t)batch * 2 * invb_cmax(batch) * QMCD_INVB_REC * 8);
+    a.kdat = (double*)sc; sc += al256((size_t)batch * 2 * 2 * QMCD_INVB_KB * 8);
+    a.lf = (double*)sc;
+    void* kargs[] = {(void*)&a};
+    CK(h, cudaLaunchCooperativeKernel((void*)qmcd_invert_blocked_kernel, dim3((unsigned)(batch * bestC)), dim3((unsigned)threads),
+                                      kargs, best_smem, h->stream));
+    *done = 1;
+    return QMCD_OK;
 }
 
 extern "C" int qmcd_invert(qmcd_handle h, const double* A_dev, double* Ainv_dev,
@@ -568,6 +615,14 @@ extern "C" int qmcd_invert(qmcd_handle h, const double* A_dev, double* Ainv_dev,
     const size_t need = qmcd_invert_scratch_bytes(N, batch);
     if (need == 0 || scratch_bytes < need || ((uintptr_t)scratch_dev & 255)) return QMCD_EINVAL;
     if (h->state != QMCD_IDLE) return QMCD_ESTATE;
+    if (h->invb_opt) {                                   // blocked kernel: the matrix crosses HBM N/16 times instead of N times
+        int* info_b = info_dev ? info_dev : (int*)((unsigned char*)scratch_dev + al256((size_t)batch * N * 4) +
+                                                   al256((size_t)batch * QMCD_INV_CMAX * 8) + al256((size_t)batch * QMCD_INV_CMAX * 4));
+        CK(h, cudaMemsetAsync(info_b, 0, (size_t)batch * 4, h->stream));
+        int done = 0;
+        const int rc = launch_invert_blocked(h, A_dev, Ainv_dev, (unsigned char*)scratch_dev, info_b, &done);
+        if (rc != QMCD_OK || done) return rc;
+    }
     const size_t smem = inv_smem_bytes(N);
     CK(h, cudaFuncSetAttribute(qmcd_invert_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int dev = 0, sms = 0;
@@ -739,6 +794,11 @@ extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
         refresh_use_tma(h);
         return QMCD_OK;
     }
+    if (!strcmp(key, "invert_blocked")) {          // 0: qmcd_invert runs the unblocked kernel (one pass over the matrix per pivot)
+        if (value < 0 || value > 1) return QMCD_EINVAL;
+        h->invb_opt = value;
+        return QMCD_OK;
+    }
     if (!strcmp(key, "ratio_kernel")) {            // 0: qmcd_ratio through the cluster kernel's look-ahead (the per-move sweep's arithmetic)
         if (value < 0 || value > 1) return QMCD_EINVAL;
         h->ratio_opt = value;
@@ -796,6 +856,7 @@ extern "C" int qmcd_get_option(qmcd_handle h, const char* key) {
     if (!strcmp(key, "tile_rows")) return h->P.tile_rows;
     if (!strcmp(key, "tma")) return h->P.use_tma;
     if (!strcmp(key, "la_tma")) return h->P.la_tma;
+    if (!strcmp(key, "invert_blocked")) return h->invb_opt;
     if (!strcmp(key, "ratio_kernel")) return h->ratio_opt;
     if (!strcmp(key, "flush_path")) return h->P.flush_path;
     if (!strcmp(key, "lookahead")) return h->lookahead;
