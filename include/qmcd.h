@@ -164,7 +164,9 @@ size_t qmcd_sweep_host_min_staging(int N, int batch);
 
 /* Batched on-device inversion (the "explicit copy of the matrix inverse" the
  * method starts from and may refresh): Ainv_dev[b] <- A_dev[b]^-1 for every walker, by
- * Gauss-Jordan elimination with partial pivoting in one cooperative launch.  A_dev, Ainv_dev:
+ * Gauss-Jordan elimination with partial pivoting in one cooperative launch -- blocked (panels of 16
+ * pivot columns: the matrix crosses HBM N/16 times) when the whole batch is co-resident, else one
+ * pass per pivot; the same pivots and arithmetic either way (option "invert_blocked").  A_dev, Ainv_dev:
  * [batch][N][N] row-major fp64 (A: row = orbital, column = electron; may be the same buffer).
  * scratch_dev: caller-owned, 256-byte aligned, >= qmcd_invert_scratch_bytes(N, batch) bytes
  * (0 = N too large for the kernel's shared memory, N <= 14528).  info_dev: [batch] int32, 0 or
@@ -204,6 +206,8 @@ int qmcd_invert_static(qmcd_handle h, const double* A_dev, double* Ainv_dev, int
  *                   operands stream through a TMA ring once (K <= 128, K even beyond 64, N >= 128, N % 64 == 0, column
  *                   slices of whole 16- / 8-column chunks); 0 = blocks of 16 proposals with LDG / cp.async strips (the
  *                   path of every other shape).
+ *   "invert_blocked" 1 (default): qmcd_invert / qmcd_invert_static run the blocked Gauss-Jordan kernel when the batch is
+ *                   co-resident; 0 = the unblocked kernel (one pass over the matrix per pivot).
  *   "ratio_kernel"  1 (default): qmcd_ratio runs the dedicated bandwidth kernel; 0 = the cluster kernel's look-ahead
  *                   (the arithmetic of the per-move sweep, bit for bit).
  *   "flush_path"    0 auto, 1 CUDA-core, 2 DMMA.

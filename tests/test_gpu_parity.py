@@ -987,6 +987,36 @@ def test_invert_matches_oracle_lu_inverse(qmcd, N, batch, seed):
     q.close()
 
 
+@pytest.mark.parametrize("N,batch", [(7, 3), (33, 2), (130, 5), (512, 16), (1000, 3)])
+def test_invert_blocked_equals_unblocked_kernel(qmcd, N, batch):
+    """The blocked Gauss-Jordan kernel (panels of 16 pivot columns, the default) against the unblocked one (option
+    invert_blocked = 0): the same pivots and the same arithmetic in the same order, so the results agree to the last
+    bits; both against the oracle's LU inverse.  Walker 0 starts with a zero (row exchange), the last one holds a NaN."""
+    import torch
+    wl = inputs.make_workload(batch, N, n_moves=1, seed=91)
+    A = wl.A.copy()
+    A[0, 0, 0] = 0.0
+    A[batch - 1, N // 2, N // 3] = np.nan
+    out = {}
+    for blk in (1, 0):
+        q = qmcd.Qmcd(N, 1, batch)
+        q.set_option("invert_blocked", blk)
+        assert q.get_option("invert_blocked") == blk
+        X, info = q.invert(_dev(A))
+        torch.cuda.synchronize()
+        out[blk] = (X.cpu().numpy(), info.cpu().numpy())
+        q.close()
+    # the NaN walker is reported by both (the blocked kernel at the first column whose candidates hold the NaN, the unblocked
+    # one when the NaN reaches a pivot), the others are fine
+    for blk in (1, 0):
+        assert out[blk][1][batch - 1] != 0 and np.all(out[blk][1][:batch - 1] == 0)
+    for w in range(batch - 1):
+        Xo = oracle.inverse(A[w])
+        for blk in (1, 0):
+            assert np.max(np.abs(out[blk][0][w] - Xo)) <= 1e-10 * max(1.0, np.abs(Xo).max())
+        assert np.max(np.abs(out[1][0][w] - out[0][0][w])) <= 1e-13 * max(1.0, np.abs(Xo).max())
+
+
 def test_invert_permutation_singular_and_pipeline(qmcd):
     import torch
     N, batch, K = 96, 3, 8
