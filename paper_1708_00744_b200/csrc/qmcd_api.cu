@@ -36,6 +36,7 @@ struct qmcd_ctx {
     double* rpart; unsigned* rcnt;   // qmcd_ratio kernel scratch
     int ratio_opt;            // option "ratio_kernel": 1 = qmcd_ratio through the dedicated kernel (qmcd_ratio.cuh)
     int invb_opt;             // option "invert_blocked": 1 = qmcd_invert runs the blocked Gauss-Jordan kernel when the batch is co-resident
+    int ratio_sms, ratio_res[2];   // SMs and resident CTAs of the ratio kernel's two variants (0 = not queried yet)
     int la_opt;               // option "la_tma": 1 = TMA-ring look-ahead in qmcd_sweep when the shape allows
     bool la_fit;              // the kernel's shared memory was sized with the look-ahead ring
     size_t ctl_off, ctl_bytes;    // job words inside the workspace (zeroed before every pooled launch)
@@ -405,33 +406,60 @@ static QmcdArgs base_args(qmcd_ctx* h, int mode) {
     return a;
 }
 
-// The dedicated ratio kernel: slices of <= 256 columns (128 when N is odd: 8-byte loads), as many row groups as it
-// takes to put ~6 CTAs on every SM.
+// The dedicated ratio kernel: column slices of 32 NU VEC columns (NU = 4 or 2 vectors per lane and row) x GR groups of queue rows,
+// chosen so that the grid is ONE wave of resident CTAs, as full as possible (measured on c3 shapes: 1024 CTAs in 2.3 waves 23 us,
+// one wave ~15 us: every wave pays the kernel's chain of dependent memory round trips again).
+template <int VEC, int NU>
+static int launch_ratio_t(qmcd_ctx* h, QmcdRatioArgs& a, int sms, int* resident_out, bool fire) {
+    const size_t smem = (size_t)4 * h->K * 8;
+    if (smem > 48 * 1024) CK(h, cudaFuncSetAttribute(qmcd_ratio_kernel<VEC, NU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (!fire) {
+        int per_sm = 0;
+        CK(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, qmcd_ratio_kernel<VEC, NU>, QMCD_THREADS, smem));
+        *resident_out = per_sm * sms;
+        return QMCD_OK;
+    }
+    dim3 grid((unsigned)a.G, (unsigned)a.GR, (unsigned)h->batch);
+    qmcd_ratio_kernel<VEC, NU><<<grid, QMCD_THREADS, smem, h->stream>>>(a);
+    CK(h, cudaGetLastError());
+    return QMCD_OK;
+}
 static int launch_ratio(qmcd_ctx* h, int j, const int* jv, const double* v_dev, double* R_dev) {
     const int N = h->N, K = h->K;
     const bool vec2 = (N % 2 == 0) && (((uintptr_t)v_dev & 15) == 0);
     const int per = 32 * (vec2 ? 2 : 1);                 // columns per lane round
-    int slice = QMCD_RATIO_NU * per;                     // at most 8 rounds per lane
     const int gmax = ratio_gmax(N);
-    while (slice > per && (size_t)h->batch * ((N + slice - 1) / slice) * 8 < 148 * 6 && (N + slice / 2 - 1) / (slice / 2) <= gmax) slice /= 2;
-    int G = (N + slice - 1) / slice;
-    if (G > gmax) { G = gmax; slice = ((N + G - 1) / G + per - 1) / per * per; G = (N + slice - 1) / slice; }
-    int GR = 1;
-    while (GR < 8 && (size_t)h->batch * G * GR < 148 * 6 && 8 * GR < K) GR *= 2;
     QmcdRatioArgs a;
     a.P = h->P; a.j = j; a.jv = jv; a.v = v_dev; a.R_out = R_dev; a.part = h->rpart; a.cnt = h->rcnt;
-    a.G = G; a.GR = GR; a.slice = slice;
-    const size_t smem = (size_t)4 * K * 8;
-    dim3 grid((unsigned)G, (unsigned)GR, (unsigned)h->batch);
-    if (vec2) {
-        if (smem > 48 * 1024) CK(h, cudaFuncSetAttribute(qmcd_ratio_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        qmcd_ratio_kernel<2><<<grid, QMCD_THREADS, smem, h->stream>>>(a);
-    } else {
-        if (smem > 48 * 1024) CK(h, cudaFuncSetAttribute(qmcd_ratio_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        qmcd_ratio_kernel<1><<<grid, QMCD_THREADS, smem, h->stream>>>(a);
+    if (h->ratio_sms == 0) {                             // once per handle: resident CTAs of the two variants
+        int dev = 0;
+        CK(h, cudaGetDevice(&dev));
+        CK(h, cudaDeviceGetAttribute(&h->ratio_sms, cudaDevAttrMultiProcessorCount, dev));
+        int rc = vec2 ? launch_ratio_t<2, 4>(h, a, h->ratio_sms, &h->ratio_res[0], false) : launch_ratio_t<1, 4>(h, a, h->ratio_sms, &h->ratio_res[0], false);
+        if (rc == QMCD_OK) rc = vec2 ? launch_ratio_t<2, 2>(h, a, h->ratio_sms, &h->ratio_res[1], false) : launch_ratio_t<1, 2>(h, a, h->ratio_sms, &h->ratio_res[1], false);
+        if (rc != QMCD_OK) { h->ratio_sms = 0; return rc; }
     }
-    CK(h, cudaGetLastError());
-    return QMCD_OK;
+    // candidates (NU, GR): the largest grid that is still one wave; ties -> wider slices (fewer partial sums)
+    int bestNU = 0, bestGR = 1, bestG = 0, best_ctas = -1;
+    for (int v = 0; v < 2; ++v) {
+        const int NU = v ? 2 : 4, slice = NU * per;
+        int G = (N + slice - 1) / slice;
+        if (G > gmax) continue;
+        for (int GR = 1; GR <= 8; GR *= 2) {
+            if (GR > 1 && 8 * (GR / 2) >= K) break;     // no more row groups than rows
+            const long long ctas = (long long)h->batch * G * GR;
+            if (ctas <= h->ratio_res[v] && ctas > best_ctas) { best_ctas = (int)ctas; bestNU = NU; bestGR = GR; bestG = G; }
+        }
+    }
+    if (bestNU == 0) {                                   // even the smallest grid is more than a wave (many walkers): widest slices, one row group
+        bestNU = 4; bestGR = 1; bestG = (N + 4 * per - 1) / (4 * per);
+        if (bestG > gmax) { bestG = gmax; }
+    }
+    int slice = bestNU * per;
+    if ((long long)bestG * slice < N) { slice = ((N + bestG - 1) / bestG + per - 1) / per * per; bestNU = 4; }   // (N > gmax slices of 4 vectors: not reachable for N <= 32768)
+    a.G = bestG; a.GR = bestGR; a.slice = slice;
+    if (vec2) return bestNU == 2 ? launch_ratio_t<2, 2>(h, a, h->ratio_sms, nullptr, true) : launch_ratio_t<2, 4>(h, a, h->ratio_sms, nullptr, true);
+    return bestNU == 2 ? launch_ratio_t<1, 2>(h, a, h->ratio_sms, nullptr, true) : launch_ratio_t<1, 4>(h, a, h->ratio_sms, nullptr, true);
 }
 
 extern "C" int qmcd_ratio(qmcd_handle h, int j, const double* v_dev, double* R_dev) {

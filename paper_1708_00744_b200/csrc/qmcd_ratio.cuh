@@ -23,7 +23,8 @@ struct QmcdRatioArgs {
     int slice;                // columns per slice (multiple of VEC)
 };
 
-#define QMCD_RATIO_NU 4       // vectors per lane and row: slice <= 128 * VEC columns
+#define QMCD_RATIO_NU 4       // most vectors per lane and row: slice <= 128 * VEC columns
+#define QMCD_RATIO_RB 2       // queue-row pairs whose loads a warp issues together
 
 template <int VEC> struct QmcdVec;
 template <> struct QmcdVec<2> {
@@ -41,8 +42,10 @@ template <> struct QmcdVec<1> {
     static __device__ __forceinline__ double dot(T a, T b, double acc) { return fma(a, b, acc); }
 };
 
-template <int VEC>
-__global__ void __launch_bounds__(QMCD_THREADS, 3) qmcd_ratio_kernel(const QmcdRatioArgs A) {
+// NU = vectors per lane and row (slice = 32 NU VEC columns).  The host sizes the grid to ONE wave of resident CTAs
+// (a second, short wave costs a full ramp of dependent memory round trips on a kernel that lasts ~15 us).
+template <int VEC, int NU>
+__global__ void __launch_bounds__(QMCD_THREADS, (NU <= 2) ? 4 : 3) qmcd_ratio_kernel(const QmcdRatioArgs A) {
     typedef QmcdVec<VEC> V;
     extern __shared__ __align__(16) double rsm[];             // last CTA only: pf | qf | cf | rf, K doubles each
     __shared__ int s_last;
@@ -64,9 +67,9 @@ __global__ void __launch_bounds__(QMCD_THREADS, 3) qmcd_ratio_kernel(const QmcdR
     double* pp = A.part + ((size_t)b * A.G + gc) * (2 * K + 2);
 
     // this lane's elements of the slice: k = lo + VEC (lane + 32 u)
-    typename V::T rj[QMCD_RATIO_NU], vx[QMCD_RATIO_NU];
+    typename V::T rj[NU], vx[NU];
 #pragma unroll
-    for (int u = 0; u < QMCD_RATIO_NU; ++u) {
+    for (int u = 0; u < NU; ++u) {
         const int k = lo + VEC * (lane + 32 * u);
         rj[u] = (k < hi) ? V::ld(rowj + k) : V::zero();
         vx[u] = (k < hi) ? V::ld(vv + k) : V::zero();
@@ -74,7 +77,7 @@ __global__ void __launch_bounds__(QMCD_THREADS, 3) qmcd_ratio_kernel(const QmcdR
     if (gr == 0 && wid == 0) {
         double d = 0.0;
 #pragma unroll
-        for (int u = 0; u < QMCD_RATIO_NU; ++u) d = V::dot(rj[u], vx[u], d);
+        for (int u = 0; u < NU; ++u) d = V::dot(rj[u], vx[u], d);
         d = qmcd_warp_sum(d);
         if (lane == 0) pp[2 * K] = d;
         // stage the move's slot: W[m] <- B0[j,:], C[m] <- v (this slice)
@@ -82,28 +85,39 @@ __global__ void __launch_bounds__(QMCD_THREADS, 3) qmcd_ratio_kernel(const QmcdR
             double* Wm = P.W + ((size_t)b * K + m) * N;
             double* Cm = P.C + ((size_t)b * K + m) * N;
 #pragma unroll
-            for (int u = 0; u < QMCD_RATIO_NU; ++u) {
+            for (int u = 0; u < NU; ++u) {
                 const int k = lo + VEC * (lane + 32 * u);
                 if (k < hi) { V::st(Wm + k, rj[u]); V::st(Cm + k, vx[u]); }
             }
         }
     }
-    // queue rows i = 8 gr + wid, step 8 GR: all loads of a row pair (C[i], W[i]) are issued before the first FMA
-    for (int i = gr * QMCD_WARPS + wid; i < m; i += QMCD_WARPS * A.GR) {
-        const double* Ci = Cw + (size_t)i * N;
-        const double* Wi = Ww + (size_t)i * N;
-        typename V::T cv[QMCD_RATIO_NU], wv[QMCD_RATIO_NU];
+    // queue rows i = 8 gr + wid, step 8 GR, QMCD_RATIO_RB of them at a time: all loads of the row pairs (C[i], W[i]) are issued
+    // before the first FMA
+    const int istep = QMCD_WARPS * A.GR;
+    for (int i0 = gr * QMCD_WARPS + wid; i0 < m; i0 += istep * QMCD_RATIO_RB) {
+        typename V::T cv[QMCD_RATIO_RB][NU], wv[QMCD_RATIO_RB][NU];
 #pragma unroll
-        for (int u = 0; u < QMCD_RATIO_NU; ++u) {
-            const int k = lo + VEC * (lane + 32 * u);
-            cv[u] = (k < hi) ? V::ld(Ci + k) : V::zero();
-            wv[u] = (k < hi) ? V::ld(Wi + k) : V::zero();
+        for (int r = 0; r < QMCD_RATIO_RB; ++r) {
+            const int i = i0 + r * istep;
+            const double* Ci = Cw + (size_t)i * N;
+            const double* Wi = Ww + (size_t)i * N;
+#pragma unroll
+            for (int u = 0; u < NU; ++u) {
+                const int k = lo + VEC * (lane + 32 * u);
+                const bool ok = (i < m) && (k < hi);
+                cv[r][u] = ok ? V::ld(Ci + k) : V::zero();
+                wv[r][u] = ok ? V::ld(Wi + k) : V::zero();
+            }
         }
-        double p = 0.0, q = 0.0;
 #pragma unroll
-        for (int u = 0; u < QMCD_RATIO_NU; ++u) { p = V::dot(rj[u], cv[u], p); q = V::dot(wv[u], vx[u], q); }
-        p = qmcd_warp_sum(p); q = qmcd_warp_sum(q);
-        if (lane == 0) { pp[i] = p; pp[K + i] = q; }
+        for (int r = 0; r < QMCD_RATIO_RB; ++r) {
+            const int i = i0 + r * istep;
+            double p = 0.0, q = 0.0;
+#pragma unroll
+            for (int u = 0; u < NU; ++u) { p = V::dot(rj[u], cv[r][u], p); q = V::dot(wv[r][u], vx[u], q); }
+            p = qmcd_warp_sum(p); q = qmcd_warp_sum(q);
+            if (lane == 0 && i < m) { pp[i] = p; pp[K + i] = q; }
+        }
     }
     // ---- ticket: the last CTA of this walker finishes the job
     __threadfence();
