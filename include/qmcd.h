@@ -212,7 +212,8 @@ int qmcd_invert_static(qmcd_handle h, const double* A_dev, double* Ainv_dev, int
  *                   (the arithmetic of the per-move sweep, bit for bit).
  *   "flush_path"    0 auto, 1 CUDA-core, 2 DMMA.
  *   "lookahead"     qmcd_sweep: 0 auto = blocked look-ahead when the shape allows (N % (8 cluster) == 0, K <= 152; for
- *                   K > ~100 the K x K inverse then stays in global memory, which needs K even), 1 = per move.
+ *                   K > 64 the K x K inverse then stays in global memory, which needs K even; see "la_tma" for the
+ *                   super-block variant), 1 = per move.
  *   "slot_replace"  0 (default): accepting an electron that is already queued flushes first (reading G7); 1: it
  *                   replaces the column of its queue slot (M updated by a column-replacement Sherman-Morrison step),
  *                   nothing is flushed; qmcd_sweep then runs the per-move look-ahead.

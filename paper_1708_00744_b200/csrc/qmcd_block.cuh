@@ -1,4 +1,6 @@
-// qmcd_block.cuh -- blocked look-ahead for qmcd_sweep (pre-staged proposals).
+// qmcd_block.cuh -- blocked look-ahead for qmcd_sweep (pre-staged proposals): the per-move chain of a block of 16
+// proposals (qmcd_blk_chain, shared with the super-blocks of qmcd_superblock.cuh, the default path) and the sweep loop
+// in 16-proposal blocks with LDG / cp.async strips (qmcd_sweep_blocked: shapes the super-block ring does not take).
 //
 // Inside one window (between two flushes) the stale inverse B0 is fixed, so every
 // quantity the look-ahead of Eq. 3 needs for the next L

@@ -603,7 +603,7 @@ def test_autotune_K_picks_a_tensor_bound_delay(qmcd):
 
 
 def test_randomized_shapes_seeds_modes_and_launch_splits(qmcd):
-    """A short randomized soak (fixed generator): shapes with and without helper clusters, random
+    """A short randomized soak (fixed generator): shapes with and without the pool of flush workers, random
     seeds, acceptance 0.2 ... 0.99 or the Metropolis rule, the run cut into 1 ... 4 sweep launches at
     random places -- every run against the oracle's delayed path.  (A 150 s version of this loop,
     434 runs, was green with a worst deviation of 1.2e-14.)"""
@@ -883,7 +883,7 @@ def _windows_with_accepts(acc, K):
     (128, 16, 3, 1, None, 0.5, 0, None),        # blocked look-ahead, one block per window
     (128, 16, 3, 2, None, 0.5, 1, None),        # per-move look-ahead
     (256, 40, 2, 4, None, 0.5, 0, [37, 301]),   # windows of 16 + 16 + 8 proposals, launches cut mid-window
-    (512, 32, 3, 4, 2, 0.99, 0, None),          # helper clusters share the flushes
+    (512, 32, 3, 4, 2, 0.99, 0, None),          # the pool shares the flushes
     (512, 64, 2, 4, None, 0.3, 0, [5]),         # DMMA flush of low, varying rank
     (96, 7, 2, 1, None, 0.1, 0, None),          # windows with no accepted move at all
     (64, 1, 2, 1, None, 0.5, 0, None),          # K = 1
@@ -1072,7 +1072,7 @@ def test_invert_c4_full_size_residual_and_lapack(qmcd):
 @pytest.mark.parametrize("mode", ["bern0.5", "metropolis"])
 def test_c1_full_size_lockstep_default_launch_vs_oracle_path3(qmcd, mode):
     """Lock-step at BASELINE configs[1]'s full size in the library's default launch configuration
-    (helper clusters, blocked look-ahead, kernel entry qmcd_kernel_sweep_ls) against the oracle's
+    (pool, look-ahead in super-blocks, kernel entry qmcd_kernel_sweep_ls) against the oracle's
     literal path 3, every walker, every ratio."""
     wl = inputs.make_config("c1")
     K = 32
