@@ -303,7 +303,10 @@ __device__ int qmcd_sweep_sb(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_g
         // (at the acceptance rate seen so far in this launch: a queue with room for 32 takes 64 proposals at 50 %; moves
         // beyond what the queue takes are looked at again by the next super-block)
         int nb = K - m;
-        if (n_acc < n_prop) nb = (int)min((long long)64, ((long long)nb * n_prop + n_acc - 1) / max(n_acc, 1));
+        if (n_acc < n_prop) {                          // (nothing accepted yet: as long as allowed; never shorter than the room itself)
+            const long long want = (n_acc > 0) ? ((long long)nb * n_prop + n_acc - 1) / n_acc : 64;
+            nb = (int)min((long long)64, max((long long)nb, want));
+        }
         nb = min(64, (nb + QMCD_TB - 1) & ~(QMCD_TB - 1));
         nb = min(nb, min(A.n_moves - t, N - j0));
         if (LS) nb = min(nb, K - pw);

@@ -328,6 +328,31 @@ def test_superblock_lookahead_matches_oracle(qmcd, N, K, batch, cluster, mode, j
         assert np.all(g["pending"] == 0)
 
 
+@pytest.mark.timeout(120, method="thread")
+@pytest.mark.parametrize("K,lockstep", [(1, 0), (1, 1), (8, 0)])
+def test_launch_starting_with_a_rejection_and_room_for_one_move(qmcd, K, lockstep):
+    """Regression, found by a randomized soak: the super-block length is the room left in the queue over the acceptance rate
+    seen so far in the launch; with room for ONE move and the launch's first proposal rejected it came out as 0 proposals and
+    the sweep never advanced.  K = 1, and K = 8 with 7 moves carried over from the launch before."""
+    N, batch = 128, 2
+    wl = inputs.make_workload(batch, N, n_moves=60, seed=5)
+    mask = np.ones((60, batch), dtype=np.uint8)
+    first = 0 if K == 1 else K - 1                       # the launch that starts at `first` begins with rejections
+    mask[first:first + 3] = 0
+    mask[20:25, 1] = 0
+    Bo = wl.Ainv.copy()
+    if lockstep:
+        Ao = wl.A.copy()
+        Ro, acco, _, _ = oracle.run_lockstep(Ao, Bo, K, wl.proposals, mask=mask)
+    else:
+        Ro, acco, _ = oracle.run(2, Bo, K, wl.proposals, mask=mask)
+    g = gpu_sweep(qmcd, wl, K, mask=mask, cluster=1, lockstep=lockstep or None, split=[first] if first else None)
+    assert g["status"] == 0 and g["la_tma"] == 1
+    assert np.array_equal(g["acc"], acco)
+    assert _rel(g["R"], Ro) <= RTOL_RATIO
+    assert np.max(np.abs(g["B"] - Bo)) <= 1e-10
+
+
 @pytest.mark.parametrize("N,K,batch,cluster,p", [
     (128, 1, 3, 1, 0.9),       # K = 1: the classic Sherman-Morrison update (Eqs. 1-2)
     (192, 1, 2, 2, 1.0),       # N a multiple of 64 but not of 128
