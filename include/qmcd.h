@@ -21,7 +21,8 @@
  *   - All `*_dev` pointers are DEVICE pointers, fp64 unless stated, owned by the
  *     caller (e.g. torch tensors).  The library never allocates device memory
  *     (one exception, outside the method: qmcd_probe_fp64 allocates and frees an
- *     8-byte scratch).
+ *     8-byte scratch; the library image itself holds a 1 MiB static device array,
+ *     the scratch of qmcd_invert_static).
  *   - Every call only ENQUEUES work on the handle's CUDA stream and returns; no
  *     call synchronises except qmcd_status, qmcd_destroy and qmcd_sweep_host.
  *   - Return value: QMCD_OK (0) or a negative QMCD_E* code.  Argument and state
