@@ -139,7 +139,8 @@ int qmcd_worker_stats(qmcd_handle h, long long* stats_dev, long long* flush_rank
  * flushed before its block instead of at its accept) with the default blocked
  * look-ahead, which needs proposals_dev 16-byte aligned; the blocked sweep also
  * flushes a walker's queue up to min(8, K/4) - 1 moves before it is full when the
- * next block would not fit -- neutral).  Move t proposes electron
+ * next block would not fit, and may cut a launch's first window short (option "stagger")
+ * -- neutral).  Move t proposes electron
  * (j_begin + t) mod N with new column proposals_dev[t][b][:].  Exactly one of
  * mask_dev ([n_moves][batch] uint8) / uniforms_dev ([n_moves][batch] fp64,
  * Metropolis u < min(1,R^2)) is non-NULL.  Outputs R_out_dev [n_moves][batch]
@@ -207,6 +208,10 @@ int qmcd_invert_static(qmcd_handle h, const double* A_dev, double* Ainv_dev, int
  *                   operands stream through a TMA ring once (K <= 128, K even beyond 64, N >= 128, N % 64 == 0, column
  *                   slices of whole 16- / 8-column chunks); 0 = blocks of 16 proposals with LDG / cp.async strips (the
  *                   path of every other shape).
+ *   "stagger"       1: the first window of walker b in a qmcd_sweep launch that starts with empty queues is cut short to
+ *                   K (b mod 8 + 1) / 8 accepted moves (flushing early is neutral), so that walkers with
+ *                   identical timing do not post their flush jobs in the same instant, window after window.  Default: on for
+ *                   2 ... 8 walkers with N >= 2048 (c4), off otherwise; ignored in lock-step.
  *   "invert_blocked" 1 (default): qmcd_invert / qmcd_invert_static run the blocked Gauss-Jordan kernel when the batch is
  *                   co-resident; 0 = the unblocked kernel (one pass over the matrix per pivot).
  *   "ratio_kernel"  1 (default): qmcd_ratio runs the dedicated bandwidth kernel; 0 = the cluster kernel's look-ahead

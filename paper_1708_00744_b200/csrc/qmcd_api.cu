@@ -277,13 +277,13 @@ static int launch(qmcd_ctx* h, QmcdArgs& a, bool with_pool) {
 static int default_S(int N, int K, int batch, int cap) {
     // measured with the super-block look-ahead (K = 64, 99 % acceptance, fraction of the DMMA peak for S = 1/2/4/8/16):
     // 1 walker N = 2048: .058/.065/.070/.072/.073, N = 8192: .26/.29/.32/.34/.34; 4 walkers N = 2048: .22/.24/.26/.27;
-    // 16 walkers N = 1024: .38/.39/.41, N = 512 (c1, K = 32): .18/.19/.20; 8 walkers N = 4096 (c4): .84/.66/.70 -- there a
-    // tile takes longer than a window's look-ahead and larger clusters lock the walkers' flushes in step (pool idle
-    // during the look-aheads); 32 and 64 walkers (c3, c2): the pool hides the look-ahead, S = 1
+    // 16 walkers N = 1024: .38/.39/.41, N = 512 (c1, K = 32): .18/.19/.20, N = 2048: .84/.80; 8 walkers N = 4096 (c4) with
+    // staggered windows: .87/.86/.72 at 99 % acceptance but .57/.69/.66 at 50 % and .36/.40/.40 at K = 16 -- the look-ahead of a
+    // window is long against a tile there, so clusters of 2; 32 and 64 walkers (c3, c2): the pool hides the look-ahead, S = 1
     int s = 1;
     if (K <= 64) {
         if (batch <= 4) s = 8; else if (batch <= 16) s = 4;
-        if (batch > 4 && (long long)N * batch >= 32768) s = 1;
+        if (batch > 4 && (long long)N * batch >= 32768) s = (batch <= 8) ? 2 : 1;    // (c4: 2, with staggered windows, see qmcd_create; 16 x 2048: 1)
     } else {                                       // the 16-proposal blocks of qmcd_block.cuh / the per-move look-ahead
         if (batch <= 4) s = 8; else if (batch <= 16) s = 2;
         if ((long long)N * batch <= 16384) s *= 2;
@@ -329,6 +329,10 @@ extern "C" int qmcd_create(qmcd_handle* out, int N, int K, int batch,
     P.ticket = (unsigned long long*)(ws + L.ticket); P.jdesc = (unsigned long long*)(ws + L.jdesc);
     P.fin = (unsigned*)(ws + L.fin); P.ctrl = (unsigned*)(ws + L.ctrl);
     P.chain_regs = 1; P.pool = 0;
+    // staggered first windows (qmcd_superblock.cuh): few walkers with long tiles lock their flushes in step otherwise (c4, clusters of
+    // 2: 0.64 -> 0.85 of the DMMA peak; clusters of 1: 0.83 -> 0.86); with many walkers or short tiles the extra low-rank flush per
+    // walker and launch only costs (c1 -3 %, c2 -2 %, c3 and 16 x 2048: 0)
+    P.stagger = (batch >= 2 && batch <= 8 && N >= 2048) ? 1 : 0;
     P.flush_path = 0; P.use_tma = 0; P.ldMg = qmcd_ldMg_host(K);
     h->tma_opt = 1; h->la_opt = 1; h->la_fit = false; h->ratio_opt = 1; h->invb_opt = 1;
     h->rpart = (double*)(ws + L.rpart); h->rcnt = (unsigned*)(ws + L.rcnt);
@@ -822,6 +826,11 @@ extern "C" int qmcd_set_option(qmcd_handle h, const char* key, int value) {
         refresh_use_tma(h);
         return QMCD_OK;
     }
+    if (!strcmp(key, "stagger")) {                 // 0: every window takes K moves (walkers that start together flush together)
+        if (value < 0 || value > 1) return QMCD_EINVAL;
+        h->P.stagger = value;
+        return QMCD_OK;
+    }
     if (!strcmp(key, "invert_blocked")) {          // 0: qmcd_invert runs the unblocked kernel (one pass over the matrix per pivot)
         if (value < 0 || value > 1) return QMCD_EINVAL;
         h->invb_opt = value;
@@ -885,6 +894,7 @@ extern "C" int qmcd_get_option(qmcd_handle h, const char* key) {
     if (!strcmp(key, "tma")) return h->P.use_tma;
     if (!strcmp(key, "la_tma")) return h->P.la_tma;
     if (!strcmp(key, "invert_blocked")) return h->invb_opt;
+    if (!strcmp(key, "stagger")) return h->P.stagger;
     if (!strcmp(key, "ratio_kernel")) return h->ratio_opt;
     if (!strcmp(key, "flush_path")) return h->P.flush_path;
     if (!strcmp(key, "lookahead")) return h->lookahead;

@@ -24,6 +24,7 @@ struct QmcdDev {
     int pool;                 // pool CTAs (flush workers serving every walker) in THIS launch, set per launch
     int tile_rows;            // rows of B per flush tile (64 or 128), host choice
     int use_tma;              // host: K <= 64 flush tiles through qmcd_flush_tma.cuh (TMA-fed, 128-row tiles)
+    int stagger;              // option: the first window of walker b in a launch is cut short so that the walkers' flushes do not coincide (qmcd_superblock.cuh)
     int la_tma;               // host: qmcd_sweep's blocked look-ahead streams its operands through a TMA ring (qmcd_block.cuh)
     int ldMg;                 // row stride of M in GLOBAL memory: 64 when K <= 64 (a 64 x 64 tile, TMA box), else K
     // ---- flush jobs (leader cluster of walker b -> every worker: its own CTAs and the pool)

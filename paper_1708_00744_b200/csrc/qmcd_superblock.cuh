@@ -295,6 +295,15 @@ __device__ int qmcd_sweep_sb(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_g
 #define QMCD_TICK(acc_) do { if (prof) { const long long c1_ = clock64(); (acc_) += c1_ - c0; c0 = c1_; } } while (0)
     const int thresh = max(1, min(QMCD_TB / 2, K / 4));
     int t = 0, n_prop = 0, n_acc = 0;                                    // proposals decided / accepted so far in this launch
+    // Stagger: walkers that start a launch together with empty queues would post their flush jobs in the same instant, window
+    // after window (their timing is identical), and the pool would idle during the look-aheads in between.  The FIRST window of
+    // walker b is therefore cut short to K (b mod G + 1) / G moves -- flushing early is neutral -- which spreads the
+    // walkers' phases over the cycle; the later windows take K moves.  Not in lock-step (the windows are the proposals').
+    int kcap = K;
+    if (!LS && P.stagger && m == 0 && A.n_moves >= 2 * K) {
+        const int G = min(P.batch, 8);
+        kcap = max(1, K * ((w.b % G) + 1) / G);
+    }
     int pw = LS ? (int)__ldcg(P.counters + (size_t)w.b * 8 + 7) : 0;     // lock-step: proposals in the current window
     while (t < A.n_moves) {
         const int j0 = (A.j_begin + t) % N;
@@ -302,7 +311,7 @@ __device__ int qmcd_sweep_sb(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_g
         // wrap-around of the electron index (the rows of B0 are one box) or, lock-step, the window's end
         // (at the acceptance rate seen so far in this launch: a queue with room for 32 takes 64 proposals at 50 %; moves
         // beyond what the queue takes are looked at again by the next super-block)
-        int nb = K - m;
+        int nb = kcap - m;
         if (n_acc < n_prop) {                          // (nothing accepted yet: as long as allowed; never shorter than the room itself)
             const long long want = (n_acc > 0) ? ((long long)nb * n_prop + n_acc - 1) / n_acc : 64;
             nb = (int)min((long long)64, max((long long)nb, want));
@@ -328,7 +337,7 @@ __device__ int qmcd_sweep_sb(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_g
                     QMCD_TICK(cy_la);
                     qmcd_flush_phase<MS>(P, s, cl, w, m);
                     QMCD_TICK(cy_fl);
-                    m = 0; pw = 0;
+                    m = 0; pw = 0; kcap = K;
                     continue;
                 }
             }
@@ -351,7 +360,7 @@ __device__ int qmcd_sweep_sb(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_g
 
         int o = 0, na_sb = 0;
         while (o < nb) {
-            const int L = min(min(QMCD_TB, nb - o), K - m);
+            const int L = min(min(QMCD_TB, nb - o), kcap - m);
             if (tid < L) {
                 const size_t tb = (size_t)(t + o + tid) * P.batch + w.b;
                 x.ub[tid] = A.uniforms ? A.uniforms[tb] : (A.mask[tb] ? 1.0 : 0.0);
@@ -391,7 +400,7 @@ __device__ int qmcd_sweep_sb(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_g
             n_prop += L; n_acc += na;
             QMCD_TICK(cy_chain);
             if (LS) { pw += L; if (pw >= K) break; }
-            else if (K - m < thresh) break;
+            else if (kcap - m < thresh) break;
         }
         // ---- append the super-block's accepted moves to the queue: C[slot] = v, W[slot] = B0[j,:]
         if (na_sb > 0) qmcd_sb_append(A, s, sb, w, t, j0, m0sb, na_sb);
@@ -404,7 +413,7 @@ __device__ int qmcd_sweep_sb(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_g
                 if (m > 0) { qmcd_flush_phase<MS>(P, s, cl, w, m); m = 0; QMCD_TICK(cy_fl); }
                 pw = 0;
             }
-        } else if (K - m < thresh) { qmcd_flush_phase<MS>(P, s, cl, w, m); m = 0; QMCD_TICK(cy_fl); }
+        } else if (kcap - m < thresh) { qmcd_flush_phase<MS>(P, s, cl, w, m); m = 0; kcap = K; QMCD_TICK(cy_fl); }
     }
     if (LS && w.r == 0 && tid == 0) P.counters[(size_t)w.b * 8 + 7] = pw;
     if (prof) {
