@@ -413,7 +413,10 @@ __device__ int qmcd_sweep_sb(const QmcdArgs& A, const QmcdSmem& s, cg::cluster_g
                 if (m > 0) { qmcd_flush_phase<MS>(P, s, cl, w, m); m = 0; QMCD_TICK(cy_fl); }
                 pw = 0;
             }
-        } else if (kcap - m < thresh) { qmcd_flush_phase<MS>(P, s, cl, w, m); m = 0; kcap = K; QMCD_TICK(cy_fl); }
+        } else if (kcap - m < thresh) {                // (m == 0: a shortened first window in which nothing was accepted)
+            if (m > 0) { qmcd_flush_phase<MS>(P, s, cl, w, m); m = 0; QMCD_TICK(cy_fl); }
+            kcap = K;
+        }
     }
     if (LS && w.r == 0 && tid == 0) P.counters[(size_t)w.b * 8 + 7] = pw;
     if (prof) {

@@ -330,7 +330,7 @@ def test_superblock_lookahead_matches_oracle(qmcd, N, K, batch, cluster, mode, j
         assert np.all(g["pending"] == 0)
 
 
-@pytest.mark.parametrize("N,K,batch,cluster,p", [(256, 64, 5, 1, 0.99), (512, 32, 8, 2, 0.6), (256, 8, 3, 1, 1.0)])
+@pytest.mark.parametrize("N,K,batch,cluster,p", [(256, 64, 5, 1, 0.99), (512, 32, 8, 2, 0.6), (256, 8, 3, 1, 1.0), (256, 32, 8, 1, 0.05)])
 def test_staggered_first_windows_are_neutral(qmcd, N, K, batch, cluster, p):
     """Option "stagger" (default for 2 ... 8 walkers with N >= 2048, forced here): the first window of walker b in a launch
     is cut short to K (b mod 8 + 1) / 8 moves so that the walkers' flushes do not coincide -- the same ratios, decisions and
