@@ -35,7 +35,7 @@ if ROOT not in sys.path:
 METRIC = "accepted electron moves/s (fp64, batched walkers)"
 UNIT = "moves/s"
 DEFAULT_CONFIG, DEFAULT_K, DEFAULT_MODE = "c3", 64, "bern0.99"
-NCU_TRAFFIC_BYTES_DEFAULT = 232.0e9       # profiles/r2_ncu_c3_sweep.md: 158.9 GB read + 73.1 GB written per sweep launch
+NCU_TRAFFIC_BYTES_DEFAULT = 232.9e9       # profiles/r2_ncu_c3_sweep.md: dram__bytes_read.sum + dram__bytes_write.sum per sweep launch
 
 
 def parse_args():
